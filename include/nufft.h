@@ -1,0 +1,144 @@
+/* nufft.h -- C ABI of the B200-native NUFFT hot path (arxiv 1710.03197, PyNUFFT).
+ *
+ * What the library computes, stage by stage (citations are PAPER.md lines; readings R1..R20 are listed in
+ * DESIGN.md "Readings of the paper"):
+ *
+ *   forward      A   = V F S         PAPER.md:48-52, eq.(1) :50     scaling :54-56, zero-pad + FFT :58-68,
+ *                                                                    interpolation :72-74
+ *   adjoint      A^H = S^H F^H V^H   PAPER.md:78-84, eq.(2) :82     gridding :76, IFFT + crop :70
+ *   selfadjoint  A^H A               PAPER.md:86-98, eq.(5) :96     applied back to back (R8)
+ *   multi-coil   A_multi x = [A(c_i.x)]_i,  A_multi^H y = sum_i conj(c_i).A^H y_i   PAPER.md:251-258, eqs.(34)-(35)
+ *   batch mode   several images per call
+ *   CG           linear CG on A^H A x = A^H y                       PAPER.md:96, 124-143 (R12)
+ *   L1TV-OLS     split Bregman, eqs.(13)-(22)                       PAPER.md:158-198 (R13-R18)
+ *
+ * Conventions (all binding):
+ *   - d in {2,3}.  Image x is C-order [batch][N0][N1]([N2]) complex64; image index n_a sits at position
+ *     n_a - N_a/2 (R4).  Samples y are [batch][M] complex64 in the caller's sample order.  om is [M][d] float64,
+ *     radians per image sample, axis a of om pairs with image axis a; values outside [-pi,pi) are wrapped.
+ *   - forward sign e^{-i om.(n - N/2)}; adjoint is the exact conjugate transpose (no 1/prod(K) factor, R5).
+ *   - interpolator: Kaiser-Bessel, width J = 6 grid cells, beta = pi sqrt((J/sigma)^2 (sigma-1/2)^2 - 0.8),
+ *     sigma = K/N = 2, scaling factors 1/Phi (R1-R3); periodic grid (R7).
+ *   - complex64 = two IEEE float32 (re, im), i.e. CUDA float2; declared here as nufft_c64 so that this header
+ *     needs no CUDA include.  `stream` arguments are a cudaStream_t passed as void* (NULL = default stream).
+ *   - POINTER KINDS.  "host" = ordinary host memory read during the call.  "device" = CUDA device memory,
+ *     owned by the caller, 8-byte aligned, valid until the stream work enqueued by the call has finished.
+ *     The library never allocates, frees or retains caller arrays, except coil maps (borrowed, see below).
+ *   - every call returns 0 (NUFFT_OK) or a negative nufft_status; nothing is printed, nothing throws or aborts.
+ *   - transform calls are asynchronous: they enqueue kernels on `stream` and return.  A plan owns one workspace:
+ *     use one stream at a time per plan.  Distinct plans are independent.
+ *   - outputs are overwritten, never accumulated into.  In-place (x_in == x_out) is allowed for selfadjoint.
+ *   - supported: d in {2,3}; Jd[a] == 6; Kd[a] == 2*Nd[a]; Kd[a] in {32,64,128,256,512,1024};
+ *     1 <= batch <= max_batch.  Anything else -> NUFFT_EINVAL (there is no slow path and no CPU fallback).
+ */
+#ifndef NUFFT_B200_H
+#define NUFFT_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { float re, im; } nufft_c64;          /* layout-identical to CUDA float2 */
+typedef struct nufft_plan_s *nufft_plan_t;
+
+typedef enum {
+    NUFFT_OK      =  0,
+    NUFFT_EINVAL  = -1,   /* bad d / sizes / Jd / batch / null pointer / unsupported option                 */
+    NUFFT_ENOMEM  = -2,   /* host or device allocation failed                                             */
+    NUFFT_ECUDA   = -3,   /* a CUDA runtime call failed; nufft_last_cuda_error() gives the cudaError_t    */
+    NUFFT_ERANGE  = -4,   /* om contains a non-finite value                                               */
+    NUFFT_ESTATE  = -5    /* call needs something not set (e.g. coil maps)                                */
+} nufft_status;
+
+/* Options.  Zero-initialise or call nufft_default_opts first. */
+typedef struct {
+    int coef_mode;      /* 0 = interpolation weights recomputed on the fly from a piecewise polynomial fit of the
+                               Kaiser-Bessel kernel (12 + 4 B per sample of plan data in 2-D);
+                           1 = weights read from a per-sample separable table (4 + 4 d J bytes per sample)       */
+    int adjoint_mode;   /* 0 = V^H by tile-sorted shared-memory accumulation, one vector-atomic flush per tile
+                               (summation order across tiles free: reproducible to rounding only);
+                           1 = deterministic: tiles flushed to private slabs and summed in fixed order
+                               (bit-reproducible run to run)                                                      */
+    int interp_mode;    /* 0 = V gathers straight from the grid through L1/L2; 1 = tile staged in shared memory */
+    int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
+    int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
+    int use_graphs;     /* 1 = capture forward/adjoint/selfadjoint into CUDA graphs on first use (default 0)     */
+} nufft_opts;
+
+int nufft_default_opts(nufft_opts *o);
+
+/* Plan creation (everything derived from the trajectory is computed once and offloaded
+ * "before iterative algorithms begin").  Nd, Kd: int64[d] host; Jd: int[d] host; om: float64 [M][d] row-major,
+ * host, copied (the caller may free it on return).  max_batch >= 1 sizes the workspace grid(s):
+ * max_batch * prod(Kd) * 8 bytes of device memory.  opts == NULL selects the defaults.
+ * Synchronous (host work + uploads on the default stream).  On failure *out is NULL. */
+int nufft_plan(int d, const int64_t *Nd, const int64_t *Kd, const int *Jd,
+               int64_t M, const double *om, int max_batch, const nufft_opts *opts, nufft_plan_t *out);
+
+/* y[b][m] = (A x_b)[m], b < batch.   x: device [batch][prod Nd];  y: device [batch][M].   eq.(1) */
+int nufft_forward(nufft_plan_t p, int batch, const nufft_c64 *x, nufft_c64 *y, void *stream);
+
+/* x[b] = A^H y_b.   y: device [batch][M];  x: device [batch][prod Nd].   eq.(2) */
+int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64 *y, nufft_c64 *x, void *stream);
+
+/* x_out[b] = A^H A x_in[b], the intermediate samples stay in the plan's workspace.   eq.(5), R8 */
+int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
+
+/* The four stages on their own (used by the per-stage parity tests and the per-stage timings).
+ * grid: device [batch][prod Kd] complex64 in natural FFT order (k = 0 is index 0), caller-owned.
+ *   scale_fft:  grid = F S x          (a1+a2)      fft_scale: x = S^H F^H grid   (a5+a6; grid is DESTROYED)
+ *   interp:     y = V grid            (a3)         gridding:  grid = V^H y       (a4; grid fully overwritten) */
+int nufft_stage_scale_fft(nufft_plan_t p, int batch, const nufft_c64 *x, nufft_c64 *grid, void *stream);
+int nufft_stage_interp   (nufft_plan_t p, int batch, const nufft_c64 *grid, nufft_c64 *y, void *stream);
+int nufft_stage_gridding (nufft_plan_t p, int batch, const nufft_c64 *y, nufft_c64 *grid, void *stream);
+int nufft_stage_fft_scale(nufft_plan_t p, int batch, nufft_c64 *grid, nufft_c64 *x, void *stream);
+
+/* Multi-coil operator, eqs.(34)-(35) PAPER.md:251-258.  c: device [ncoil][prod Nd], BORROWED: it must stay valid
+ * and unchanged until the plan is destroyed or other maps are set.  ncoil <= max_batch.  ncoil = 0 clears.
+ *   forward_coils:      y[i] = A (c_i . x)                     x: [prod Nd]   y: [ncoil][M]
+ *   adjoint_coils:      x    = sum_i conj(c_i) . A^H y[i]
+ *   selfadjoint_coils:  x_out = sum_i conj(c_i) . A^H A (c_i . x_in)                                            */
+int nufft_set_coils(nufft_plan_t p, int ncoil, const nufft_c64 *c);
+int nufft_forward_coils(nufft_plan_t p, const nufft_c64 *x, nufft_c64 *y, void *stream);
+int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64 *y, nufft_c64 *x, void *stream);
+int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
+
+/* Linear conjugate gradient on the normal equation A^H A x = A^H y, x0 = 0, exactly niter iterations, no
+ * preconditioner (eq.(5), :124-143; R12).  If coil maps are set and use_coils != 0 the multi-coil
+ * operator is used and y is [ncoil][M]; else y is [M].  x: device [prod Nd] (output).  Scalars (alpha, beta,
+ * inner products) are float64 on the device; nothing is read back during the iteration.
+ * resnorm_host: NULL, or host double[niter+1] receiving ||r_k||_2, k = 0..niter (forces a stream sync at the end). */
+int nufft_solve_cg(nufft_plan_t p, int use_coils, const nufft_c64 *y, nufft_c64 *x, int niter,
+                   double *resnorm_host, void *stream);
+
+/* Split-Bregman L1TV-OLS, eqs.(13)-(22) PAPER.md:158-198 with readings R13-R18 (2-D images only):
+ *   scale the problem by 1/max|A^H y| (R17); repeat n_outer times { repeat n_inner times { rhs = mu A^H y^k +
+ *   lam sum_a grad_a^T(d_a - b_a) (16);  x <- n_cg CG steps on (mu A^H A + lam sum_a grad_a^T grad_a) x = rhs warm
+ *   started (15),(17),R16;  d_a = shrink(grad_a x + b_a, 1/lam) (18)-(19);  b_a += grad_a x - d_a (20)-(21) }
+ *   A^H y^{k+1} = A^H y^k + A^H y - A^H A x (22) };  result scaled back.
+ * grad_a = periodic forward difference along image axis a (eq.(12), R15).
+ * y, x as in nufft_solve_cg.  Synchronises the stream once (to read max|A^H y|). */
+int nufft_solve_l1tv_ols(nufft_plan_t p, int use_coils, const nufft_c64 *y, nufft_c64 *x,
+                         double mu, double lam, int n_outer, int n_inner, int n_cg, void *stream);
+
+/* Plan facts.  Any pointer may be NULL.  bytes_plan = device bytes of per-sample plan data; bytes_work = device
+ * bytes of workspace (grids, sample buffers, solver vectors); n_tiles / n_work = V^H tiles and work items (after
+ * hot-tile splitting); max_tile_samples = the largest tile's sample count. */
+int nufft_plan_info(nufft_plan_t p, int64_t *bytes_plan, int64_t *bytes_work,
+                    int64_t *n_tiles, int64_t *n_work, int64_t *max_tile_samples);
+
+/* Number of kernel launches the library has enqueued for this plan since creation (bench.py's gpu_launches). */
+int64_t nufft_launch_count(nufft_plan_t p);
+
+int nufft_destroy(nufft_plan_t p);
+
+const char *nufft_strerror(int code);
+int nufft_last_cuda_error(void);         /* the cudaError_t of the last NUFFT_ECUDA on this thread, else 0 */
+const char *nufft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NUFFT_B200_H */

@@ -1,0 +1,678 @@
+// nufft.cu -- the C-ABI library of the B200-native NUFFT hot path (include/nufft.h): plan creation (host, float64),
+// kernel launches for A = V F S, A^H = S^H F^H V^H, A^H A, the multi-coil operator and the CG / L1TV-OLS drivers.
+// Product path: no CPU fallback, no cuFFT, nothing from oracle/.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/nufft.h"
+#include "common.cuh"
+#include "fft.cuh"
+#include "plan.hpp"
+#include "solver.cuh"
+#include "spread_interp.cuh"
+
+using namespace nufft;
+
+static thread_local int g_last_cuda_error = 0;
+
+#define CU_TRY(expr)                                        \
+    do {                                                    \
+        cudaError_t e__ = (expr);                           \
+        if (e__ != cudaSuccess) {                           \
+            g_last_cuda_error = (int)e__;                   \
+            (void)cudaGetLastError();                       \
+            return NUFFT_ECUDA;                             \
+        }                                                   \
+    } while (0)
+#define NU_TRY(expr)                 \
+    do {                             \
+        int r__ = (expr);            \
+        if (r__ != NUFFT_OK) return r__; \
+    } while (0)
+
+struct nufft_plan_s {
+    int d = 0;
+    int N[3] = {1, 1, 1}, K[3] = {1, 1, 1};
+    int64_t M = 0, nimg = 0, cells = 0;
+    int max_batch = 1;
+    nufft_opts opts{};
+    KernelPoly poly{};
+    double poly_err = 0.0;
+    // device plan data
+    float* d_scale[3] = {nullptr, nullptr, nullptr};
+    float2* d_tw[3] = {nullptr, nullptr, nullptr};
+    uint32_t* d_kpack = nullptr;
+    float* d_delta = nullptr;
+    int32_t* d_perm = nullptr;
+    // workspace
+    float2* d_grid = nullptr;       // [max_batch][cells]
+    float2* d_ywork = nullptr;      // [max_batch][M]     (selfadjoint intermediate)
+    float2* d_imgwork = nullptr;    // [max_batch][nimg]  (per-coil images of the multi-coil adjoint), lazy
+    float2* d_solver = nullptr;     // solver vectors, lazy
+    int64_t solver_vecs = 0;
+    CgScalars* d_scal = nullptr;
+    double* d_hist = nullptr;
+    int hist_cap = 0;
+    // coils (borrowed)
+    int ncoil = 0;
+    const float2* d_coils = nullptr;
+    // tiles
+    int tile[3] = {1, 1, 1}, ntile[3] = {1, 1, 1};
+    int64_t n_tiles = 0, n_work = 0, max_tile_samples = 0;
+    int64_t bytes_plan = 0, bytes_work = 0;
+    int64_t launches = 0;
+};
+
+// ------------------------------------------------------------------------------------------------------------
+// kernel configuration (dynamic shared memory opt-in), once per process
+// ------------------------------------------------------------------------------------------------------------
+template <int K> static size_t smem_rows() { return (size_t)Rad<K>::LC * FftGeom<K>::PITCH_C * sizeof(float2); }
+template <int K> static size_t smem_cols() { return (size_t)Rad<K>::TS * FftGeom<K>::SIZE_S * sizeof(float2); }
+
+template <int K> static cudaError_t configure_fft() {
+    cudaError_t e;
+    e = cudaFuncSetAttribute(fft_rows_fwd_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_rows_adj_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_cols_kernel<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_cols_kernel<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    return e;
+}
+
+static cudaError_t configure_all() {
+    cudaError_t e;
+    if ((e = configure_fft<32>()) != cudaSuccess) return e;
+    if ((e = configure_fft<64>()) != cudaSuccess) return e;
+    if ((e = configure_fft<128>()) != cudaSuccess) return e;
+    if ((e = configure_fft<256>()) != cudaSuccess) return e;
+    if ((e = configure_fft<512>()) != cudaSuccess) return e;
+    if ((e = configure_fft<1024>()) != cudaSuccess) return e;
+    return cudaSuccess;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// FFT pass launchers
+// ------------------------------------------------------------------------------------------------------------
+template <int K> static void launch_rows(bool adj, const RowPassParams& p, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::LC;
+    const int blocks = (p.nlines + Rad<K>::LC - 1) / Rad<K>::LC;
+    if (adj) fft_rows_adj_kernel<K><<<blocks, threads, smem_rows<K>(), st>>>(p);
+    else     fft_rows_fwd_kernel<K><<<blocks, threads, smem_rows<K>(), st>>>(p);
+}
+template <int K> static void launch_cols(bool adj, const ColPassParams& p, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
+    if (adj) fft_cols_kernel<K, true><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
+    else     fft_cols_kernel<K, false><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
+}
+static int tile_T(int K) {
+    switch (K) {
+        case 32: return Rad<32>::TS; case 64: return Rad<64>::TS; case 128: return Rad<128>::TS;
+        case 256: return Rad<256>::TS; case 512: return Rad<512>::TS; case 1024: return Rad<1024>::TS;
+    }
+    return 0;
+}
+static int dispatch_rows(int K, bool adj, const RowPassParams& p, cudaStream_t st) {
+    switch (K) {
+        case 32: launch_rows<32>(adj, p, st); break;
+        case 64: launch_rows<64>(adj, p, st); break;
+        case 128: launch_rows<128>(adj, p, st); break;
+        case 256: launch_rows<256>(adj, p, st); break;
+        case 512: launch_rows<512>(adj, p, st); break;
+        case 1024: launch_rows<1024>(adj, p, st); break;
+        default: return NUFFT_EINVAL;
+    }
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+static int dispatch_cols(int K, bool adj, const ColPassParams& p, cudaStream_t st) {
+    switch (K) {
+        case 32: launch_cols<32>(adj, p, st); break;
+        case 64: launch_cols<64>(adj, p, st); break;
+        case 128: launch_cols<128>(adj, p, st); break;
+        case 256: launch_cols<256>(adj, p, st); break;
+        case 512: launch_cols<512>(adj, p, st); break;
+        case 1024: launch_cols<1024>(adj, p, st); break;
+        default: return NUFFT_EINVAL;
+    }
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+
+static RowPassParams row_params(nufft_plan_t p, int batch, const float2* img_in, float2* img_out, float2* grid,
+                                const float2* coil, bool same_image) {
+    RowPassParams r{};
+    r.img_in = img_in; r.img_out = img_out; r.grid = grid; r.coil = coil;
+    const int d = p->d;
+    r.s_line = p->d_scale[d - 1];
+    r.tw = p->d_tw[d - 1];
+    if (d == 2) {
+        r.s_outer0 = p->d_scale[0]; r.s_outer1 = nullptr;
+        r.n_outer0 = p->N[0]; r.n_outer1 = 1; r.k_outer0 = p->K[0]; r.k_outer1 = 1;
+    } else {
+        r.s_outer0 = p->d_scale[0]; r.s_outer1 = p->d_scale[1];
+        r.n_outer0 = p->N[0]; r.n_outer1 = p->N[1]; r.k_outer0 = p->K[0]; r.k_outer1 = p->K[1];
+    }
+    r.nlines = batch * r.n_outer0 * r.n_outer1;
+    r.img_batch_stride_is_zero = same_image ? 1 : 0;
+    return r;
+}
+
+// a1 + a2: grid = F S x  (coil != nullptr: grid_b = F S (c_b . x))
+static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* grid, const float2* coil,
+                         bool same_image, cudaStream_t st) {
+    const int d = p->d;
+    RowPassParams r = row_params(p, batch, x, nullptr, grid, coil, same_image);
+    NU_TRY(dispatch_rows(p->K[d - 1], false, r, st));
+    p->launches++;
+    if (d == 2) {
+        ColPassParams c{};
+        c.grid = grid; c.tw = p->d_tw[0];
+        c.batch_stride = p->cells; c.outer_stride = 0; c.line_stride = p->K[1];
+        c.n_outer = 1; c.k_outer = 0; c.inner = p->K[1];
+        c.ngroups = batch * (c.inner / tile_T(p->K[0]));
+        NU_TRY(dispatch_cols(p->K[0], false, c, st));
+        p->launches++;
+    } else {
+        ColPassParams c{};
+        c.grid = grid; c.tw = p->d_tw[1];
+        c.batch_stride = p->cells; c.outer_stride = (int64_t)p->K[1] * p->K[2]; c.line_stride = p->K[2];
+        c.n_outer = p->N[0]; c.k_outer = p->K[0]; c.inner = p->K[2];
+        c.ngroups = batch * c.n_outer * (c.inner / tile_T(p->K[1]));
+        NU_TRY(dispatch_cols(p->K[1], false, c, st));
+        ColPassParams c0{};
+        c0.grid = grid; c0.tw = p->d_tw[0];
+        c0.batch_stride = p->cells; c0.outer_stride = 0; c0.line_stride = (int64_t)p->K[1] * p->K[2];
+        c0.n_outer = 1; c0.k_outer = 0; c0.inner = p->K[1] * p->K[2];
+        c0.ngroups = batch * (c0.inner / tile_T(p->K[0]));
+        NU_TRY(dispatch_cols(p->K[0], false, c0, st));
+        p->launches += 2;
+    }
+    return NUFFT_OK;
+}
+
+// a5 + a6: x = S^H F^H grid  (grid destroyed; coil != nullptr: x_b = conj(c_b) . S^H F^H grid_b)
+static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
+    const int d = p->d;
+    if (d == 2) {
+        ColPassParams c{};
+        c.grid = grid; c.tw = p->d_tw[0];
+        c.batch_stride = p->cells; c.outer_stride = 0; c.line_stride = p->K[1];
+        c.n_outer = 1; c.k_outer = 0; c.inner = p->K[1];
+        c.ngroups = batch * (c.inner / tile_T(p->K[0]));
+        NU_TRY(dispatch_cols(p->K[0], true, c, st));
+        p->launches++;
+    } else {
+        ColPassParams c0{};
+        c0.grid = grid; c0.tw = p->d_tw[0];
+        c0.batch_stride = p->cells; c0.outer_stride = 0; c0.line_stride = (int64_t)p->K[1] * p->K[2];
+        c0.n_outer = 1; c0.k_outer = 0; c0.inner = p->K[1] * p->K[2];
+        c0.ngroups = batch * (c0.inner / tile_T(p->K[0]));
+        NU_TRY(dispatch_cols(p->K[0], true, c0, st));
+        ColPassParams c{};
+        c.grid = grid; c.tw = p->d_tw[1];
+        c.batch_stride = p->cells; c.outer_stride = (int64_t)p->K[1] * p->K[2]; c.line_stride = p->K[2];
+        c.n_outer = p->N[0]; c.k_outer = p->K[0]; c.inner = p->K[2];
+        c.ngroups = batch * c.n_outer * (c.inner / tile_T(p->K[1]));
+        NU_TRY(dispatch_cols(p->K[1], true, c, st));
+        p->launches += 2;
+    }
+    RowPassParams r = row_params(p, batch, nullptr, x, grid, coil, false);
+    NU_TRY(dispatch_rows(p->K[d - 1], true, r, st));
+    p->launches++;
+    return NUFFT_OK;
+}
+
+static GridGeom grid_geom(nufft_plan_t p) {
+    GridGeom g{};
+    g.K[0] = p->K[0]; g.K[1] = p->K[1]; g.K[2] = p->K[2];
+    g.cells = p->cells; g.M = p->M;
+    return g;
+}
+static SampleData sample_data(nufft_plan_t p) {
+    SampleData s{};
+    s.kpack = p->d_kpack; s.delta = p->d_delta; s.perm = p->d_perm;
+    return s;
+}
+
+// a3: y = V grid
+static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, cudaStream_t st) {
+    if (p->M == 0) return NUFFT_OK;
+    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
+    if (p->d == 2) interp_direct_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
+    else           interp_direct_kernel<3><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+
+// a4: grid = V^H y
+static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid, cudaStream_t st) {
+    CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st));
+    if (p->M == 0) return NUFFT_OK;
+    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
+    if (p->d == 2) gridding_atomic_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), y, grid, p->poly);
+    else           gridding_atomic_kernel<3><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), y, grid, p->poly);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// plan
+// ------------------------------------------------------------------------------------------------------------
+static bool supported_K(int64_t K) { return K == 32 || K == 64 || K == 128 || K == 256 || K == 512 || K == 1024; }
+
+template <class T> static int dev_upload(T** dptr, const std::vector<T>& h, int64_t* bytes) {
+    *dptr = nullptr;
+    if (h.empty()) return NUFFT_OK;
+    cudaError_t e = cudaMalloc((void**)dptr, h.size() * sizeof(T));
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? NUFFT_ENOMEM : NUFFT_ECUDA; }
+    CU_TRY(cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    if (bytes) *bytes += (int64_t)(h.size() * sizeof(T));
+    return NUFFT_OK;
+}
+static int dev_alloc(void** dptr, size_t bytes, int64_t* acct) {
+    *dptr = nullptr;
+    if (bytes == 0) return NUFFT_OK;
+    cudaError_t e = cudaMalloc(dptr, bytes);
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? NUFFT_ENOMEM : NUFFT_ECUDA; }
+    if (acct) *acct += (int64_t)bytes;
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_default_opts(nufft_opts* o) {
+    if (!o) return NUFFT_EINVAL;
+    std::memset(o, 0, sizeof(*o));
+    return NUFFT_OK;
+}
+
+static int plan_build(nufft_plan_t p, const double* om) {
+    const int d = p->d;
+    const double J = (double)kJ;
+    // kernel polynomial, scaling vectors, twiddles (float64 on the host, rounded once)
+    p->poly = host::fit_kernel_poly(J, 2.0, &p->poly_err);
+    for (int a = 0; a < d; ++a) {
+        NU_TRY(dev_upload(&p->d_scale[a], host::scaling_vector(p->N[a], p->K[a], J), &p->bytes_plan));
+        NU_TRY(dev_upload(&p->d_tw[a], host::twiddle_table(p->K[a]), &p->bytes_plan));
+    }
+    // tiles
+    const int def2[3] = {16, 32, 1}, def3[3] = {8, 8, 8};
+    for (int a = 0; a < 3; ++a) {
+        int t = (a < d) ? p->opts.tile[a] : 1;
+        if (a < d && t <= 0) t = (d == 2) ? def2[a] : def3[a];
+        if (a < d && (t > p->K[a] || (p->K[a] % t) != 0)) return NUFFT_EINVAL;
+        p->tile[a] = t;
+        p->ntile[a] = (a < d) ? p->K[a] / t : 1;
+    }
+    p->n_tiles = (int64_t)p->ntile[0] * p->ntile[1] * p->ntile[2];
+    // per-sample split (float64) and tile id
+    const int64_t M = p->M;
+    std::vector<uint32_t> kpack(M);
+    std::vector<float> delta((size_t)d * M);
+    std::vector<int32_t> tid(M);
+    for (int64_t m = 0; m < M; ++m) {
+        uint32_t kp = 0;
+        int64_t t = 0;
+        for (int a = 0; a < d; ++a) {
+            const double w = om[m * d + a];
+            if (!std::isfinite(w)) return NUFFT_ERANGE;
+            float df;
+            const int k0 = host::split_coordinate(w, p->K[a], J, &df);
+            kp |= (uint32_t)k0 << (10 * a);
+            delta[(size_t)a * M + m] = df;
+            t = t * p->ntile[a] + k0 / p->tile[a];
+        }
+        kpack[m] = kp;
+        tid[m] = (int32_t)t;
+    }
+    // stable counting sort by tile
+    std::vector<int64_t> start(p->n_tiles + 1, 0);
+    for (int64_t m = 0; m < M; ++m) start[tid[m] + 1]++;
+    p->max_tile_samples = 0;
+    for (int64_t t = 0; t < p->n_tiles; ++t) {
+        p->max_tile_samples = std::max<int64_t>(p->max_tile_samples, start[t + 1]);
+        start[t + 1] += start[t];
+    }
+    std::vector<int32_t> perm(M);
+    {
+        std::vector<int64_t> cur(start.begin(), start.end() - 1);
+        for (int64_t m = 0; m < M; ++m) perm[cur[tid[m]]++] = (int32_t)m;
+    }
+    std::vector<uint32_t> kpack_s(M);
+    std::vector<float> delta_s((size_t)d * M);
+    for (int64_t i = 0; i < M; ++i) {
+        kpack_s[i] = kpack[perm[i]];
+        for (int a = 0; a < d; ++a) delta_s[(size_t)a * M + i] = delta[(size_t)a * M + perm[i]];
+    }
+    NU_TRY(dev_upload(&p->d_kpack, kpack_s, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_delta, delta_s, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_perm, perm, &p->bytes_plan));
+    p->n_work = p->n_tiles;
+    // workspace
+    NU_TRY(dev_alloc((void**)&p->d_grid, (size_t)p->max_batch * p->cells * sizeof(float2), &p->bytes_work));
+    NU_TRY(dev_alloc((void**)&p->d_ywork, (size_t)p->max_batch * std::max<int64_t>(M, 1) * sizeof(float2), &p->bytes_work));
+    NU_TRY(dev_alloc((void**)&p->d_scal, sizeof(CgScalars), &p->bytes_work));
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int* Jd, int64_t M, const double* om,
+                          int max_batch, const nufft_opts* opts, nufft_plan_t* out) {
+    if (out) *out = nullptr;
+    if (!out || !Nd || !Kd || !Jd || (d != 2 && d != 3) || M < 0 || (M > 0 && !om) || max_batch < 1) return NUFFT_EINVAL;
+    if (M > (int64_t)0x7fffffff) return NUFFT_EINVAL;
+    for (int a = 0; a < d; ++a) {
+        if (Jd[a] != kJ || !supported_K(Kd[a]) || Kd[a] != 2 * Nd[a]) return NUFFT_EINVAL;
+    }
+    if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
+                 opts->interp_mode > 1))
+        return NUFFT_EINVAL;
+    static cudaError_t cfg = configure_all();
+    if (cfg != cudaSuccess) { g_last_cuda_error = (int)cfg; return NUFFT_ECUDA; }
+    nufft_plan_t p = new (std::nothrow) nufft_plan_s();
+    if (!p) return NUFFT_ENOMEM;
+    p->d = d;
+    p->M = M;
+    p->max_batch = max_batch;
+    if (opts) p->opts = *opts;
+    p->nimg = 1; p->cells = 1;
+    for (int a = 0; a < d; ++a) {
+        p->N[a] = (int)Nd[a]; p->K[a] = (int)Kd[a];
+        p->nimg *= Nd[a]; p->cells *= Kd[a];
+    }
+    int rc = NUFFT_OK;
+    try {
+        rc = plan_build(p, om);
+    } catch (const std::bad_alloc&) {
+        rc = NUFFT_ENOMEM;
+    }
+    if (rc != NUFFT_OK) { nufft_destroy(p); return rc; }
+    *out = p;
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_destroy(nufft_plan_t p) {
+    if (!p) return NUFFT_EINVAL;
+    for (int a = 0; a < 3; ++a) { cudaFree(p->d_scale[a]); cudaFree(p->d_tw[a]); }
+    cudaFree(p->d_kpack); cudaFree(p->d_delta); cudaFree(p->d_perm);
+    cudaFree(p->d_grid); cudaFree(p->d_ywork); cudaFree(p->d_imgwork); cudaFree(p->d_solver);
+    cudaFree(p->d_scal); cudaFree(p->d_hist);
+    (void)cudaGetLastError();
+    delete p;
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_plan_info(nufft_plan_t p, int64_t* bytes_plan, int64_t* bytes_work, int64_t* n_tiles,
+                               int64_t* n_work, int64_t* max_tile_samples) {
+    if (!p) return NUFFT_EINVAL;
+    if (bytes_plan) *bytes_plan = p->bytes_plan;
+    if (bytes_work) *bytes_work = p->bytes_work;
+    if (n_tiles) *n_tiles = p->n_tiles;
+    if (n_work) *n_work = p->n_work;
+    if (max_tile_samples) *max_tile_samples = p->max_tile_samples;
+    return NUFFT_OK;
+}
+
+extern "C" int64_t nufft_launch_count(nufft_plan_t p) { return p ? p->launches : -1; }
+
+// ------------------------------------------------------------------------------------------------------------
+// transforms
+// ------------------------------------------------------------------------------------------------------------
+static bool bad_batch(nufft_plan_t p, int batch) { return !p || batch < 1 || batch > p->max_batch; }
+
+extern "C" int nufft_stage_scale_fft(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* grid, void* stream) {
+    if (bad_batch(p, batch) || !x || !grid) return NUFFT_EINVAL;
+    return run_scale_fft(p, batch, (const float2*)x, (float2*)grid, nullptr, false, (cudaStream_t)stream);
+}
+extern "C" int nufft_stage_interp(nufft_plan_t p, int batch, const nufft_c64* grid, nufft_c64* y, void* stream) {
+    if (bad_batch(p, batch) || !grid || (!y && p->M > 0)) return NUFFT_EINVAL;
+    return run_interp(p, batch, (const float2*)grid, (float2*)y, (cudaStream_t)stream);
+}
+extern "C" int nufft_stage_gridding(nufft_plan_t p, int batch, const nufft_c64* y, nufft_c64* grid, void* stream) {
+    if (bad_batch(p, batch) || !grid || (!y && p->M > 0)) return NUFFT_EINVAL;
+    return run_gridding(p, batch, (const float2*)y, (float2*)grid, (cudaStream_t)stream);
+}
+extern "C" int nufft_stage_fft_scale(nufft_plan_t p, int batch, nufft_c64* grid, nufft_c64* x, void* stream) {
+    if (bad_batch(p, batch) || !x || !grid) return NUFFT_EINVAL;
+    return run_fft_scale(p, batch, (float2*)grid, (float2*)x, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* y, void* stream) {
+    if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_scale_fft(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
+    return run_interp(p, batch, p->d_grid, (float2*)y, st);
+}
+
+extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nufft_c64* x, void* stream) {
+    if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_gridding(p, batch, (const float2*)y, p->d_grid, st));
+    return run_fft_scale(p, batch, p->d_grid, (float2*)x, nullptr, st);
+}
+
+extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
+    if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_scale_fft(p, batch, (const float2*)x_in, p->d_grid, nullptr, false, st));
+    NU_TRY(run_interp(p, batch, p->d_grid, p->d_ywork, st));
+    NU_TRY(run_gridding(p, batch, p->d_ywork, p->d_grid, st));
+    return run_fft_scale(p, batch, p->d_grid, (float2*)x_out, nullptr, st);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// multi-coil operator, eqs. (34)-(35)
+// ------------------------------------------------------------------------------------------------------------
+extern "C" int nufft_set_coils(nufft_plan_t p, int ncoil, const nufft_c64* c) {
+    if (!p || ncoil < 0 || ncoil > p->max_batch || (ncoil > 0 && !c)) return NUFFT_EINVAL;
+    p->ncoil = ncoil;
+    p->d_coils = (ncoil > 0) ? (const float2*)c : nullptr;
+    if (ncoil > 0 && !p->d_imgwork)
+        NU_TRY(dev_alloc((void**)&p->d_imgwork, (size_t)p->max_batch * p->nimg * sizeof(float2), &p->bytes_work));
+    return NUFFT_OK;
+}
+
+static int coil_reduce(nufft_plan_t p, float2* x, cudaStream_t st) {
+    const int blocks = (int)std::min<int64_t>((p->nimg + 255) / 256, 148 * 8);
+    coil_sum_kernel<<<blocks, 256, 0, st>>>(x, p->d_imgwork, p->ncoil, p->nimg);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_forward_coils(nufft_plan_t p, const nufft_c64* x, nufft_c64* y, void* stream) {
+    if (!p || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    if (p->ncoil < 1) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_scale_fft(p, p->ncoil, (const float2*)x, p->d_grid, p->d_coils, true, st));
+    return run_interp(p, p->ncoil, p->d_grid, (float2*)y, st);
+}
+
+extern "C" int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64* y, nufft_c64* x, void* stream) {
+    if (!p || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    if (p->ncoil < 1) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_gridding(p, p->ncoil, (const float2*)y, p->d_grid, st));
+    NU_TRY(run_fft_scale(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
+    return coil_reduce(p, (float2*)x, st);
+}
+
+extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
+    if (!p || !x_in || !x_out) return NUFFT_EINVAL;
+    if (p->ncoil < 1) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_scale_fft(p, p->ncoil, (const float2*)x_in, p->d_grid, p->d_coils, true, st));
+    NU_TRY(run_interp(p, p->ncoil, p->d_grid, p->d_ywork, st));
+    NU_TRY(run_gridding(p, p->ncoil, p->d_ywork, p->d_grid, st));
+    NU_TRY(run_fft_scale(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
+    return coil_reduce(p, (float2*)x_out, st);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// solvers
+// ------------------------------------------------------------------------------------------------------------
+static int ew_blocks(int64_t n) { return (int)std::max<int64_t>(1, std::min<int64_t>((n + 255) / 256, 148 * 8)); }
+
+static int ensure_solver(nufft_plan_t p, int64_t nvec, int hist) {
+    if (p->solver_vecs < nvec) {
+        cudaFree(p->d_solver);
+        p->d_solver = nullptr;
+        p->solver_vecs = 0;
+        NU_TRY(dev_alloc((void**)&p->d_solver, (size_t)nvec * p->nimg * sizeof(float2), &p->bytes_work));
+        p->solver_vecs = nvec;
+    }
+    if (p->hist_cap < hist) {
+        cudaFree(p->d_hist);
+        p->d_hist = nullptr;
+        p->hist_cap = 0;
+        NU_TRY(dev_alloc((void**)&p->d_hist, (size_t)hist * sizeof(double), &p->bytes_work));
+        p->hist_cap = hist;
+    }
+    return NUFFT_OK;
+}
+
+static int apply_aha(nufft_plan_t p, bool coils, const float2* in, float2* out, cudaStream_t st) {
+    if (coils) return nufft_selfadjoint_coils(p, (const nufft_c64*)in, (nufft_c64*)out, st);
+    return nufft_selfadjoint(p, 1, (const nufft_c64*)in, (nufft_c64*)out, st);
+}
+
+// operator of the L1TV inner problem, eq. (15): out = mu A^H A z + lam sum_a grad_a^T grad_a z   (mu = 1, lam = 0: A^H A)
+struct NormalOp {
+    bool coils;
+    bool tv;
+    float mu, lam;
+};
+static int apply_op(nufft_plan_t p, const NormalOp& op, const float2* in, float2* out, cudaStream_t st) {
+    NU_TRY(apply_aha(p, op.coils, in, out, st));
+    if (op.tv) {
+        tv_normal_kernel<<<ew_blocks(p->nimg), 256, 0, st>>>(out, in, op.mu, op.lam, p->N[0], p->N[1]);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+    }
+    return NUFFT_OK;
+}
+
+// niter CG steps on op(x) = rhs from the x already in `x` (warm = true) or from 0 (warm = false, x is overwritten).
+// r, pv, Ap: work vectors.  hist: device double[niter + 1] or nullptr.
+static int cg_run(nufft_plan_t p, const NormalOp& op, const float2* rhs, float2* x, bool warm, int niter, float2* r,
+                  float2* pv, float2* Ap, double* hist, cudaStream_t st) {
+    const int64_t n = p->nimg;
+    const int nb = ew_blocks(n);
+    scalars_clear_kernel<<<1, 1, 0, st>>>(p->d_scal);
+    if (warm) {
+        NU_TRY(apply_op(p, op, x, Ap, st));
+        cg_init_kernel<<<nb, 256, 0, st>>>(rhs, Ap, r, pv, n, p->d_scal);
+    } else {
+        CU_TRY(cudaMemsetAsync(x, 0, (size_t)n * sizeof(float2), st));
+        cg_init_kernel<<<nb, 256, 0, st>>>(rhs, nullptr, r, pv, n, p->d_scal);
+    }
+    cg_shift_kernel<<<1, 1, 0, st>>>(p->d_scal, hist, 1);
+    p->launches += 3;
+    for (int k = 0; k < niter; ++k) {
+        NU_TRY(apply_op(p, op, pv, Ap, st));
+        dot_real_kernel<<<nb, 256, 0, st>>>(pv, Ap, n, &p->d_scal->pAp);
+        cg_update_xr_kernel<<<nb, 256, 0, st>>>(x, r, pv, Ap, n, p->d_scal);
+        cg_update_p_kernel<<<nb, 256, 0, st>>>(pv, r, n, p->d_scal);
+        cg_shift_kernel<<<1, 1, 0, st>>>(p->d_scal, hist ? hist + k + 1 : nullptr, 0);
+        p->launches += 4;
+    }
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+
+static int adjoint_any(nufft_plan_t p, bool coils, const float2* y, float2* x, cudaStream_t st) {
+    if (coils) return nufft_adjoint_coils(p, (const nufft_c64*)y, (nufft_c64*)x, st);
+    return nufft_adjoint(p, 1, (const nufft_c64*)y, (nufft_c64*)x, st);
+}
+
+extern "C" int nufft_solve_cg(nufft_plan_t p, int use_coils, const nufft_c64* y, nufft_c64* x, int niter,
+                              double* resnorm_host, void* stream) {
+    if (!p || !y || !x || niter < 0) return NUFFT_EINVAL;
+    const bool coils = use_coils != 0;
+    if (coils && p->ncoil < 1) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(ensure_solver(p, 4, niter + 1));
+    float2* rhs = p->d_solver;
+    float2* r = rhs + p->nimg;
+    float2* pv = r + p->nimg;
+    float2* Ap = pv + p->nimg;
+    NU_TRY(adjoint_any(p, coils, (const float2*)y, rhs, st));
+    NormalOp op{coils, false, 1.f, 0.f};
+    NU_TRY(cg_run(p, op, rhs, (float2*)x, false, niter, r, pv, Ap, p->d_hist, st));
+    if (resnorm_host) {
+        CU_TRY(cudaMemcpyAsync(resnorm_host, p->d_hist, (size_t)(niter + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+    }
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_solve_l1tv_ols(nufft_plan_t p, int use_coils, const nufft_c64* y, nufft_c64* x, double mu,
+                                    double lam, int n_outer, int n_inner, int n_cg, void* stream) {
+    if (!p || !y || !x || n_outer < 0 || n_inner < 0 || n_cg < 0 || p->d != 2 || lam < 0.0) return NUFFT_EINVAL;
+    const bool coils = use_coils != 0;
+    if (coils && p->ncoil < 1) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n = p->nimg;
+    NU_TRY(ensure_solver(p, 12, 1));
+    float2* v = p->d_solver;
+    float2 *ahy_s = v, *ahy_k = v + n, *rhs = v + 2 * n, *r = v + 3 * n, *pv = v + 4 * n, *Ap = v + 5 * n;
+    float2 *d0 = v + 6 * n, *b0 = v + 7 * n, *d1 = v + 8 * n, *b1 = v + 9 * n, *xs = v + 10 * n, *tmp = v + 11 * n;
+    const int nb = ew_blocks(n);
+    // A^H y and the problem scale c = 1 / max |A^H y|   (R17)
+    NU_TRY(adjoint_any(p, coils, (const float2*)y, tmp, st));
+    scalars_clear_kernel<<<1, 1, 0, st>>>(p->d_scal);
+    maxabs_kernel<<<nb, 256, 0, st>>>(tmp, n, p->d_scal);
+    p->launches += 2;
+    double mx = 0.0;
+    CU_TRY(cudaMemcpyAsync(&mx, &p->d_scal->maxabs, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    if (!(mx > 0.0)) {   // A^H y = 0: the solution is 0
+        CU_TRY(cudaMemsetAsync(x, 0, (size_t)n * sizeof(float2), st));
+        return NUFFT_OK;
+    }
+    const float c = (float)(1.0 / mx);
+    scale_kernel<<<nb, 256, 0, st>>>(ahy_s, tmp, c, n);
+    CU_TRY(cudaMemcpyAsync(ahy_k, ahy_s, (size_t)n * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    CU_TRY(cudaMemsetAsync(d0, 0, (size_t)4 * n * sizeof(float2), st));     // d0, b0, d1, b1 are contiguous
+    CU_TRY(cudaMemsetAsync(xs, 0, (size_t)n * sizeof(float2), st));
+    p->launches += 1;
+    const float fmu = (float)mu, flam = (float)lam;
+    const float thr = (lam > 0.0) ? (float)(1.0 / lam) : -1.0f;
+    NormalOp op{coils, true, fmu, flam};
+    for (int o = 0; o < n_outer; ++o) {
+        for (int i = 0; i < n_inner; ++i) {
+            tv_rhs_kernel<<<nb, 256, 0, st>>>(rhs, ahy_k, d0, b0, d1, b1, fmu, flam, p->N[0], p->N[1]);   // eq. (16)
+            p->launches++;
+            NU_TRY(cg_run(p, op, rhs, xs, true, n_cg, r, pv, Ap, nullptr, st));                           // eq. (17)
+            tv_shrink_kernel<<<nb, 256, 0, st>>>(xs, d0, b0, d1, b1, thr, p->N[0], p->N[1]);             // eqs. (18)-(21)
+            p->launches++;
+        }
+        NU_TRY(apply_aha(p, coils, xs, tmp, st));
+        tv_outer_kernel<<<nb, 256, 0, st>>>(ahy_k, ahy_s, tmp, n);                                        // eq. (22)
+        p->launches++;
+    }
+    scale_kernel<<<nb, 256, 0, st>>>((float2*)x, xs, (float)mx, n);
+    p->launches++;
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+extern "C" const char* nufft_strerror(int code) {
+    switch (code) {
+        case NUFFT_OK: return "ok";
+        case NUFFT_EINVAL: return "invalid argument or unsupported configuration";
+        case NUFFT_ENOMEM: return "out of memory";
+        case NUFFT_ECUDA: return "CUDA runtime error (see nufft_last_cuda_error)";
+        case NUFFT_ERANGE: return "non-finite sample location";
+        case NUFFT_ESTATE: return "missing state (coil maps not set)";
+    }
+    return "unknown error";
+}
+extern "C" int nufft_last_cuda_error(void) { return g_last_cuda_error; }
+extern "C" const char* nufft_version(void) { return "nufft-b200 0.1 (sm_100a)"; }
