@@ -1,0 +1,433 @@
+#!/usr/bin/env python
+"""bench.py -- NUFFT forward+adjoint pairs/s on one B200 (BASELINE.json metric), with roofline and CPU baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--batch B] [--no-extra]
+
+A "step" is one pass of the whole hot path over one batch: y = A x (nufft_forward: S + zero-pad + F + V) followed by
+x' = A^H y (nufft_adjoint: V^H + F^H + crop + S^H) for a batch of B independent images that share one trajectory
+(the paper's batch mode).  Workload at N = 1: BASELINE config 2 (configs[1]): 2-D golden-angle radial,
+Nd = 256^2, Kd = 512^2, Jd = 6^2, M = 131072, complex64, synthetic seeded inputs (workloads.py).
+
+  value      pairs/s, inputs resident in HBM, device time from CUDA events around each step on the launch stream;
+             L2 is flushed (256 MiB memset) between steps, outside the event brackets.
+  e2e        same metric through the host-buffer call: pinned host x -> H2D -> forward -> adjoint -> D2H x'.
+  roofline   the dominant kernel of the step: ALGORITHMIC bytes per launch / its average
+             duration measured live with CUDA events by the library (nufft_profile_*), against the measured HBM copy
+             bandwidth in MEASURED_PEAKS.json.
+  cpu_baseline  the float64 oracle, as it stands, timed on this box's host cores on a bounded sample.
+
+N > 1 (torchrun): replicas only -- every rank runs the same independent job on its own GPU, no collective in the data
+path; value = total pairs over the max-over-ranks time; scaling = weak.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "nufft_fwd_adj_pairs_per_s"
+UNIT = "pairs/s"
+WORKLOAD = "cfg2_2d_radial: Nd=256x256 Kd=512x512 Jd=6x6 golden-angle radial 256x512 (M=131072), complex64"
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            v = float(json.load(f)["hbm_gbs"])
+        return v, "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def algorithmic_bytes(d, N, K, M, B, cov=1.0):
+    """Per-launch algorithmic bytes of every kernel label."""
+    rec = 4 + 4 * d
+    if d == 2:
+        return {
+            "fft_rows_fwd": 8 * B * (N * N + N * K),
+            "fft_cols_fwd": 8 * B * (N * K + K * K),
+            "interp": B * (8 * K * K * cov + 8 * M) + M * rec,
+            "gridding": B * (8 * M + 8 * K * K) + M * rec,
+            "fft_cols_adj": 8 * B * (K * K + N * K),
+            "fft_rows_adj": 8 * B * (N * K + N * N),
+        }
+    return {
+        "fft_rows_fwd": 8 * B * (N ** 3 + N * N * K),
+        "fft_cols_fwd_axis1": 8 * B * (N * N * K + N * K * K),
+        "fft_cols_fwd_axis0": 8 * B * (N * K * K + K ** 3),
+        "interp": B * (8 * K ** 3 * cov + 8 * M) + M * rec,
+        "gridding": B * (8 * M + 8 * K ** 3) + M * rec,
+        "fft_cols_adj_axis0": 8 * B * (K ** 3 + N * K * K),
+        "fft_cols_adj_axis1": 8 * B * (N * K * K + N * N * K),
+        "fft_rows_adj": 8 * B * (N * N * K + N ** 3),
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = str(gpu_index)
+        self.lines = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", self.gpu], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# the oracle legs (CPU)
+# ----------------------------------------------------------------------------------------------------------------
+def oracle_pair_seconds(cfg, x, min_seconds, max_pairs):
+    from oracle import nufft_oracle as orc
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    x128 = x.astype(np.complex128)
+    n, t0, c0 = 0, time.perf_counter(), time.process_time()
+    while True:
+        y = orc.forward(x128, om, Nd, Kd, Jd)
+        orc.adjoint(y, om, Nd, Kd, Jd)
+        n += 1
+        el = time.perf_counter() - t0
+        if el >= min_seconds or n >= max_pairs:
+            return el / n, n, cores_used(time.process_time() - c0, el)
+
+
+def cores_used(cpu_seconds, wall_seconds):
+    """Threads the oracle actually kept busy: process CPU time / wall time, rounded (numpy's FFT and the vectorised
+    stencil loops are single-threaded, so this is normally 1)."""
+    return max(1, int(round(cpu_seconds / max(wall_seconds, 1e-9))))
+
+
+def run_reference(args):
+    """--impl reference: the float64 oracle (oracle/), as it stands, on the host cores.  One step = one
+    forward+adjoint pair on ONE image of the workload (a bounded sample of the batch the CUDA arm processes)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = wl.config(1)
+    x = wl.image_gaussian(cfg["Nd"])
+    from oracle import nufft_oracle as orc
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    x128 = x.astype(np.complex128)
+    steps = max(1, min(args.steps, 40))
+    for _ in range(max(1, min(args.warmup, 3))):
+        orc.adjoint(orc.forward(x128, om, Nd, Kd, Jd), om, Nd, Kd, Jd)
+    t0, c0 = time.perf_counter(), time.process_time()
+    for _ in range(steps):
+        orc.adjoint(orc.forward(x128, om, Nd, Kd, Jd), om, Nd, Kd, Jd)
+    el = time.perf_counter() - t0
+    ncores = cores_used(time.process_time() - c0, el)
+    v = steps / el
+    sample = "1 image (batch element 0) of the workload per step, %d steps" % steps
+    out = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "complex128", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "batch": 1, "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": ncores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ----------------------------------------------------------------------------------------------------------------
+def kernel_table(prof, bytes_per_launch, peak):
+    rows = {}
+    for name, (ms, n) in prof.items():
+        if n == 0:
+            continue
+        avg_ms = ms / n
+        b = bytes_per_launch.get(name)
+        rows[name] = {"ms_per_launch": avg_ms, "launches": n}
+        if b is not None and avg_ms > 0:
+            gbs = b / (avg_ms * 1e-3) / 1e9
+            rows[name].update({"alg_bytes": int(b), "gbs": gbs, "frac": gbs / peak})
+    return rows
+
+
+def stage_of(rows, keys):
+    return sum(rows[k]["ms_per_launch"] for k in keys if k in rows)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1710_03197_b200 as nb
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    nb.lib()   # fail loudly here if the extension is missing
+
+    B, K_steps, W = args.batch, args.steps, max(args.warmup, 3)
+    cfg = wl.config(1)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    M = om.shape[0]
+    plan = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=B)
+    x_host = torch.from_numpy(wl.image_gaussian(Nd, seed=wl.SEED_IMAGE + rank, batch=B)).pin_memory()
+    x = x_host.cuda()
+    y = torch.empty((B, M), dtype=torch.complex64, device="cuda")
+    xo = torch.empty((B,) + tuple(Nd), dtype=torch.complex64, device="cuda")
+    xo_host = torch.empty((B,) + tuple(Nd), dtype=torch.complex64).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.forward(x, y)
+        plan.adjoint(y, xo)
+
+    def step_e2e():
+        xd = x_host.to("cuda", non_blocking=True)
+        plan.forward(xd, y)
+        plan.adjoint(y, xo)
+        xo_host.copy_(xo, non_blocking=True)
+
+    def timed(fn, nsteps):
+        evs = []
+        for _ in range(nsteps):
+            flush.zero_()                     # L2 flush, outside the event bracket
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(W):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    l0 = plan.launch_count()
+    total_ms = timed(step, K_steps)
+    l1 = plan.launch_count()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    e2e_ms = timed(step_e2e, K_steps)
+    barrier()
+
+    if world > 1:
+        t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = float(t[0]), float(t[1])
+
+    # per-kernel device times of the same step (library-side CUDA events on the launch stream)
+    peak, peak_src = measured_peak()
+    plan.profile_enable(True)
+    plan.profile_reset()
+    timed(step, K_steps)
+    rows = kernel_table(plan.profile(), algorithmic_bytes(2, Nd[0], Kd[0], M, B), peak)
+    plan.profile_enable(False)
+
+    result = None
+    if rank == 0:
+        ms_per_step = total_ms / K_steps
+        value = world * B / (ms_per_step * 1e-3)
+        timed_kernels = {k: v for k, v in rows.items() if "alg_bytes" in v}
+        dom = max(timed_kernels, key=lambda k: timed_kernels[k]["ms_per_launch"])
+        traffic = None
+        try:
+            with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
+                traffic = json.load(f).get("cfg2_batch%d" % B, {}).get(dom)
+        except Exception:
+            pass
+        step_bytes = sum(v["alg_bytes"] for v in timed_kernels.values())
+        roofline = {
+            "bound": "hbm", "kernel": dom, "achieved": timed_kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
+            "frac": timed_kernels[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+            "alg_bytes_per_launch": timed_kernels[dom]["alg_bytes"],
+            "ms_per_launch": timed_kernels[dom]["ms_per_launch"],
+            "step_alg_bytes": int(step_bytes),
+            "step_frac_of_roofline": (step_bytes / (ms_per_step * 1e-3) / 1e9) / peak,
+            "kernels": rows,
+            "stages_ms": {
+                "F (S+pad+FFT)": stage_of(rows, ["fft_rows_fwd", "fft_cols_fwd"]),
+                "V": stage_of(rows, ["interp"]),
+                "V^H": stage_of(rows, ["grid_zero", "gridding", "gridding_merge"]),
+                "F^H (IFFT+crop+S^H)": stage_of(rows, ["fft_cols_adj", "fft_rows_adj"]),
+            },
+            "note": "2-D grids of this batch are partly L2-resident between kernels of one step; V and V^H are "
+                    "bound by shared-memory/L1 gather bandwidth before HBM (SURVEY.md 7.3-1)",
+        }
+        cpu_s, cpu_n, cpu_cores = oracle_pair_seconds(cfg, wl.image_gaussian(Nd), args.cpu_seconds, 200)
+        result = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K_steps, "warmup": W,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "batch": B, "pairs_per_step": B, "l2": "flushed between steps (256 MiB memset)",
+                       "parallelism": "replicas x%d" % world, "adjoint_mode": 0},
+            "clocks": clocks,
+            "e2e": {"value": world * B / (e2e_ms / K_steps * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(x_host.numel() * 8), "d2h_bytes_per_step": int(xo_host.numel() * 8),
+                    "ms_per_step": e2e_ms / K_steps},
+            "gpu_launches": int(l1 - l0),
+            "roofline": roofline,
+            "cpu_baseline": {"value": 1.0 / cpu_s, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
+                             "sample": "%d forward+adjoint pairs on one image of the workload (batch element 0)" % cpu_n},
+            "paper_context": "PAPER.md Table 1 (:299-300): forward 6 ms + adjoint 6 ms on one K80 GK210 (PyCUDA), "
+                             "workload sizes not stated by the paper",
+        }
+        if world == 1 and not args.no_extra:
+            try:
+                result["extra"] = extra_legs(nb, torch, peak, args)
+            except Exception as e:  # extras never break the contract line
+                result["extra"] = {"error": repr(e)}
+    plan.destroy()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(result))
+    return 0
+
+
+def extra_legs(nb, torch, peak, args):
+    """Other BASELINE configs on one GPU: batch-1 latency of config 2 and the 3-D config 4 (forward and adjoint)."""
+    out = {}
+
+    def time_calls(fn, n, flush):
+        evs = []
+        for _ in range(n):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return float(np.median([a.elapsed_time(b) for a, b in evs]))
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    # config 2, batch 1 (latency)
+    cfg = wl.config(1)
+    p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1)
+    x = torch.from_numpy(wl.image_gaussian(cfg["Nd"])).cuda().reshape(1, *cfg["Nd"])
+    y = p.forward(x)
+    xo = p.adjoint(y)
+    for _ in range(3):
+        p.forward(x, y), p.adjoint(y, xo)
+    out["cfg2_batch1"] = {"forward_ms": time_calls(lambda: p.forward(x, y), 20, flush),
+                          "adjoint_ms": time_calls(lambda: p.adjoint(y, xo), 20, flush),
+                          "selfadjoint_ms": time_calls(lambda: p.selfadjoint(x, xo), 20, flush)}
+    p.destroy()
+    # config 4, 3-D
+    cfg = wl.config(3)
+    N, K, M = cfg["Nd"][0], cfg["Kd"][0], cfg["om"].shape[0]
+    p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1)
+    x = torch.from_numpy(wl.image_gaussian(cfg["Nd"])).cuda().reshape(1, *cfg["Nd"])
+    y = p.forward(x)
+    xo = p.adjoint(y)
+    for _ in range(2):
+        p.forward(x, y), p.adjoint(y, xo)
+    f_ms = time_calls(lambda: p.forward(x, y), 5, flush)
+    a_ms = time_calls(lambda: p.adjoint(y, xo), 5, flush)
+    p.profile_enable(True)
+    p.profile_reset()
+    for _ in range(3):
+        flush.zero_()
+        p.forward(x, y)
+        p.adjoint(y, xo)
+    torch.cuda.synchronize()
+    rows = kernel_table(p.profile(), algorithmic_bytes(3, N, K, M, 1, cov=0.55), peak)
+    info = p.info()
+    p.destroy()
+    out["cfg4_3d_kooshball"] = {
+        "workload": "Nd=128^3 Kd=256^3 Jd=6^3 M=2097152 kooshball, batch 1", "forward_ms": f_ms, "adjoint_ms": a_ms,
+        "pairs_per_s": 1e3 / (f_ms + a_ms), "kernels": rows, "plan": info,
+        "note": "interp alg_bytes use coverage 0.55 of the 256^3 grid (SURVEY.md 8(d))"}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=64)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-extra", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", "29533", os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -132,6 +132,15 @@ int nufft_plan_info(nufft_plan_t p, int64_t *bytes_plan, int64_t *bytes_work,
 /* Number of kernel launches the library has enqueued for this plan since creation (bench.py's gpu_launches). */
 int64_t nufft_launch_count(nufft_plan_t p);
 
+/* Per-kernel device timing (bench.py's roofline leg).  While enabled, every kernel the library launches for this
+ * plan is bracketed by a pair of CUDA events on the launching stream.  nufft_profile_get synchronises those events
+ * and returns, for kernel label i (0 <= i < nufft_profile_count), its name (static string), the summed device time
+ * in milliseconds and the number of launches since the last reset.  Timing is off by default (no events recorded). */
+int nufft_profile_enable(nufft_plan_t p, int on);
+int nufft_profile_reset(nufft_plan_t p);
+int nufft_profile_count(nufft_plan_t p);
+int nufft_profile_get(nufft_plan_t p, int i, const char **name, double *total_ms, int64_t *launches);
+
 int nufft_destroy(nufft_plan_t p);
 
 const char *nufft_strerror(int code);

@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = [
     "nufft_stage_scale_fft", "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale",
     "nufft_set_coils", "nufft_forward_coils", "nufft_adjoint_coils", "nufft_selfadjoint_coils",
     "nufft_solve_cg", "nufft_solve_l1tv_ols", "nufft_plan_info", "nufft_launch_count", "nufft_destroy",
+    "nufft_profile_enable", "nufft_profile_reset", "nufft_profile_count", "nufft_profile_get",
     "nufft_strerror", "nufft_last_cuda_error", "nufft_version",
 ]
 
@@ -66,6 +67,10 @@ def lib():
     L.nufft_launch_count.argtypes = [_PLAN]
     L.nufft_launch_count.restype = _c.c_int64
     L.nufft_destroy.argtypes = [_PLAN]
+    L.nufft_profile_enable.argtypes = [_PLAN, _c.c_int]
+    L.nufft_profile_reset.argtypes = [_PLAN]
+    L.nufft_profile_count.argtypes = [_PLAN]
+    L.nufft_profile_get.argtypes = [_PLAN, _c.c_int, _c.POINTER(_c.c_char_p), _c.POINTER(_c.c_double), _I64P]
     L.nufft_strerror.argtypes = [_c.c_int]
     L.nufft_strerror.restype = _c.c_char_p
     L.nufft_last_cuda_error.restype = _c.c_int
@@ -276,6 +281,21 @@ class NufftPlan:
 
     def launch_count(self):
         return int(lib().nufft_launch_count(self._h))
+
+    def profile_enable(self, on=True):
+        _check(lib().nufft_profile_enable(self._h, int(bool(on))), "nufft_profile_enable")
+
+    def profile_reset(self):
+        _check(lib().nufft_profile_reset(self._h), "nufft_profile_reset")
+
+    def profile(self):
+        """{kernel label: (total device ms, launches)} since the last reset (synchronises the recorded events)."""
+        out = {}
+        for i in range(lib().nufft_profile_count(self._h)):
+            name, ms, n = _c.c_char_p(), _c.c_double(), _c.c_int64()
+            _check(lib().nufft_profile_get(self._h, i, _c.byref(name), _c.byref(ms), _c.byref(n)), "nufft_profile_get")
+            out[name.value.decode()] = (float(ms.value), int(n.value))
+        return out
 
     # -- host-buffer convenience (the e2e path) ---------------------------------------------------------------
     def forward_host(self, x_host, y_host=None):

@@ -60,12 +60,48 @@ struct nufft_plan_s {
     // coils (borrowed)
     int ncoil = 0;
     const float2* d_coils = nullptr;
-    // tiles
+    // tiles and V^H work items
     int tile[3] = {1, 1, 1}, ntile[3] = {1, 1, 1};
+    TileGeom tg{};
+    WorkItem* d_items = nullptr;
+    int32_t* d_tile_item_start = nullptr;
+    int n_items = 0;
+    float2* d_slabs = nullptr;      // deterministic mode: [max_batch][n_items][tile_cells], lazy
     int64_t n_tiles = 0, n_work = 0, max_tile_samples = 0;
     int64_t bytes_plan = 0, bytes_work = 0;
     int64_t launches = 0;
+    // optional per-kernel event timing (nufft_profile_*)
+    bool prof_on = false;
+    struct ProfRec { int label; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof;
+    std::vector<const char*> prof_labels;
+    std::vector<double> prof_ms;
+    std::vector<int64_t> prof_n;
 };
+
+// Brackets the launches issued during its lifetime with a pair of events when profiling is enabled.
+struct ProfScope {
+    nufft_plan_t p;
+    cudaStream_t st;
+    int idx = -1;
+    ProfScope(nufft_plan_t p_, const char* label, cudaStream_t st_) : p(p_), st(st_) {
+        if (!p->prof_on) return;
+        int li = -1;
+        for (size_t i = 0; i < p->prof_labels.size(); ++i)
+            if (p->prof_labels[i] == label || std::strcmp(p->prof_labels[i], label) == 0) { li = (int)i; break; }
+        if (li < 0) { li = (int)p->prof_labels.size(); p->prof_labels.push_back(label); p->prof_ms.push_back(0.0); p->prof_n.push_back(0); }
+        nufft_plan_s::ProfRec r{li, nullptr, nullptr};
+        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+        cudaEventRecord(r.a, st);
+        idx = (int)p->prof.size();
+        p->prof.push_back(r);
+    }
+    ~ProfScope() {
+        if (idx >= 0) cudaEventRecord(p->prof[idx].b, st);
+    }
+};
+
+static int dev_alloc(void** dptr, size_t bytes, int64_t* acct);
 
 // ------------------------------------------------------------------------------------------------------------
 // kernel configuration (dynamic shared memory opt-in), once per process
@@ -93,6 +129,11 @@ static cudaError_t configure_all() {
     if ((e = configure_fft<256>()) != cudaSuccess) return e;
     if ((e = configure_fft<512>()) != cudaSuccess) return e;
     if ((e = configure_fft<1024>()) != cudaSuccess) return e;
+    const int big = 200 * 1024;
+    if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     return cudaSuccess;
 }
 
@@ -168,7 +209,7 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
                          bool same_image, cudaStream_t st) {
     const int d = p->d;
     RowPassParams r = row_params(p, batch, x, nullptr, grid, coil, same_image);
-    NU_TRY(dispatch_rows(p->K[d - 1], false, r, st));
+    { ProfScope ps(p, "fft_rows_fwd", st); NU_TRY(dispatch_rows(p->K[d - 1], false, r, st)); }
     p->launches++;
     if (d == 2) {
         ColPassParams c{};
@@ -176,7 +217,7 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
         c.batch_stride = p->cells; c.outer_stride = 0; c.line_stride = p->K[1];
         c.n_outer = 1; c.k_outer = 0; c.inner = p->K[1];
         c.ngroups = batch * (c.inner / tile_T(p->K[0]));
-        NU_TRY(dispatch_cols(p->K[0], false, c, st));
+        { ProfScope ps(p, "fft_cols_fwd", st); NU_TRY(dispatch_cols(p->K[0], false, c, st)); }
         p->launches++;
     } else {
         ColPassParams c{};
@@ -184,13 +225,13 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
         c.batch_stride = p->cells; c.outer_stride = (int64_t)p->K[1] * p->K[2]; c.line_stride = p->K[2];
         c.n_outer = p->N[0]; c.k_outer = p->K[0]; c.inner = p->K[2];
         c.ngroups = batch * c.n_outer * (c.inner / tile_T(p->K[1]));
-        NU_TRY(dispatch_cols(p->K[1], false, c, st));
+        { ProfScope ps(p, "fft_cols_fwd_axis1", st); NU_TRY(dispatch_cols(p->K[1], false, c, st)); }
         ColPassParams c0{};
         c0.grid = grid; c0.tw = p->d_tw[0];
         c0.batch_stride = p->cells; c0.outer_stride = 0; c0.line_stride = (int64_t)p->K[1] * p->K[2];
         c0.n_outer = 1; c0.k_outer = 0; c0.inner = p->K[1] * p->K[2];
         c0.ngroups = batch * (c0.inner / tile_T(p->K[0]));
-        NU_TRY(dispatch_cols(p->K[0], false, c0, st));
+        { ProfScope ps(p, "fft_cols_fwd_axis0", st); NU_TRY(dispatch_cols(p->K[0], false, c0, st)); }
         p->launches += 2;
     }
     return NUFFT_OK;
@@ -205,7 +246,7 @@ static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, con
         c.batch_stride = p->cells; c.outer_stride = 0; c.line_stride = p->K[1];
         c.n_outer = 1; c.k_outer = 0; c.inner = p->K[1];
         c.ngroups = batch * (c.inner / tile_T(p->K[0]));
-        NU_TRY(dispatch_cols(p->K[0], true, c, st));
+        { ProfScope ps(p, "fft_cols_adj", st); NU_TRY(dispatch_cols(p->K[0], true, c, st)); }
         p->launches++;
     } else {
         ColPassParams c0{};
@@ -213,17 +254,17 @@ static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, con
         c0.batch_stride = p->cells; c0.outer_stride = 0; c0.line_stride = (int64_t)p->K[1] * p->K[2];
         c0.n_outer = 1; c0.k_outer = 0; c0.inner = p->K[1] * p->K[2];
         c0.ngroups = batch * (c0.inner / tile_T(p->K[0]));
-        NU_TRY(dispatch_cols(p->K[0], true, c0, st));
+        { ProfScope ps(p, "fft_cols_adj_axis0", st); NU_TRY(dispatch_cols(p->K[0], true, c0, st)); }
         ColPassParams c{};
         c.grid = grid; c.tw = p->d_tw[1];
         c.batch_stride = p->cells; c.outer_stride = (int64_t)p->K[1] * p->K[2]; c.line_stride = p->K[2];
         c.n_outer = p->N[0]; c.k_outer = p->K[0]; c.inner = p->K[2];
         c.ngroups = batch * c.n_outer * (c.inner / tile_T(p->K[1]));
-        NU_TRY(dispatch_cols(p->K[1], true, c, st));
+        { ProfScope ps(p, "fft_cols_adj_axis1", st); NU_TRY(dispatch_cols(p->K[1], true, c, st)); }
         p->launches += 2;
     }
     RowPassParams r = row_params(p, batch, nullptr, x, grid, coil, false);
-    NU_TRY(dispatch_rows(p->K[d - 1], true, r, st));
+    { ProfScope ps(p, "fft_rows_adj", st); NU_TRY(dispatch_rows(p->K[d - 1], true, r, st)); }
     p->launches++;
     return NUFFT_OK;
 }
@@ -244,6 +285,7 @@ static SampleData sample_data(nufft_plan_t p) {
 static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, cudaStream_t st) {
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
+    ProfScope ps(p, "interp", st);
     if (p->d == 2) interp_direct_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     else           interp_direct_kernel<3><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     CU_TRY(cudaGetLastError());
@@ -252,14 +294,42 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
 }
 
 // a4: grid = V^H y
+static constexpr int kGrid2dWarps = 8;
+static size_t smem_grid2d(nufft_plan_t p) { return (size_t)kGrid2dWarps * ((size_t)p->tg.tile_cells * 8 + kStageBytes); }
+static size_t smem_grid3d(nufft_plan_t p) { return (size_t)p->tg.tile_cells * 8 + 6 * (size_t)kStageBytes; }
+
 static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid, cudaStream_t st) {
-    CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st));
-    if (p->M == 0) return NUFFT_OK;
-    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
-    if (p->d == 2) gridding_atomic_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), y, grid, p->poly);
-    else           gridding_atomic_kernel<3><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), y, grid, p->poly);
+    const bool det = p->opts.adjoint_mode == 1;
+    if (p->M == 0 || p->n_items == 0) {
+        CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st));
+        return NUFFT_OK;
+    }
+    const int64_t slab_stride = (int64_t)p->n_items * p->tg.tile_cells;
+    if (det && !p->d_slabs)
+        NU_TRY(dev_alloc((void**)&p->d_slabs, (size_t)p->max_batch * slab_stride * sizeof(float2), &p->bytes_work));
+    if (!det) { ProfScope ps(p, "grid_zero", st); CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st)); }
+    ProfScope ps(p, "gridding", st);
+    if (p->d == 2) {
+        const dim3 blocks((unsigned)((p->n_items + kGrid2dWarps - 1) / kGrid2dWarps), (unsigned)batch);
+        const size_t sm = smem_grid2d(p);
+        if (det) gridding_tiled_2d_kernel<true><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly);
+        else     gridding_tiled_2d_kernel<false><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, nullptr, 0, p->poly);
+    } else {
+        const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
+        const size_t sm = smem_grid3d(p);
+        if (det) gridding_tiled_3d_kernel<true><<<blocks, 192, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly);
+        else     gridding_tiled_3d_kernel<false><<<blocks, 192, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, nullptr, 0, p->poly);
+    }
     CU_TRY(cudaGetLastError());
     p->launches++;
+    if (det) {
+        ProfScope pm(p, "gridding_merge", st);
+        const dim3 blocks((unsigned)((p->cells + 255) / 256), (unsigned)batch);
+        if (p->d == 2) gridding_merge_kernel<2><<<blocks, 256, 0, st>>>(grid_geom(p), p->tg, p->ntile[0], p->ntile[1], p->ntile[2], p->d_tile_item_start, p->d_slabs, slab_stride, grid);
+        else           gridding_merge_kernel<3><<<blocks, 256, 0, st>>>(grid_geom(p), p->tg, p->ntile[0], p->ntile[1], p->ntile[2], p->d_tile_item_start, p->d_slabs, slab_stride, grid);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+    }
     return NUFFT_OK;
 }
 
@@ -302,15 +372,26 @@ static int plan_build(nufft_plan_t p, const double* om) {
         NU_TRY(dev_upload(&p->d_tw[a], host::twiddle_table(p->K[a]), &p->bytes_plan));
     }
     // tiles
-    const int def2[3] = {16, 32, 1}, def3[3] = {8, 8, 8};
+    const int def2[3] = {16, 32, 1}, def3[3] = {8, 8, 16};
     for (int a = 0; a < 3; ++a) {
         int t = (a < d) ? p->opts.tile[a] : 1;
-        if (a < d && t <= 0) t = (d == 2) ? def2[a] : def3[a];
-        if (a < d && (t > p->K[a] || (p->K[a] % t) != 0)) return NUFFT_EINVAL;
+        if (a < d && t <= 0) t = std::min((d == 2) ? def2[a] : def3[a], p->K[a]);
+        if (a < d && (t < 8 || t > p->K[a] || (p->K[a] % t) != 0 || (t & 1))) return NUFFT_EINVAL;
         p->tile[a] = t;
         p->ntile[a] = (a < d) ? p->K[a] / t : 1;
     }
     p->n_tiles = (int64_t)p->ntile[0] * p->ntile[1] * p->ntile[2];
+    {
+        TileGeom& tg = p->tg;
+        for (int a = 0; a < 3; ++a) { tg.T[a] = p->tile[a]; tg.P[a] = (a < d) ? p->tile[a] + kJ - 1 : 1; }
+        // row pitch: >= T + J (8-cell aligned windows reach one cell past the halo) and = 8 (mod 16) cells, so that the
+        // two stencil rows of an 8-lane shared-memory phase fall into different 64-byte bank halves
+        int pitch = p->tile[d - 1] + kJ;
+        pitch += ((8 - pitch % 16) + 16) % 16;
+        tg.pitch = pitch;
+        tg.plane = (d == 3) ? tg.P[1] * pitch : 0;
+        tg.tile_cells = (d == 3) ? tg.P[0] * tg.P[1] * pitch : tg.P[0] * pitch;
+    }
     // per-sample split (float64) and tile id
     const int64_t M = p->M;
     std::vector<uint32_t> kpack(M);
@@ -353,7 +434,40 @@ static int plan_build(nufft_plan_t p, const double* om) {
     NU_TRY(dev_upload(&p->d_kpack, kpack_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_delta, delta_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_perm, perm, &p->bytes_plan));
-    p->n_work = p->n_tiles;
+    // V^H work items: (tile, sample range), hot tiles split into chunks of at most max_subtile samples
+    {
+        int cap = p->opts.max_subtile > 0 ? p->opts.max_subtile : (d == 2 ? 1024 : 512);
+        std::vector<WorkItem> items;
+        std::vector<int32_t> tstart(p->n_tiles + 1, 0);
+        for (int64_t t = 0; t < p->n_tiles; ++t) {
+            tstart[t] = (int32_t)items.size();
+            const int64_t b = start[t], e = start[t + 1];
+            if (e == b) continue;
+            int tc[3];
+            int64_t r = t;
+            for (int a = d - 1; a >= 0; --a) { tc[a] = (int)(r % p->ntile[a]); r /= p->ntile[a]; }
+            uint32_t origin = 0;
+            for (int a = 0; a < d; ++a) origin |= (uint32_t)(tc[a] * p->tile[a]) << (10 * a);
+            const int64_t nchunk = (e - b + cap - 1) / cap;
+            for (int64_t c = 0; c < nchunk; ++c) {
+                WorkItem w;
+                w.origin = origin;
+                w.s_begin = (int32_t)(b + (e - b) * c / nchunk);
+                w.s_end = (int32_t)(b + (e - b) * (c + 1) / nchunk);
+                w.slab = (int32_t)items.size();
+                items.push_back(w);
+            }
+        }
+        tstart[p->n_tiles] = (int32_t)items.size();
+        p->n_items = (int)items.size();
+        p->n_work = p->n_items;
+        // longest first: CTAs that start late get the short items
+        std::stable_sort(items.begin(), items.end(), [](const WorkItem& a, const WorkItem& b) {
+            return (a.s_end - a.s_begin) > (b.s_end - b.s_begin);
+        });
+        NU_TRY(dev_upload(&p->d_items, items, &p->bytes_plan));
+        NU_TRY(dev_upload(&p->d_tile_item_start, tstart, &p->bytes_plan));
+    }
     // workspace
     NU_TRY(dev_alloc((void**)&p->d_grid, (size_t)p->max_batch * p->cells * sizeof(float2), &p->bytes_work));
     NU_TRY(dev_alloc((void**)&p->d_ywork, (size_t)p->max_batch * std::max<int64_t>(M, 1) * sizeof(float2), &p->bytes_work));
@@ -396,12 +510,15 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     return NUFFT_OK;
 }
 
+static void prof_drain(nufft_plan_t p);
 extern "C" int nufft_destroy(nufft_plan_t p) {
     if (!p) return NUFFT_EINVAL;
+    prof_drain(p);
     for (int a = 0; a < 3; ++a) { cudaFree(p->d_scale[a]); cudaFree(p->d_tw[a]); }
     cudaFree(p->d_kpack); cudaFree(p->d_delta); cudaFree(p->d_perm);
     cudaFree(p->d_grid); cudaFree(p->d_ywork); cudaFree(p->d_imgwork); cudaFree(p->d_solver);
     cudaFree(p->d_scal); cudaFree(p->d_hist);
+    cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
     (void)cudaGetLastError();
     delete p;
     return NUFFT_OK;
@@ -419,6 +536,43 @@ extern "C" int nufft_plan_info(nufft_plan_t p, int64_t* bytes_plan, int64_t* byt
 }
 
 extern "C" int64_t nufft_launch_count(nufft_plan_t p) { return p ? p->launches : -1; }
+
+static void prof_drain(nufft_plan_t p) {
+    for (auto& r : p->prof) {
+        if (cudaEventSynchronize(r.b) == cudaSuccess) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) { p->prof_ms[r.label] += ms; p->prof_n[r.label]++; }
+        }
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    (void)cudaGetLastError();
+    p->prof.clear();
+}
+extern "C" int nufft_profile_enable(nufft_plan_t p, int on) {
+    if (!p) return NUFFT_EINVAL;
+    p->prof_on = on != 0;
+    return NUFFT_OK;
+}
+extern "C" int nufft_profile_reset(nufft_plan_t p) {
+    if (!p) return NUFFT_EINVAL;
+    prof_drain(p);
+    std::fill(p->prof_ms.begin(), p->prof_ms.end(), 0.0);
+    std::fill(p->prof_n.begin(), p->prof_n.end(), 0);
+    return NUFFT_OK;
+}
+extern "C" int nufft_profile_count(nufft_plan_t p) {
+    if (!p) return NUFFT_EINVAL;
+    return (int)p->prof_labels.size();
+}
+extern "C" int nufft_profile_get(nufft_plan_t p, int i, const char** name, double* total_ms, int64_t* launches) {
+    if (!p || i < 0 || i >= (int)p->prof_labels.size()) return NUFFT_EINVAL;
+    prof_drain(p);
+    if (name) *name = p->prof_labels[i];
+    if (total_ms) *total_ms = p->prof_ms[i];
+    if (launches) *launches = p->prof_n[i];
+    return NUFFT_OK;
+}
 
 // ------------------------------------------------------------------------------------------------------------
 // transforms

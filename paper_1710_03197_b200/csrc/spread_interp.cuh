@@ -127,4 +127,230 @@ gridding_atomic_kernel(SampleData s, GridGeom g, const float2* __restrict__ y, f
     }
 }
 
+
+
+// ============================================================================================================
+// Tiled V^H (step a4): samples are sorted into grid tiles at plan time; a work item is (tile, sample range).  The
+// padded tile (tile + J-1 halo cells per axis) is accumulated in shared memory WITHOUT atomics and flushed once.
+//
+// Shared-memory floating-point atomics are compare-and-swap loops on sm_100a (ATOMS.CAST.SPIN), so accumulation is
+// organised so that no two warps ever touch the same cell:
+//   2-D: every warp owns a private padded tile and walks its own work item sample by sample.  One sample is one
+//        warp instruction group: lane (r, q), r = stencil row 0..5, q = 0..3, read-modify-writes the 16-byte pair of
+//        cells q of row r of an 8-cell window aligned to an even column (24 active lanes, 3 + 3 wavefronts).
+//   3-D: the six warps of a CTA share one padded tile; warp w handles, for every sample, the one stencil plane
+//        whose tile-local index is = w (mod 6).  Planes of different warps are disjoint, so no synchronisation is
+//        needed between samples.
+// Weights are prepared 32 samples at a time, one sample per lane (kb_weights), and staged in shared memory as
+//   rowrec[s][r] = (w_row * y.re, w_row * y.im, cell index of the window start of that row)      16 B
+//   colrec[s][q] = the two column weights of cell pair q (0 outside the 6-cell support)          8 B
+// so that the per-sample loop costs two small broadcast loads, one 16-byte RMW and four FMAs per lane.
+// ============================================================================================================
+struct WorkItem {
+    uint32_t origin;     // tile origin per axis, packed like kpack
+    int32_t s_begin;     // first sorted sample
+    int32_t s_end;       // one past the last
+    int32_t slab;        // deterministic mode: index of this item's private slab
+};
+
+struct TileGeom {
+    int T[3];            // tile size per axis (cells)
+    int P[3];            // padded extents: T + J - 1 (last axis rounded up to even = PITCH)
+    int pitch;           // row pitch of the shared tile in cells (even)
+    int plane;           // plane pitch in cells (3-D), P[1] * pitch
+    int tile_cells;      // cells of one padded tile in shared memory
+};
+
+constexpr int kStageRow = 7;   // float4 slots per sample in rowrec (6 used; 7 keeps 8-lane phases conflict-free)
+constexpr int kStageCol = 5;   // float2 slots per sample in colrec (4 used)
+constexpr int kStageBytes = 32 * (kStageRow * 16 + kStageCol * 8);
+
+// One lane prepares one sample of a 2-D work item.
+__device__ __forceinline__ void stage_sample_2d(const KernelPoly& P, float4* rowrec, float2* colrec, int lane,
+                                                int c0, int c1, float d0, float d1, float2 yv, int pitch, int base_off) {
+    float w0[kJ], w1[kJ];
+    kb_weights(P, d0, w0);
+    kb_weights(P, d1, w1);
+    const int par = c1 & 1, base = base_off + c0 * pitch + (c1 - par);
+#pragma unroll
+    for (int r = 0; r < kJ; ++r)
+        rowrec[lane * kStageRow + r] = make_float4(w0[r] * yv.x, w0[r] * yv.y, __int_as_float(base + r * pitch), 0.f);
+    colrec[lane * kStageCol + 0] = par ? make_float2(0.f, w1[0]) : make_float2(w1[0], w1[1]);
+    colrec[lane * kStageCol + 1] = par ? make_float2(w1[1], w1[2]) : make_float2(w1[2], w1[3]);
+    colrec[lane * kStageCol + 2] = par ? make_float2(w1[3], w1[4]) : make_float2(w1[4], w1[5]);
+    colrec[lane * kStageCol + 3] = par ? make_float2(w1[5], 0.f) : make_float2(0.f, 0.f);
+}
+
+// Apply `cnt` staged samples to the shared tile: lane (r, q) handles cell pair q of stencil row r.
+__device__ __forceinline__ void apply_staged(float2* tile, const float4* rowrec, const float2* colrec, int cnt, int lane) {
+    if (lane >= 24) return;
+    const int r = lane >> 2, q = lane & 3;
+    for (int s = 0; s < cnt; ++s) {
+        const float4 rr = rowrec[s * kStageRow + r];
+        const float2 cc = colrec[s * kStageCol + q];
+        float4* cell = reinterpret_cast<float4*>(tile + __float_as_int(rr.z) + 2 * q);
+        float4 a = *cell;
+        a.x = fmaf(rr.x, cc.x, a.x);
+        a.y = fmaf(rr.y, cc.x, a.y);
+        a.z = fmaf(rr.x, cc.y, a.z);
+        a.w = fmaf(rr.y, cc.y, a.w);
+        *cell = a;
+    }
+}
+
+// Flush a padded tile: pair p of the shared tile goes to grid (atomic add) or to the item's private slab (store).
+template <int D, bool DET>
+__device__ __forceinline__ void flush_tile(const float2* tile, const TileGeom& tg, const GridGeom& g, uint32_t origin,
+                                           float2* __restrict__ G, float2* __restrict__ slab, int tid, int nthreads) {
+    int o[3];
+    unpack_k0(origin, o);
+    const int pairs_per_row = tg.pitch / 2;
+    const int rows = (D == 2) ? tg.P[0] : tg.P[0] * tg.P[1];
+    const int npairs = rows * pairs_per_row;
+    for (int p = tid; p < npairs; p += nthreads) {
+        const float4 v = reinterpret_cast<const float4*>(tile)[p];
+        if (DET) {
+            reinterpret_cast<float4*>(slab)[p] = v;
+        } else {
+            if (v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f) continue;
+            const int row = p / pairs_per_row, cp = p - row * pairs_per_row;
+            const int col = (o[D - 1] + 2 * cp) & (g.K[D - 1] - 1);
+            int64_t gi;
+            if (D == 2) {
+                gi = (int64_t)((o[0] + row) & (g.K[0] - 1)) * g.K[1] + col;
+            } else {
+                const int lz = row / tg.P[1], ly = row - lz * tg.P[1];
+                gi = ((int64_t)((o[0] + lz) & (g.K[0] - 1)) * g.K[1] + ((o[1] + ly) & (g.K[1] - 1))) * g.K[2] + col;
+            }
+            atomicAdd(reinterpret_cast<float4*>(G + gi), v);
+        }
+    }
+}
+
+// 2-D: NW independent warps per CTA, each with a private tile + staging area.
+template <bool DET>
+__global__ void __launch_bounds__(256)
+gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items, int n_items,
+                         const float2* __restrict__ y, float2* __restrict__ grid, float2* __restrict__ slabs,
+                         int64_t slab_batch_stride, KernelPoly P) {
+    extern __shared__ float4 smem4[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int item = blockIdx.x * nw + warp;
+    if (item >= n_items) return;
+    const int b = blockIdx.y;
+    const int per_warp4 = (tg.tile_cells * 8 + kStageBytes) / 16;
+    float2* tile = reinterpret_cast<float2*>(smem4 + (size_t)warp * per_warp4);
+    float4* rowrec = reinterpret_cast<float4*>(tile + tg.tile_cells);
+    float2* colrec = reinterpret_cast<float2*>(rowrec + 32 * kStageRow);
+    const WorkItem wi = items[item];
+    int o[3];
+    unpack_k0(wi.origin, o);
+    for (int i = lane; i < tg.tile_cells / 2; i += 32) reinterpret_cast<float4*>(tile)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+    const float2* __restrict__ yb = y + (int64_t)b * g.M;
+    for (int s0 = wi.s_begin; s0 < wi.s_end; s0 += 32) {
+        const int si = s0 + lane;
+        const int cnt = min(32, wi.s_end - s0);
+        if (si < wi.s_end) {
+            int k0[3];
+            unpack_k0(__ldg(&s.kpack[si]), k0);
+            const float d0 = __ldg(&s.delta[si]), d1 = __ldg(&s.delta[g.M + si]);
+            const float2 yv = __ldg(&yb[__ldg(&s.perm[si])]);
+            stage_sample_2d(P, rowrec, colrec, lane, (k0[0] - o[0]) & (g.K[0] - 1), (k0[1] - o[1]) & (g.K[1] - 1), d0, d1,
+                            yv, tg.pitch, 0);
+        }
+        __syncwarp();
+        apply_staged(tile, rowrec, colrec, cnt, lane);
+        __syncwarp();
+    }
+    flush_tile<2, DET>(tile, tg, g, wi.origin, grid + (int64_t)b * g.cells,
+                       DET ? slabs + (int64_t)b * slab_batch_stride + (int64_t)wi.slab * tg.tile_cells : nullptr, lane, 32);
+}
+
+// 3-D: one work item per CTA of 6 warps; warp w owns the tile-local planes = w (mod 6).
+template <bool DET>
+__global__ void __launch_bounds__(192)
+gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items, int n_items,
+                         const float2* __restrict__ y, float2* __restrict__ grid, float2* __restrict__ slabs,
+                         int64_t slab_batch_stride, KernelPoly P) {
+    extern __shared__ float4 smem4[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.y;
+    float2* tile = reinterpret_cast<float2*>(smem4);
+    float4* rowrec = reinterpret_cast<float4*>(tile + tg.tile_cells) + (size_t)warp * (kStageBytes / 16);
+    float2* colrec = reinterpret_cast<float2*>(rowrec + 32 * kStageRow);
+    const WorkItem wi = items[blockIdx.x];
+    int o[3];
+    unpack_k0(wi.origin, o);
+    for (int i = threadIdx.x; i < tg.tile_cells / 2; i += blockDim.x)
+        reinterpret_cast<float4*>(tile)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+    const float2* __restrict__ yb = y + (int64_t)b * g.M;
+    for (int s0 = wi.s_begin; s0 < wi.s_end; s0 += 32) {
+        const int si = s0 + lane;
+        const int cnt = min(32, wi.s_end - s0);
+        if (si < wi.s_end) {
+            int k0[3];
+            unpack_k0(__ldg(&s.kpack[si]), k0);
+            const float d0 = __ldg(&s.delta[si]), d1 = __ldg(&s.delta[g.M + si]), d2 = __ldg(&s.delta[2 * g.M + si]);
+            const float2 yv = __ldg(&yb[__ldg(&s.perm[si])]);
+            const int c0 = (k0[0] - o[0]) & (g.K[0] - 1), c1 = (k0[1] - o[1]) & (g.K[1] - 1);
+            const int c2 = (k0[2] - o[2]) & (g.K[2] - 1);
+            // this warp's plane of the sample: tile-local plane c0 + j0 = warp (mod 6)
+            const int j0 = (warp - c0 % 6 + 6) % 6;
+            float wz[kJ];
+            kb_weights(P, d0, wz);
+            float wsel = wz[0];
+#pragma unroll
+            for (int j = 1; j < kJ; ++j) wsel = (j0 == j) ? wz[j] : wsel;
+            stage_sample_2d(P, rowrec, colrec, lane, c1, c2, d1, d2, cscale(yv, wsel), tg.pitch, (c0 + j0) * tg.plane);
+        }
+        __syncwarp();
+        apply_staged(tile, rowrec, colrec, cnt, lane);
+        __syncwarp();
+    }
+    __syncthreads();
+    flush_tile<3, DET>(tile, tg, g, wi.origin, grid + (int64_t)b * g.cells,
+                       DET ? slabs + (int64_t)b * slab_batch_stride + (int64_t)wi.slab * tg.tile_cells : nullptr,
+                       threadIdx.x, blockDim.x);
+}
+
+// Deterministic merge: every grid cell sums, in fixed order, the slabs of the work items whose padded tile covers it.
+// tile_item_start[t] .. tile_item_start[t+1] are the slabs of tile t (work items of one tile are contiguous).
+template <int D>
+__global__ void __launch_bounds__(256)
+gridding_merge_kernel(GridGeom g, TileGeom tg, int nt0, int nt1, int nt2, const int32_t* __restrict__ tile_item_start,
+                      const float2* __restrict__ slabs, int64_t slab_batch_stride, float2* __restrict__ grid) {
+    const int64_t cell = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= g.cells) return;
+    const int b = blockIdx.y;
+    int c[3];
+    if (D == 2) { c[0] = (int)(cell / g.K[1]); c[1] = (int)(cell % g.K[1]); c[2] = 0; }
+    else { c[2] = (int)(cell % g.K[2]); const int64_t q = cell / g.K[2]; c[1] = (int)(q % g.K[1]); c[0] = (int)(q / g.K[1]); }
+    const int nt[3] = {nt0, nt1, nt2};
+    // per axis: the tile containing the cell, and (if the cell lies in the first J-1 cells of it) the previous tile
+    int t[3][2], l[3][2], n[3];
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        const int ti = c[a] / tg.T[a], li = c[a] - ti * tg.T[a];
+        // previous tile first (fixed order): its local index is li + T
+        n[a] = 0;
+        if (li < kJ - 1) {
+            t[a][n[a]] = (ti + nt[a] - 1) % nt[a]; l[a][n[a]] = li + tg.T[a]; n[a]++;
+        }
+        t[a][n[a]] = ti; l[a][n[a]] = li; n[a]++;
+    }
+    const float2* __restrict__ S = slabs + (int64_t)b * slab_batch_stride;
+    float2 acc = make_float2(0.f, 0.f);
+    for (int i0 = 0; i0 < n[0]; ++i0)
+        for (int i1 = 0; i1 < n[1]; ++i1)
+            for (int i2 = 0; i2 < (D == 3 ? n[2] : 1); ++i2) {
+                int tid_, off;
+                if (D == 2) { tid_ = t[0][i0] * nt1 + t[1][i1]; off = l[0][i0] * tg.pitch + l[1][i1]; }
+                else { tid_ = (t[0][i0] * nt1 + t[1][i1]) * nt2 + t[2][i2]; off = l[0][i0] * tg.plane + l[1][i1] * tg.pitch + l[2][i2]; }
+                for (int w = tile_item_start[tid_]; w < tile_item_start[tid_ + 1]; ++w)
+                    acc = cadd(acc, S[(int64_t)w * tg.tile_cells + off]);
+            }
+    grid[(int64_t)b * g.cells + cell] = acc;
+}
 }  // namespace nufft

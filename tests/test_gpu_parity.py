@@ -216,9 +216,9 @@ def test_adjoint_identity_on_gpu():
     y = wl.data_gaussian(cfg["om"].shape[0])
     Ax = host(p.forward(dev(x)))[0].astype(np.complex128)
     AHy = host(p.adjoint(dev(y)))[0].astype(np.complex128)
-    lhs = np.vdot(y.astype(np.complex128), Ax)
-    rhs = np.vdot(AHy.ravel(), x.astype(np.complex128).ravel())
-    assert abs(lhs - np.conj(rhs)) / abs(lhs) < 1e-5
+    lhs = np.vdot(Ax, y.astype(np.complex128))                          # <Ax, y>
+    rhs = np.vdot(x.astype(np.complex128).ravel(), AHy.ravel())         # <x, A^H y>
+    assert abs(lhs - rhs) / abs(lhs) < 1e-5
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -243,9 +243,9 @@ def test_config4_full_size_sampled():
     ref = orc.interp(G, om[sel], Nd, Kd, Jd)
     assert rel(Ax[sel], ref) < TOL
     # adjoint: identity <Ax, y> = <x, A^H y> with the GPU forward already validated above
-    lhs = np.vdot(y.astype(np.complex128), Ax.astype(np.complex128))
-    rhs = np.vdot(AHy.astype(np.complex128).ravel(), x.astype(np.complex128).ravel())
-    assert abs(lhs - np.conj(rhs)) / abs(lhs) < 2e-5
+    lhs = np.vdot(Ax.astype(np.complex128), y.astype(np.complex128))
+    rhs = np.vdot(x.astype(np.complex128).ravel(), AHy.astype(np.complex128).ravel())
+    assert abs(lhs - rhs) / abs(lhs) < 2e-5
     # adjoint: sampled voxels against the plain definition (brute force over all M samples)
     vox = [(0, 0, 0), (64, 64, 64), (127, 127, 127), (5, 100, 77), (64, 0, 127)]
     for v in vox:
