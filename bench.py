@@ -315,7 +315,7 @@ def run_ours(args):
             "stages_ms": {
                 "F (S+pad+FFT)": stage_of(rows, ["fft_rows_fwd", "fft_cols_fwd"]),
                 "V": stage_of(rows, ["interp"]),
-                "V^H": stage_of(rows, ["grid_zero", "gridding", "gridding_merge"]),
+                "V^H": stage_of(rows, ["y_gather", "grid_zero", "gridding", "gridding_merge"]),
                 "F^H (IFFT+crop+S^H)": stage_of(rows, ["fft_cols_adj", "fft_rows_adj"]),
             },
             "note": "2-D grids of this batch are partly L2-resident between kernels of one step; V and V^H are "
@@ -327,7 +327,8 @@ def run_ours(args):
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
             "config": {"workload": WORKLOAD, "batch": B, "pairs_per_step": B, "l2": "flushed between steps (256 MiB memset)",
-                       "parallelism": "replicas x%d" % world, "adjoint_mode": 0},
+                       "parallelism": "replicas x%d" % world, "adjoint_mode": 0,
+                       "batch_layout": "interleaved [group][K0][K1][32] (batch >= 16)" if B >= 16 else "planar"},
             "clocks": clocks,
             "e2e": {"value": world * B / (e2e_ms / K_steps * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": int(x_host.numel() * 8), "d2h_bytes_per_step": int(xo_host.numel() * 8),

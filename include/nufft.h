@@ -65,6 +65,11 @@ typedef struct {
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
     int use_graphs;     /* 1 = capture forward/adjoint/selfadjoint into CUDA graphs on first use (default 0)     */
+    int batch_layout;   /* workspace layout of batched 2-D transforms (PAPER.md:52 batch mode, :251-258 coils):
+                           0 = auto: calls with batch >= 16 use the batch-interleaved grid [group][K0][K1][32]
+                               (lanes = images; V^H in gather form with register accumulators, deterministic),
+                               smaller batches and 3-D use the planar grid [batch][K0][K1]([K2]);
+                           1 = always planar                                                                      */
 } nufft_opts;
 
 int nufft_default_opts(nufft_opts *o);

@@ -26,7 +26,8 @@ EXPORTED_SYMBOLS = [
 
 class NufftOpts(_c.Structure):
     _fields_ = [("coef_mode", _c.c_int), ("adjoint_mode", _c.c_int), ("interp_mode", _c.c_int),
-                ("tile", _c.c_int * 3), ("max_subtile", _c.c_int), ("use_graphs", _c.c_int)]
+                ("tile", _c.c_int * 3), ("max_subtile", _c.c_int), ("use_graphs", _c.c_int),
+                ("batch_layout", _c.c_int)]
 
 
 class NufftError(RuntimeError):
@@ -122,7 +123,8 @@ class NufftPlan:
     what bench.py's `e2e` leg times.
     """
 
-    def __init__(self, Nd, Kd, Jd, om, max_batch=1, adjoint_mode=0, interp_mode=0, tile=None, max_subtile=0):
+    def __init__(self, Nd, Kd, Jd, om, max_batch=1, adjoint_mode=0, interp_mode=0, tile=None, max_subtile=0,
+                 batch_layout=0):
         L = lib()
         self.Nd = tuple(int(n) for n in Nd)
         self.Kd = tuple(int(k) for k in Kd)
@@ -141,6 +143,7 @@ class NufftPlan:
         opts.adjoint_mode = int(adjoint_mode)
         opts.interp_mode = int(interp_mode)
         opts.max_subtile = int(max_subtile)
+        opts.batch_layout = int(batch_layout)
         if tile is not None:
             for a, t in enumerate(tile):
                 opts.tile[a] = int(t)

@@ -1,0 +1,284 @@
+// batch_il.cuh -- the batch-interleaved 2-D path (steps a1..a6 and a8 of SURVEY.md 8(a) for batches >= 16 images that
+// share one trajectory: the paper's batch mode PAPER.md:52 and the multi-coil operator PAPER.md:251-258).
+//
+// Why a second layout.  At J = 6 every sample touches 36 complex64 grid cells; with a planar grid and one thread per
+// sample that is 36 loads of ~21 sectors per warp and the L1 data pipe saturates (profiles/r01b: l1tex 96 %).  Here
+// the workspace grid is stored as  grid_il[group][K0][K1][32]  (32 images of a group side by side, 256 contiguous
+// bytes per grid cell) and LANES ARE IMAGES: one warp load fetches one stencil point of 32 images as two full 128-B
+// lines, interpolation weights are warp-uniform, and nothing is gathered per lane.
+//
+//   F   rows: fft_il_rows_{fwd,adj}_kernel  planar image <-> interleaved grid (S, zero-pad / crop, coil multiply fused)
+//       cols: the generic strided pass fft_cols_kernel over [K0][K1*32]
+//   V   interp_il_kernel     one warp = 32 consecutive cell-sorted samples x 32 images
+//   V^H gridding_il_kernel   GATHER form, accumulation in REGISTERS: warp = one grid row x 8 columns x 32 images;
+//                            it walks the samples whose stencil covers that row (contiguous ranges of the
+//                            cell-sorted order, found through rowptr) and adds w0 * w1 * y.  No atomics, no
+//                            shared-memory read-modify-write, no zero-fill; every grid cell is written exactly once,
+//                            in a fixed summation order (bit-reproducible).
+#pragma once
+#include "common.cuh"
+#include "fft.cuh"
+#include "spread_interp.cuh"
+
+namespace nufft {
+
+constexpr int kIL = 32;      // images per interleaved group (= lanes per warp)
+constexpr int kBandW = 8;    // grid columns per V^H band (accumulators per lane: kBandW complex)
+constexpr int kTabW = 24;    // floats per sample in the V^H weight table: w0[6], 2 pad, w1 band-aligned A[8], B[8]
+
+// ------------------------------------------------------------------------------------------------------------
+// FFT row passes between the caller's planar images and the interleaved grid
+// ------------------------------------------------------------------------------------------------------------
+struct IlRowParams {
+    const float2* img_in;     // forward: x [batch][N0][N1]
+    float2* img_out;          // adjoint: x [batch][N0][N1]
+    float2* grid;             // grid_il [groups][K0][K1][32]
+    const float2* coil;       // optional [batch][N0][N1]
+    const float* s_outer;     // scaling vector of axis 0 (length N0)
+    const float* s_line;      // scaling vector of axis 1 (length N1)
+    const float2* tw;         // twiddles of length K1
+    int n_outer, k_outer;     // N0, K0
+    int batch;                // images present (lanes >= batch of the last group are idle)
+    int same_image;           // forward: every batch item reads image 0 (multi-coil forward)
+};
+
+// a1 + first pass of a2: x (scaled, circularly zero-padded) -> FFT along axis 1 -> grid_il rows
+// CTA = T images of one image row; thread (t, q0) works on image t.
+template <int K>
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
+fft_il_rows_fwd_kernel(IlRowParams p) {
+    constexpr int N = K / 2, T = Rad<K>::TS;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, q0 = threadIdx.x / T;
+    const int n0 = blockIdx.x % p.n_outer;
+    const int b = (blockIdx.x / p.n_outer) * T + t;
+    const bool active = b < p.batch;
+    const int bb = active ? b : 0;
+    const int g0 = (n0 - p.n_outer / 2) & (p.k_outer - 1);
+    const float2* __restrict__ src = p.img_in + ((int64_t)(p.same_image ? 0 : bb) * p.n_outer + n0) * N;
+    const float2* __restrict__ csrc = p.coil ? p.coil + ((int64_t)bb * p.n_outer + n0) * N : nullptr;
+    float2* __restrict__ dst = p.grid + (((int64_t)(b / kIL) * p.k_outer + g0) * K) * kIL + (b % kIL);
+    const float so = __ldg(&p.s_outer[n0]);
+    const float* __restrict__ sl = p.s_line;
+    LayStrided<K, T> lay{smem + t};
+    auto ld = [&](int i) -> float2 {
+        const int n = (i + N / 2) & (K - 1);
+        float2 xv = __ldg(&src[n]);
+        if (csrc) xv = cmul(xv, __ldg(&csrc[n]));
+        return cscale(xv, so * __ldg(&sl[n]));
+    };
+    auto st = [&](int i, float2 v) { dst[(int64_t)i * kIL] = v; };
+    fft_line<K, true, false>(q0, active, lay, p.tw, ld, st);
+}
+
+// last pass of a5 + a6: grid_il rows -> inverse FFT along axis 1 -> crop -> S^H (-> conj(coil)) -> planar images
+template <int K>
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
+fft_il_rows_adj_kernel(IlRowParams p) {
+    constexpr int N = K / 2, T = Rad<K>::TS;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, q0 = threadIdx.x / T;
+    const int n0 = blockIdx.x % p.n_outer;
+    const int b = (blockIdx.x / p.n_outer) * T + t;
+    const bool active = b < p.batch;
+    const int bb = active ? b : 0;
+    const int g0 = (n0 - p.n_outer / 2) & (p.k_outer - 1);
+    const float2* __restrict__ src = p.grid + (((int64_t)(b / kIL) * p.k_outer + g0) * K) * kIL + (b % kIL);
+    float2* __restrict__ dst = p.img_out + ((int64_t)bb * p.n_outer + n0) * N;
+    const float2* __restrict__ csrc = p.coil ? p.coil + ((int64_t)bb * p.n_outer + n0) * N : nullptr;
+    const float so = __ldg(&p.s_outer[n0]);
+    const float* __restrict__ sl = p.s_line;
+    LayStrided<K, T> lay{smem + t};
+    auto ld = [&](int i) -> float2 { return cconj(src[(int64_t)i * kIL]); };
+    auto st = [&](int i, float2 v) {
+        const int n = (i + N / 2) & (K - 1);
+        float2 r = cscale(cconj(v), so * __ldg(&sl[n]));
+        if (csrc) r = cmul(r, cconj(__ldg(&csrc[n])));
+        dst[n] = r;
+    };
+    fft_line<K, false, true>(q0, active, lay, p.tw, ld, st);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// plan data of the interleaved path: samples in CELL-SORTED order, key = (column band, row k0_0, 7 - (k0_1 mod 8))
+// ------------------------------------------------------------------------------------------------------------
+struct IlPlan {
+    const uint32_t* kpack;    // stencil base index per axis (10 bits each), sorted order
+    const float* delta;       // [2][M]
+    const int32_t* perm;      // sorted position -> caller's sample index
+    const float* wtab;        // [M][kTabW] V^H weight table (float64-built)
+    const int32_t* rowptr;    // [K1/8][K0 + 1]: first sorted sample of (band, row)
+    const int32_t* rowsplit;  // [K1/8][K0]: samples of (band, row) whose stencil reaches into the next band (they come first)
+};
+
+// a3: y = V grid.  One warp = 32 consecutive sorted samples x the 32 images of group blockIdx.y.
+// Each lane prepares the weights of one sample (kb_weights) and stages them in shared memory; the warp then walks
+// the samples one by one with warp-uniform weights: 36 loads of 256 contiguous bytes and 72 + 12 FMAs per lane.
+// SORTED_OUT: y is written as y_il[group][sorted sample][32] (selfadjoint intermediate) instead of y[b][perm].
+template <bool SORTED_OUT>
+__global__ void __launch_bounds__(256)
+interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y, int batch,
+                 KernelPoly P) {
+    __shared__ float4 wrec[8][32 * 4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = blockIdx.y;
+    const int64_t s0 = ((int64_t)blockIdx.x * 8 + warp) * 32;
+    if (s0 >= g.M) return;
+    const int cnt = (int)min((int64_t)32, g.M - s0);
+    if (lane < cnt) {
+        const int64_t si = s0 + lane;
+        const uint32_t kp = __ldg(&s.kpack[si]);
+        float w0[kJ], w1[kJ];
+        kb_weights(P, __ldg(&s.delta[si]), w0);
+        kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
+        float4* r = &wrec[warp][lane * 4];
+        r[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
+        r[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
+        r[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
+        r[3] = make_float4(__int_as_float((int)(kp & 1023u)), __int_as_float((int)((kp >> 10) & 1023u)),
+                           __int_as_float(SORTED_OUT ? 0 : __ldg(&s.perm[si])), 0.f);
+    }
+    __syncwarp();
+    const int K0 = g.K[0], K1 = g.K[1];
+    const float2* __restrict__ G = grid_il + (int64_t)grp * g.cells * kIL + lane;
+    const int b = grp * kIL + lane;
+    for (int sidx = 0; sidx < cnt; ++sidx) {
+        const float4 ra = wrec[warp][sidx * 4 + 0], rb = wrec[warp][sidx * 4 + 1];
+        const float4 rc = wrec[warp][sidx * 4 + 2], rd = wrec[warp][sidx * 4 + 3];
+        const float w0[kJ] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y};
+        const float w1[kJ] = {rb.z, rb.w, rc.x, rc.y, rc.z, rc.w};
+        const int r0 = __float_as_int(rd.x), c0 = __float_as_int(rd.y);
+        float2 acc = make_float2(0.f, 0.f);
+        if (c0 + kJ <= K1) {
+#pragma unroll
+            for (int j0 = 0; j0 < kJ; ++j0) {
+                const float2* __restrict__ pr = G + ((int64_t)((r0 + j0) & (K0 - 1)) * K1 + c0) * kIL;
+                float2 r = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int j1 = 0; j1 < kJ; ++j1) {
+                    const float2 v = __ldg(pr + j1 * kIL);
+                    r.x = fmaf(w1[j1], v.x, r.x);
+                    r.y = fmaf(w1[j1], v.y, r.y);
+                }
+                acc.x = fmaf(w0[j0], r.x, acc.x);
+                acc.y = fmaf(w0[j0], r.y, acc.y);
+            }
+        } else {      // stencil crosses the periodic seam of axis 1
+#pragma unroll
+            for (int j0 = 0; j0 < kJ; ++j0) {
+                const float2* __restrict__ pr = G + (int64_t)((r0 + j0) & (K0 - 1)) * K1 * kIL;
+                float2 r = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int j1 = 0; j1 < kJ; ++j1) {
+                    const float2 v = __ldg(pr + (int64_t)((c0 + j1) & (K1 - 1)) * kIL);
+                    r.x = fmaf(w1[j1], v.x, r.x);
+                    r.y = fmaf(w1[j1], v.y, r.y);
+                }
+                acc.x = fmaf(w0[j0], r.x, acc.x);
+                acc.y = fmaf(w0[j0], r.y, acc.y);
+            }
+        }
+        if (SORTED_OUT) y[((int64_t)grp * g.M + s0 + sidx) * kIL + lane] = acc;
+        else if (b < batch) y[(int64_t)b * g.M + __float_as_int(rd.z)] = acc;
+    }
+}
+
+// y (caller's order, [batch][M]) -> y_il[group][sorted sample][32]; idle lanes of the last group get zeros.
+__global__ void __launch_bounds__(128)
+y_gather_il_kernel(const int32_t* __restrict__ perm, const float2* __restrict__ y, float2* __restrict__ y_il, int64_t M,
+                   int batch) {
+    __shared__ float2 tile[4][32][33];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = blockIdx.y;
+    const int64_t s0 = ((int64_t)blockIdx.x * 4 + warp) * 32;
+    if (s0 >= M) return;
+    const int cnt = (int)min((int64_t)32, M - s0);
+    const int64_t pm = (lane < cnt) ? (int64_t)__ldg(&perm[s0 + lane]) : -1;
+#pragma unroll 4
+    for (int l = 0; l < kIL; ++l) {
+        const int b = grp * kIL + l;
+        tile[warp][lane][l] = (pm >= 0 && b < batch) ? __ldg(&y[(int64_t)b * M + pm]) : make_float2(0.f, 0.f);
+    }
+    __syncwarp();
+    float2* __restrict__ dst = y_il + ((int64_t)grp * M + s0) * kIL + lane;
+    for (int sidx = 0; sidx < cnt; ++sidx) dst[(int64_t)sidx * kIL] = tile[warp][sidx][lane];
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a4: grid = V^H y, gather form with register accumulators (see the header of this file)
+// ------------------------------------------------------------------------------------------------------------
+struct IlItem {
+    int32_t cb;       // column band: grid columns 8 cb .. 8 cb + 7
+    int32_t r0;       // first grid row of the item
+    int32_t nrows;    // 8, 4, 2 or 1 rows; the 8 warps of the CTA split each row's sample list 8 / nrows ways
+    int32_t load;     // row-sample interactions of the item (plan-time cost estimate; sort key)
+};
+
+template <int OFF>
+__device__ __forceinline__ void il_accumulate(float2 (&acc)[kBandW], const float* __restrict__ wtab,
+                                              const float2* __restrict__ Y, int j0, int b, int e) {
+#pragma unroll 2
+    for (int i = b; i < e; ++i) {
+        const float* __restrict__ rec = wtab + (int64_t)i * kTabW;
+        const float w0 = __ldg(rec + j0);
+        const float4 pa = __ldg(reinterpret_cast<const float4*>(rec + OFF));
+        const float4 pb = __ldg(reinterpret_cast<const float4*>(rec + OFF + 4));
+        const float2 yv = __ldg(Y + (int64_t)i * kIL);
+        const float tx = w0 * yv.x, ty = w0 * yv.y;
+        acc[0].x = fmaf(pa.x, tx, acc[0].x); acc[0].y = fmaf(pa.x, ty, acc[0].y);
+        acc[1].x = fmaf(pa.y, tx, acc[1].x); acc[1].y = fmaf(pa.y, ty, acc[1].y);
+        acc[2].x = fmaf(pa.z, tx, acc[2].x); acc[2].y = fmaf(pa.z, ty, acc[2].y);
+        acc[3].x = fmaf(pa.w, tx, acc[3].x); acc[3].y = fmaf(pa.w, ty, acc[3].y);
+        acc[4].x = fmaf(pb.x, tx, acc[4].x); acc[4].y = fmaf(pb.x, ty, acc[4].y);
+        acc[5].x = fmaf(pb.y, tx, acc[5].x); acc[5].y = fmaf(pb.y, ty, acc[5].y);
+        acc[6].x = fmaf(pb.z, tx, acc[6].x); acc[6].y = fmaf(pb.z, ty, acc[6].y);
+        acc[7].x = fmaf(pb.w, tx, acc[7].x); acc[7].y = fmaf(pb.w, ty, acc[7].y);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const float2* __restrict__ y_il,
+                   float2* __restrict__ grid_il) {
+    __shared__ float2 red[8][kBandW][kIL];
+    const IlItem it = items[blockIdx.x];
+    const int grp = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nsplit = 8 / it.nrows;
+    const int row = it.r0 + warp / nsplit, part = warp % nsplit;
+    const int K0 = g.K[0], K1 = g.K[1], nb = K1 / kBandW;
+    const int cbp = (it.cb + nb - 1) % nb;
+    const float2* __restrict__ Y = y_il + (int64_t)grp * g.M * kIL + lane;
+    float2 acc[kBandW];
+#pragma unroll
+    for (int c = 0; c < kBandW; ++c) acc[c] = make_float2(0.f, 0.f);
+#pragma unroll 1
+    for (int j0 = 0; j0 < kJ; ++j0) {
+        const int r = (row - j0) & (K0 - 1);
+        {   // samples of this band: columns relative to the band start, table part A
+            const int b = __ldg(&s.rowptr[it.cb * (K0 + 1) + r]), n = __ldg(&s.rowptr[it.cb * (K0 + 1) + r + 1]) - b;
+            il_accumulate<8>(acc, s.wtab, Y, j0, b + (int)((int64_t)n * part / nsplit),
+                             b + (int)((int64_t)n * (part + 1) / nsplit));
+        }
+        {   // samples of the previous band whose stencil reaches into this one: table part B
+            const int b = __ldg(&s.rowptr[cbp * (K0 + 1) + r]), n = __ldg(&s.rowsplit[cbp * K0 + r]);
+            il_accumulate<16>(acc, s.wtab, Y, j0, b + (int)((int64_t)n * part / nsplit),
+                              b + (int)((int64_t)n * (part + 1) / nsplit));
+        }
+    }
+    if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row
+#pragma unroll
+        for (int c = 0; c < kBandW; ++c) red[warp][c][lane] = acc[c];
+        __syncthreads();
+        if (part != 0) return;
+        for (int q = 1; q < nsplit; ++q)
+#pragma unroll
+            for (int c = 0; c < kBandW; ++c) acc[c] = cadd(acc[c], red[warp + q][c][lane]);
+    }
+    float2* __restrict__ dst = grid_il + (((int64_t)grp * K0 + row) * K1 + it.cb * kBandW) * kIL + lane;
+#pragma unroll
+    for (int c = 0; c < kBandW; ++c) dst[c * kIL] = acc[c];
+}
+
+// x[n] = sum_b img[b][n]  is done by coil_sum_kernel (solver.cuh).
+
+}  // namespace nufft

@@ -14,6 +14,7 @@
 #include "plan.hpp"
 #include "solver.cuh"
 #include "spread_interp.cuh"
+#include "batch_il.cuh"
 
 using namespace nufft;
 
@@ -70,6 +71,18 @@ struct nufft_plan_s {
     int64_t n_tiles = 0, n_work = 0, max_tile_samples = 0;
     int64_t bytes_plan = 0, bytes_work = 0;
     int64_t launches = 0;
+    // batch-interleaved 2-D path (batch_il.cuh): cell-sorted plan data, V^H weight table, row pointers, work items
+    bool il_ok = false;
+    int batch_pad = 1;              // max_batch rounded up to whole groups of 32 when il_ok
+    uint32_t* d_il_kpack = nullptr;
+    float* d_il_delta = nullptr;
+    int32_t* d_il_perm = nullptr;
+    float* d_il_wtab = nullptr;
+    int32_t* d_il_rowptr = nullptr;
+    int32_t* d_il_rowsplit = nullptr;
+    IlItem* d_il_items = nullptr;
+    int n_il_items = 0;
+    float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
     // optional per-kernel event timing (nufft_profile_*)
     bool prof_on = false;
     struct ProfRec { int label; cudaEvent_t a, b; };
@@ -118,6 +131,10 @@ template <int K> static cudaError_t configure_fft() {
     e = cudaFuncSetAttribute(fft_cols_kernel<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_cols_kernel<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_il_rows_fwd_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_il_rows_adj_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     return e;
 }
 
@@ -333,6 +350,111 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
     return NUFFT_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------------------------
+// batch-interleaved 2-D path (batch_il.cuh)
+// ------------------------------------------------------------------------------------------------------------
+static bool use_il(nufft_plan_t p, int batch) { return p->il_ok && batch >= 16; }
+static int il_groups(int batch) { return (batch + kIL - 1) / kIL; }
+
+template <int K> static void launch_il_rows(bool adj, const IlRowParams& p, int blocks, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
+    if (adj) fft_il_rows_adj_kernel<K><<<blocks, threads, smem_cols<K>(), st>>>(p);
+    else     fft_il_rows_fwd_kernel<K><<<blocks, threads, smem_cols<K>(), st>>>(p);
+}
+static int dispatch_il_rows(int K, bool adj, const IlRowParams& p, cudaStream_t st) {
+    const int T = tile_T(K);
+    if (T == 0) return NUFFT_EINVAL;
+    const int blocks = ((il_groups(p.batch) * kIL) / T) * p.n_outer;
+    switch (K) {
+        case 32: launch_il_rows<32>(adj, p, blocks, st); break;
+        case 64: launch_il_rows<64>(adj, p, blocks, st); break;
+        case 128: launch_il_rows<128>(adj, p, blocks, st); break;
+        case 256: launch_il_rows<256>(adj, p, blocks, st); break;
+        case 512: launch_il_rows<512>(adj, p, blocks, st); break;
+        case 1024: launch_il_rows<1024>(adj, p, blocks, st); break;
+        default: return NUFFT_EINVAL;
+    }
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+static IlRowParams il_row_params(nufft_plan_t p, int batch, const float2* img_in, float2* img_out, float2* grid,
+                                 const float2* coil, bool same_image) {
+    IlRowParams r{};
+    r.img_in = img_in; r.img_out = img_out; r.grid = grid; r.coil = coil;
+    r.s_outer = p->d_scale[0]; r.s_line = p->d_scale[1]; r.tw = p->d_tw[1];
+    r.n_outer = p->N[0]; r.k_outer = p->K[0]; r.batch = batch; r.same_image = same_image ? 1 : 0;
+    return r;
+}
+static ColPassParams il_col_params(nufft_plan_t p, int batch, float2* grid) {
+    ColPassParams c{};
+    c.grid = grid; c.tw = p->d_tw[0];
+    c.batch_stride = p->cells * kIL; c.outer_stride = 0; c.line_stride = (int64_t)p->K[1] * kIL;
+    c.n_outer = 1; c.k_outer = 0; c.inner = p->K[1] * kIL;
+    c.ngroups = il_groups(batch) * (c.inner / tile_T(p->K[0]));
+    return c;
+}
+static IlPlan il_plan(nufft_plan_t p) {
+    IlPlan s{};
+    s.kpack = p->d_il_kpack; s.delta = p->d_il_delta; s.perm = p->d_il_perm; s.wtab = p->d_il_wtab;
+    s.rowptr = p->d_il_rowptr; s.rowsplit = p->d_il_rowsplit;
+    return s;
+}
+
+// a1 + a2 on the interleaved grid
+static int run_scale_fft_il(nufft_plan_t p, int batch, const float2* x, float2* grid, const float2* coil,
+                            bool same_image, cudaStream_t st) {
+    IlRowParams r = il_row_params(p, batch, x, nullptr, grid, coil, same_image);
+    { ProfScope ps(p, "fft_rows_fwd", st); NU_TRY(dispatch_il_rows(p->K[1], false, r, st)); }
+    { ProfScope ps(p, "fft_cols_fwd", st); NU_TRY(dispatch_cols(p->K[0], false, il_col_params(p, batch, grid), st)); }
+    p->launches += 2;
+    return NUFFT_OK;
+}
+// a5 + a6 on the interleaved grid
+static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
+    { ProfScope ps(p, "fft_cols_adj", st); NU_TRY(dispatch_cols(p->K[0], true, il_col_params(p, batch, grid), st)); }
+    IlRowParams r = il_row_params(p, batch, nullptr, x, grid, coil, false);
+    { ProfScope ps(p, "fft_rows_adj", st); NU_TRY(dispatch_il_rows(p->K[1], true, r, st)); }
+    p->launches += 2;
+    return NUFFT_OK;
+}
+// a3: sorted_out = false: y[batch][M] in the caller's order; true: y_il[group][sorted sample][32]
+static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* y, bool sorted_out, cudaStream_t st) {
+    if (p->M == 0) return NUFFT_OK;
+    const dim3 blocks((unsigned)((p->M + 255) / 256), (unsigned)il_groups(batch));
+    ProfScope ps(p, "interp", st);
+    if (sorted_out) interp_il_kernel<true><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
+    else            interp_il_kernel<false><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+// caller's y -> y_il
+static int run_y_gather_il(nufft_plan_t p, int batch, const float2* y, cudaStream_t st) {
+    if (p->M == 0) return NUFFT_OK;
+    if (!p->d_yil)
+        NU_TRY(dev_alloc((void**)&p->d_yil, (size_t)p->batch_pad * p->M * sizeof(float2), &p->bytes_work));
+    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)il_groups(batch));
+    ProfScope ps(p, "y_gather", st);
+    y_gather_il_kernel<<<blocks, 128, 0, st>>>(p->d_il_perm, y, p->d_yil, p->M, batch);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+// a4 from y_il
+static int run_gridding_il(nufft_plan_t p, int batch, const float2* y_il, float2* grid, cudaStream_t st) {
+    if (p->M == 0) {
+        CU_TRY(cudaMemsetAsync(grid, 0, (size_t)il_groups(batch) * kIL * p->cells * sizeof(float2), st));
+        return NUFFT_OK;
+    }
+    const dim3 blocks((unsigned)p->n_il_items, (unsigned)il_groups(batch));
+    ProfScope ps(p, "gridding", st);
+    gridding_il_kernel<<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------------------------
@@ -359,6 +481,101 @@ static int dev_alloc(void** dptr, size_t bytes, int64_t* acct) {
 extern "C" int nufft_default_opts(nufft_opts* o) {
     if (!o) return NUFFT_EINVAL;
     std::memset(o, 0, sizeof(*o));
+    return NUFFT_OK;
+}
+
+// Plan data of the batch-interleaved path (batch_il.cuh): cell-sorted sample order, V^H weight table (float64-built),
+// row pointers per column band, V^H work items.
+static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, const std::vector<float>& delta,
+                         const std::vector<double>& delta64) {
+    const int64_t M = p->M;
+    const int K0 = p->K[0], K1 = p->K[1], nb = K1 / kBandW;
+    const double J = (double)kJ, beta = host::kb_beta(J, 2.0);
+    // counting sort, key = ((band * K0 + row) * 8 + (7 - column offset in the band))
+    const int64_t nbins = (int64_t)nb * K0 * kBandW;
+    std::vector<int32_t> binstart(nbins + 1, 0);
+    auto key_of = [&](uint32_t kp) -> int64_t {
+        const int r = kp & 1023u, c = (kp >> 10) & 1023u;
+        return ((int64_t)(c / kBandW) * K0 + r) * kBandW + (kBandW - 1 - (c % kBandW));
+    };
+    for (int64_t m = 0; m < M; ++m) binstart[key_of(kpack[m]) + 1]++;
+    for (int64_t b = 0; b < nbins; ++b) binstart[b + 1] += binstart[b];
+    std::vector<int32_t> perm(M);
+    {
+        std::vector<int32_t> cur(binstart.begin(), binstart.end() - 1);
+        for (int64_t m = 0; m < M; ++m) perm[cur[key_of(kpack[m])]++] = (int32_t)m;
+    }
+    std::vector<uint32_t> kp_s(M);
+    std::vector<float> dl_s((size_t)2 * M);
+    std::vector<float> wtab((size_t)M * kTabW, 0.f);
+    for (int64_t i = 0; i < M; ++i) {
+        const int64_t m = perm[i];
+        kp_s[i] = kpack[m];
+        dl_s[i] = delta[m];
+        dl_s[M + i] = delta[M + m];
+        double w0[kJ], w1[kJ];
+        host::kb_weights_f64(delta64[m], J, beta, w0);
+        host::kb_weights_f64(delta64[M + m], J, beta, w1);
+        float* rec = &wtab[(size_t)i * kTabW];
+        for (int j = 0; j < kJ; ++j) rec[j] = (float)w0[j];
+        const int off = ((kpack[m] >> 10) & 1023u) % kBandW;
+        for (int j = 0; j < kJ; ++j) {
+            const int c = off + j;                       // column relative to the start of the sample's own band
+            if (c < kBandW) rec[8 + c] = (float)w1[j];   // part A: this band
+            else rec[16 + c - kBandW] = (float)w1[j];    // part B: the next band
+        }
+    }
+    // row pointers; rowsplit = samples of (band, row) with column offset >= 3 (stencil reaches the next band)
+    std::vector<int32_t> rowptr((size_t)nb * (K0 + 1)), rowsplit((size_t)nb * K0);
+    for (int cb = 0; cb < nb; ++cb) {
+        for (int r = 0; r <= K0; ++r) {
+            const int64_t bin = ((int64_t)cb * K0 + std::min(r, K0 - 1)) * kBandW + (r == K0 ? kBandW : 0);
+            rowptr[(size_t)cb * (K0 + 1) + r] = binstart[bin];
+        }
+        for (int r = 0; r < K0; ++r) {
+            const int64_t bin = ((int64_t)cb * K0 + r) * kBandW;
+            rowsplit[(size_t)cb * K0 + r] = binstart[bin + (kBandW - 3)] - binstart[bin];   // offsets 7,6,5,4,3
+        }
+    }
+    // work items: blocks of 8 rows; rows whose interaction count is far above the mean are split among warps
+    std::vector<int64_t> rowload((size_t)nb * K0);
+    int64_t total = 0;
+    for (int cb = 0; cb < nb; ++cb) {
+        const int cbp = (cb + nb - 1) % nb;
+        for (int r = 0; r < K0; ++r) {
+            int64_t l = 0;
+            for (int j0 = 0; j0 < kJ; ++j0) {
+                const int rr = (r - j0 + K0) % K0;
+                l += rowptr[(size_t)cb * (K0 + 1) + rr + 1] - rowptr[(size_t)cb * (K0 + 1) + rr];
+                l += rowsplit[(size_t)cbp * K0 + rr];
+            }
+            rowload[(size_t)cb * K0 + r] = l;
+            total += l;
+        }
+    }
+    const int64_t thr = std::max<int64_t>(192, 3 * total / std::max<int64_t>(1, (int64_t)nb * K0));
+    std::vector<IlItem> items;
+    for (int cb = 0; cb < nb; ++cb)
+        for (int r0 = 0; r0 < K0; r0 += 8) {
+            int64_t mx = 0;
+            for (int r = r0; r < r0 + 8; ++r) mx = std::max(mx, rowload[(size_t)cb * K0 + r]);
+            int nrows = 8;
+            while (nrows > 1 && mx * nrows / 8 > thr) nrows /= 2;     // per-warp share of the heaviest row
+            for (int q = 0; q < 8; q += nrows) {
+                int64_t l = 0;
+                for (int r = r0 + q; r < r0 + q + nrows; ++r) l += rowload[(size_t)cb * K0 + r];
+                items.push_back(IlItem{cb, r0 + q, nrows, (int32_t)std::min<int64_t>(l, 0x7fffffff)});
+            }
+        }
+    std::stable_sort(items.begin(), items.end(), [](const IlItem& a, const IlItem& b) { return a.load > b.load; });
+    p->n_il_items = (int)items.size();
+    NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_delta, dl_s, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_perm, perm, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_wtab, wtab, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_rowptr, rowptr, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_rowsplit, rowsplit, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_items, items, &p->bytes_plan));
     return NUFFT_OK;
 }
 
@@ -396,6 +613,7 @@ static int plan_build(nufft_plan_t p, const double* om) {
     const int64_t M = p->M;
     std::vector<uint32_t> kpack(M);
     std::vector<float> delta((size_t)d * M);
+    std::vector<double> delta64(p->il_ok ? (size_t)d * M : 0);
     std::vector<int32_t> tid(M);
     for (int64_t m = 0; m < M; ++m) {
         uint32_t kp = 0;
@@ -404,7 +622,9 @@ static int plan_build(nufft_plan_t p, const double* om) {
             const double w = om[m * d + a];
             if (!std::isfinite(w)) return NUFFT_ERANGE;
             float df;
-            const int k0 = host::split_coordinate(w, p->K[a], J, &df);
+            double d64;
+            const int k0 = host::split_coordinate(w, p->K[a], J, &df, &d64);
+            if (p->il_ok) delta64[(size_t)a * M + m] = d64;
             kp |= (uint32_t)k0 << (10 * a);
             delta[(size_t)a * M + m] = df;
             t = t * p->ntile[a] + k0 / p->tile[a];
@@ -468,9 +688,12 @@ static int plan_build(nufft_plan_t p, const double* om) {
         NU_TRY(dev_upload(&p->d_items, items, &p->bytes_plan));
         NU_TRY(dev_upload(&p->d_tile_item_start, tstart, &p->bytes_plan));
     }
-    // workspace
-    NU_TRY(dev_alloc((void**)&p->d_grid, (size_t)p->max_batch * p->cells * sizeof(float2), &p->bytes_work));
-    NU_TRY(dev_alloc((void**)&p->d_ywork, (size_t)p->max_batch * std::max<int64_t>(M, 1) * sizeof(float2), &p->bytes_work));
+    if (p->il_ok) NU_TRY(plan_build_il(p, kpack, delta, delta64));
+    // workspace (batch_pad = max_batch, or whole groups of 32 for the interleaved layout); zeroed once so that the idle
+    // lanes of a partly filled group hold finite values
+    NU_TRY(dev_alloc((void**)&p->d_grid, (size_t)p->batch_pad * p->cells * sizeof(float2), &p->bytes_work));
+    CU_TRY(cudaMemset(p->d_grid, 0, (size_t)p->batch_pad * p->cells * sizeof(float2)));
+    NU_TRY(dev_alloc((void**)&p->d_ywork, (size_t)p->batch_pad * std::max<int64_t>(M, 1) * sizeof(float2), &p->bytes_work));
     NU_TRY(dev_alloc((void**)&p->d_scal, sizeof(CgScalars), &p->bytes_work));
     return NUFFT_OK;
 }
@@ -484,7 +707,7 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
         if (Jd[a] != kJ || !supported_K(Kd[a]) || Kd[a] != 2 * Nd[a]) return NUFFT_EINVAL;
     }
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
-                 opts->interp_mode > 1))
+                 opts->interp_mode > 1 || opts->batch_layout < 0 || opts->batch_layout > 1))
         return NUFFT_EINVAL;
     static cudaError_t cfg = configure_all();
     if (cfg != cudaSuccess) { g_last_cuda_error = (int)cfg; return NUFFT_ECUDA; }
@@ -494,6 +717,8 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     p->M = M;
     p->max_batch = max_batch;
     if (opts) p->opts = *opts;
+    p->il_ok = (d == 2) && max_batch >= 16 && p->opts.batch_layout == 0 && Kd[1] >= 2 * kBandW;
+    p->batch_pad = p->il_ok ? ((max_batch + kIL - 1) / kIL) * kIL : max_batch;
     p->nimg = 1; p->cells = 1;
     for (int a = 0; a < d; ++a) {
         p->N[a] = (int)Nd[a]; p->K[a] = (int)Kd[a];
@@ -519,6 +744,8 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_grid); cudaFree(p->d_ywork); cudaFree(p->d_imgwork); cudaFree(p->d_solver);
     cudaFree(p->d_scal); cudaFree(p->d_hist);
     cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
+    cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_perm); cudaFree(p->d_il_wtab);
+    cudaFree(p->d_il_rowptr); cudaFree(p->d_il_rowsplit); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     (void)cudaGetLastError();
     delete p;
     return NUFFT_OK;
@@ -599,6 +826,10 @@ extern "C" int nufft_stage_fft_scale(nufft_plan_t p, int batch, nufft_c64* grid,
 extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* y, void* stream) {
     if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
+    if (use_il(p, batch)) {
+        NU_TRY(run_scale_fft_il(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
+        return run_interp_il(p, batch, p->d_grid, (float2*)y, false, st);
+    }
     NU_TRY(run_scale_fft(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
     return run_interp(p, batch, p->d_grid, (float2*)y, st);
 }
@@ -606,6 +837,11 @@ extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nuff
 extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nufft_c64* x, void* stream) {
     if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
+    if (use_il(p, batch)) {
+        NU_TRY(run_y_gather_il(p, batch, (const float2*)y, st));
+        NU_TRY(run_gridding_il(p, batch, p->d_yil, p->d_grid, st));
+        return run_fft_scale_il(p, batch, p->d_grid, (float2*)x, nullptr, st);
+    }
     NU_TRY(run_gridding(p, batch, (const float2*)y, p->d_grid, st));
     return run_fft_scale(p, batch, p->d_grid, (float2*)x, nullptr, st);
 }
@@ -613,6 +849,12 @@ extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nuff
 extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
     if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
+    if (use_il(p, batch)) {     // the intermediate samples stay sorted and interleaved: no scatter, no gather
+        NU_TRY(run_scale_fft_il(p, batch, (const float2*)x_in, p->d_grid, nullptr, false, st));
+        NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, true, st));
+        NU_TRY(run_gridding_il(p, batch, p->d_ywork, p->d_grid, st));
+        return run_fft_scale_il(p, batch, p->d_grid, (float2*)x_out, nullptr, st);
+    }
     NU_TRY(run_scale_fft(p, batch, (const float2*)x_in, p->d_grid, nullptr, false, st));
     NU_TRY(run_interp(p, batch, p->d_grid, p->d_ywork, st));
     NU_TRY(run_gridding(p, batch, p->d_ywork, p->d_grid, st));
@@ -643,6 +885,10 @@ extern "C" int nufft_forward_coils(nufft_plan_t p, const nufft_c64* x, nufft_c64
     if (!p || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
+    if (use_il(p, p->ncoil)) {
+        NU_TRY(run_scale_fft_il(p, p->ncoil, (const float2*)x, p->d_grid, p->d_coils, true, st));
+        return run_interp_il(p, p->ncoil, p->d_grid, (float2*)y, false, st);
+    }
     NU_TRY(run_scale_fft(p, p->ncoil, (const float2*)x, p->d_grid, p->d_coils, true, st));
     return run_interp(p, p->ncoil, p->d_grid, (float2*)y, st);
 }
@@ -651,6 +897,12 @@ extern "C" int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64* y, nufft_c64
     if (!p || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
+    if (use_il(p, p->ncoil)) {
+        NU_TRY(run_y_gather_il(p, p->ncoil, (const float2*)y, st));
+        NU_TRY(run_gridding_il(p, p->ncoil, p->d_yil, p->d_grid, st));
+        NU_TRY(run_fft_scale_il(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
+        return coil_reduce(p, (float2*)x, st);
+    }
     NU_TRY(run_gridding(p, p->ncoil, (const float2*)y, p->d_grid, st));
     NU_TRY(run_fft_scale(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
     return coil_reduce(p, (float2*)x, st);
@@ -660,6 +912,13 @@ extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nu
     if (!p || !x_in || !x_out) return NUFFT_EINVAL;
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
+    if (use_il(p, p->ncoil)) {
+        NU_TRY(run_scale_fft_il(p, p->ncoil, (const float2*)x_in, p->d_grid, p->d_coils, true, st));
+        NU_TRY(run_interp_il(p, p->ncoil, p->d_grid, p->d_ywork, true, st));
+        NU_TRY(run_gridding_il(p, p->ncoil, p->d_ywork, p->d_grid, st));
+        NU_TRY(run_fft_scale_il(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
+        return coil_reduce(p, (float2*)x_out, st);
+    }
     NU_TRY(run_scale_fft(p, p->ncoil, (const float2*)x_in, p->d_grid, p->d_coils, true, st));
     NU_TRY(run_interp(p, p->ncoil, p->d_grid, p->d_ywork, st));
     NU_TRY(run_gridding(p, p->ncoil, p->d_ywork, p->d_grid, st));

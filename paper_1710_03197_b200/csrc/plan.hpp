@@ -110,16 +110,23 @@ inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {
 
 // Per-sample split of the coordinate, in float64 (reading R6/R11):
 //   u = om * (K / (2 pi));  k0 = ceil(u - J/2);  delta = k0 - (u - J/2) in [0,1);  returns k0 mod K.
-inline int split_coordinate(double om, int K, double J, float* delta) {
+inline int split_coordinate(double om, int K, double J, float* delta, double* delta64 = nullptr) {
     const double u = om * ((double)K / (2.0 * kPi));
     const double k0 = std::ceil(u - 0.5 * J);
     double dl = k0 - (u - 0.5 * J);
+    if (delta64) *delta64 = dl;
     float df = (float)dl;
     if (df >= 1.0f) df = 0.99999994f;      // float rounding of 1 - tiny; phi is continuous there
     *delta = df;
     long long k = (long long)k0 % K;
     if (k < 0) k += K;
     return (int)k;
+}
+
+// Six weights of one axis in float64: w[j] = phi(J/2 - delta - j), with phi(+J/2) = 0 (open support, reading R6).
+inline void kb_weights_f64(double delta, double J, double beta, double (&w)[kJ]) {
+    for (int j = 0; j < kJ; ++j) w[j] = kb_phi(0.5 * J - delta - (double)j, J, beta);
+    if (delta == 0.0) w[0] = 0.0;
 }
 
 }  // namespace host

@@ -341,3 +341,77 @@ def test_l1tv_ols_single_coil_lambda_zero_reduces_to_cg():
     xo = sol.l1tv_ols(AHA, AHy, 1.0, 0.0, 1, 2, 3)
     xg = p.solve_l1tv_ols(dev(y), 1.0, 0.0, 1, 2, 3)
     assert rel(host(xg), xo) < 1e-4
+
+
+# ---------------------------------------------------------------------------------------------------------
+# batch-interleaved 2-D path (batch >= 16: lanes = images, register-accumulated gather-form V^H; batch_il.cuh)
+# ---------------------------------------------------------------------------------------------------------
+def check_batched(cfg, B, sample_imgs, seed=0):
+    """forward / adjoint / A^H A of a batch of B images: the images in `sample_imgs` against the oracle, all of them
+    against the planar path of the same library (batch_layout = 1)."""
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    M = om.shape[0]
+    p = make_plan(cfg, max_batch=B)
+    q = make_plan(cfg, max_batch=B, batch_layout=1)
+    x = wl.image_gaussian(Nd, seed=wl.SEED_IMAGE + seed, batch=B)
+    y = wl.data_gaussian(M, seed=wl.SEED_Y + seed, batch=B)
+    yg, xg, sg = host(p.forward(dev(x))), host(p.adjoint(dev(y))), host(p.selfadjoint(dev(x)))
+    yq, xq, sq = host(q.forward(dev(x))), host(q.adjoint(dev(y))), host(q.selfadjoint(dev(x)))
+    assert rel(yg, yq) < 2e-6 and rel(xg, xq) < 2e-6 and rel(sg, sq) < 2e-6
+    for b in sample_imgs:
+        yo = orc.forward(x[b].astype(np.complex128), om, Nd, Kd, Jd)
+        xo = orc.adjoint(y[b].astype(np.complex128), om, Nd, Kd, Jd)
+        so = orc.adjoint(yo, om, Nd, Kd, Jd)
+        errs = (rel(yg[b], yo), rel(xg[b], xo), rel(sg[b], so))
+        assert max(errs) < TOL, (b, errs)
+    # gather-form V^H: bit-reproducible run to run
+    again = host(p.adjoint(dev(y)))
+    assert np.array_equal(xg.view(np.uint32), again.view(np.uint32))
+    p.destroy()
+    q.destroy()
+
+
+def test_interleaved_config1_ragged_batch40():
+    check_batched(wl.config(0), 40, [0, 31, 32, 39])
+
+
+def test_interleaved_config2_radial_batch32():
+    check_batched(wl.config(1), 32, [0, 17])
+
+
+@pytest.mark.parametrize("Nd,M,B", [((16, 16), 1000, 16), ((32, 128), 4097, 33), ((256, 64), 3001, 17),
+                                    ((512, 16), 777, 16)])
+def test_interleaved_odd_shapes(Nd, M, B):
+    check_batched(custom_cfg(Nd, M), B, [0, B - 1], seed=2)
+
+
+def test_interleaved_seam_grid_points_and_hot_cell():
+    Nd = (32, 32)
+    K = 64
+    rng = np.random.default_rng(5)
+    on_grid = 2 * np.pi * rng.integers(-K // 2, K // 2, size=(300, 2)) / K
+    seam = np.stack([np.full(200, -np.pi), rng.uniform(-np.pi, np.pi, 200)], axis=1)
+    seam2 = np.stack([rng.uniform(-np.pi, np.pi, 200), np.full(200, -np.pi)], axis=1)
+    near_seam = np.stack([rng.uniform(np.pi - 0.3, np.pi, 200), rng.uniform(-np.pi, -np.pi + 0.3, 200)], axis=1)
+    outside = rng.uniform(-3 * np.pi, 3 * np.pi, size=(300, 2))
+    hot = 0.3 + 1e-3 * rng.uniform(-1, 1, size=(5000, 2))       # one hot cell: rows split among the warps of a CTA
+    om = np.concatenate([on_grid, seam, seam2, near_seam, outside, hot, np.zeros((5, 2))])
+    check_batched(custom_cfg(Nd, 0, om=om), 16, [0, 15])
+
+
+def test_interleaved_multicoil_operator_16_coils():
+    cfg = wl.config(4, scale=2)            # 128^2
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    nc = 16
+    c = wl.coil_maps(nc, Nd)
+    p = make_plan(cfg, max_batch=nc)
+    p.set_coils(dev(c))
+    x = wl.image_gaussian(Nd)
+    y = wl.data_gaussian(om.shape[0], batch=nc)
+    c128 = c.astype(np.complex128)
+    yo = orc.forward_coils(x.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    xo = orc.adjoint_coils(y.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    so = orc.adjoint_coils(yo, c128, om, Nd, Kd, Jd)
+    assert rel(host(p.forward_coils(dev(x))), yo) < TOL
+    assert rel(host(p.adjoint_coils(dev(y))), xo) < TOL
+    assert rel(host(p.selfadjoint_coils(dev(x))), so) < TOL
