@@ -114,37 +114,40 @@ struct IlPlan {
 // a3: y = V grid.  One warp = 32 consecutive sorted samples x the 32 images of group blockIdx.y.
 // Each lane prepares the weights of one sample (kb_weights) and stages them in shared memory; the warp then walks
 // the samples one by one with warp-uniform weights: 36 loads of 256 contiguous bytes and 72 + 12 FMAs per lane.
+constexpr int kInterpWarps = 8;
+constexpr int kInterpChunk = 128;    // consecutive sorted samples per CTA
 // SORTED_OUT: y is written as y_il[group][sorted sample][32] (selfadjoint intermediate) instead of y[b][perm].
 template <bool SORTED_OUT>
 __global__ void __launch_bounds__(256)
 interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y, int batch,
                  KernelPoly P) {
-    __shared__ float4 wrec[8][32 * 4];
+    __shared__ float4 wrec[kInterpChunk * 4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = blockIdx.y;
-    const int64_t s0 = ((int64_t)blockIdx.x * 8 + warp) * 32;
-    if (s0 >= g.M) return;
-    const int cnt = (int)min((int64_t)32, g.M - s0);
-    if (lane < cnt) {
-        const int64_t si = s0 + lane;
+    const int64_t s0 = (int64_t)blockIdx.x * kInterpChunk;
+    const int cnt = (int)min((int64_t)kInterpChunk, g.M - s0);
+    for (int t = threadIdx.x; t < cnt; t += blockDim.x) {
+        const int64_t si = s0 + t;
         const uint32_t kp = __ldg(&s.kpack[si]);
         float w0[kJ], w1[kJ];
         kb_weights(P, __ldg(&s.delta[si]), w0);
         kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
-        float4* r = &wrec[warp][lane * 4];
+        float4* r = &wrec[t * 4];
         r[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
         r[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
         r[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
         r[3] = make_float4(__int_as_float((int)(kp & 1023u)), __int_as_float((int)((kp >> 10) & 1023u)),
                            __int_as_float(SORTED_OUT ? 0 : __ldg(&s.perm[si])), 0.f);
     }
-    __syncwarp();
+    __syncthreads();
     const int K0 = g.K[0], K1 = g.K[1];
     const float2* __restrict__ G = grid_il + (int64_t)grp * g.cells * kIL + lane;
     const int b = grp * kIL + lane;
-    for (int sidx = 0; sidx < cnt; ++sidx) {
-        const float4 ra = wrec[warp][sidx * 4 + 0], rb = wrec[warp][sidx * 4 + 1];
-        const float4 rc = wrec[warp][sidx * 4 + 2], rd = wrec[warp][sidx * 4 + 3];
+    // the warps of a CTA interleave over consecutive sorted samples: their stencils overlap, so the CTA's working set in
+    // L1 is one moving window of a few rows instead of one window per warp
+    for (int sidx = warp; sidx < cnt; sidx += kInterpWarps) {
+        const float4 ra = wrec[sidx * 4 + 0], rb = wrec[sidx * 4 + 1];
+        const float4 rc = wrec[sidx * 4 + 2], rd = wrec[sidx * 4 + 3];
         const float w0[kJ] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y};
         const float w1[kJ] = {rb.z, rb.w, rc.x, rc.y, rc.z, rc.w};
         const int r0 = __float_as_int(rd.x), c0 = __float_as_int(rd.y);
@@ -217,13 +220,14 @@ struct IlItem {
 template <int OFF>
 __device__ __forceinline__ void il_accumulate(float2 (&acc)[kBandW], const float* __restrict__ wtab,
                                               const float2* __restrict__ Y, int j0, int b, int e) {
-#pragma unroll 2
-    for (int i = b; i < e; ++i) {
-        const float* __restrict__ rec = wtab + (int64_t)i * kTabW;
-        const float w0 = __ldg(rec + j0);
-        const float4 pa = __ldg(reinterpret_cast<const float4*>(rec + OFF));
-        const float4 pb = __ldg(reinterpret_cast<const float4*>(rec + OFF + 4));
-        const float2 yv = __ldg(Y + (int64_t)i * kIL);
+    const float* __restrict__ rec = wtab + (int64_t)b * kTabW + j0;
+    const float2* __restrict__ yp = Y + (int64_t)b * kIL;
+#pragma unroll 4
+    for (int i = b; i < e; ++i, rec += kTabW, yp += kIL) {
+        const float w0 = __ldg(rec);
+        const float4 pa = __ldg(reinterpret_cast<const float4*>(rec - j0 + OFF));
+        const float4 pb = __ldg(reinterpret_cast<const float4*>(rec - j0 + OFF + 4));
+        const float2 yv = __ldg(yp);
         const float tx = w0 * yv.x, ty = w0 * yv.y;
         acc[0].x = fmaf(pa.x, tx, acc[0].x); acc[0].y = fmaf(pa.x, ty, acc[0].y);
         acc[1].x = fmaf(pa.y, tx, acc[1].x); acc[1].y = fmaf(pa.y, ty, acc[1].y);
@@ -243,8 +247,8 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
     const IlItem it = items[blockIdx.x];
     const int grp = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nsplit = 8 / it.nrows;
-    const int row = it.r0 + warp / nsplit, part = warp % nsplit;
+    const int nsplit = 8 / it.nrows, lsplit = 31 - __clz(nsplit);       // nsplit is a power of two
+    const int row = it.r0 + (warp >> lsplit), part = warp & (nsplit - 1);
     const int K0 = g.K[0], K1 = g.K[1], nb = K1 / kBandW;
     const int cbp = (it.cb + nb - 1) % nb;
     const float2* __restrict__ Y = y_il + (int64_t)grp * g.M * kIL + lane;
@@ -256,13 +260,11 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
         const int r = (row - j0) & (K0 - 1);
         {   // samples of this band: columns relative to the band start, table part A
             const int b = __ldg(&s.rowptr[it.cb * (K0 + 1) + r]), n = __ldg(&s.rowptr[it.cb * (K0 + 1) + r + 1]) - b;
-            il_accumulate<8>(acc, s.wtab, Y, j0, b + (int)((int64_t)n * part / nsplit),
-                             b + (int)((int64_t)n * (part + 1) / nsplit));
+            il_accumulate<8>(acc, s.wtab, Y, j0, b + ((n * part) >> lsplit), b + ((n * (part + 1)) >> lsplit));
         }
         {   // samples of the previous band whose stencil reaches into this one: table part B
             const int b = __ldg(&s.rowptr[cbp * (K0 + 1) + r]), n = __ldg(&s.rowsplit[cbp * K0 + r]);
-            il_accumulate<16>(acc, s.wtab, Y, j0, b + (int)((int64_t)n * part / nsplit),
-                              b + (int)((int64_t)n * (part + 1) / nsplit));
+            il_accumulate<16>(acc, s.wtab, Y, j0, b + ((n * part) >> lsplit), b + ((n * (part + 1)) >> lsplit));
         }
     }
     if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row

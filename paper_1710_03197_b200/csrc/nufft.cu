@@ -421,7 +421,7 @@ static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, 
 // a3: sorted_out = false: y[batch][M] in the caller's order; true: y_il[group][sorted sample][32]
 static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* y, bool sorted_out, cudaStream_t st) {
     if (p->M == 0) return NUFFT_OK;
-    const dim3 blocks((unsigned)((p->M + 255) / 256), (unsigned)il_groups(batch));
+    const dim3 blocks((unsigned)((p->M + kInterpChunk - 1) / kInterpChunk), (unsigned)il_groups(batch));
     ProfScope ps(p, "interp", st);
     if (sorted_out) interp_il_kernel<true><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
     else            interp_il_kernel<false><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
