@@ -314,8 +314,8 @@ def run_ours(args):
             "kernels": rows,
             "stages_ms": {
                 "F (S+pad+FFT)": stage_of(rows, ["fft_rows_fwd", "fft_cols_fwd"]),
-                "V": stage_of(rows, ["interp"]),
-                "V^H": stage_of(rows, ["y_gather", "grid_zero", "gridding", "gridding_merge"]),
+                "V": stage_of(rows, ["interp", "y_from_il"]),
+                "V^H": stage_of(rows, ["y_to_il", "grid_zero", "gridding", "gridding_merge"]),
                 "F^H (IFFT+crop+S^H)": stage_of(rows, ["fft_cols_adj", "fft_rows_adj"]),
             },
             "note": "2-D grids of this batch are partly L2-resident between kernels of one step; V and V^H are "

@@ -105,7 +105,7 @@ fft_il_rows_adj_kernel(IlRowParams p) {
 struct IlPlan {
     const uint32_t* kpack;    // stencil base index per axis (10 bits each), sorted order
     const float* delta;       // [2][M]
-    const int32_t* perm;      // sorted position -> caller's sample index
+    const int32_t* pos;       // caller's sample index -> sorted position
     const float* wtab;        // [M][kTabW] V^H weight table (float64-built)
     const int32_t* rowptr;    // [K1/8][K0 + 1]: first sorted sample of (band, row)
     const int32_t* rowsplit;  // [K1/8][K0]: samples of (band, row) whose stencil reaches into the next band (they come first)
@@ -116,11 +116,9 @@ struct IlPlan {
 // the samples one by one with warp-uniform weights: 36 loads of 256 contiguous bytes and 72 + 12 FMAs per lane.
 constexpr int kInterpWarps = 8;
 constexpr int kInterpChunk = 128;    // consecutive sorted samples per CTA
-// SORTED_OUT: y is written as y_il[group][sorted sample][32] (selfadjoint intermediate) instead of y[b][perm].
-template <bool SORTED_OUT>
+// Output: y_il[group][sorted sample][32] (coalesced); y_from_il_kernel restores the caller's order when needed.
 __global__ void __launch_bounds__(256)
-interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y, int batch,
-                 KernelPoly P) {
+interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y_il, KernelPoly P) {
     __shared__ float4 wrec[kInterpChunk * 4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = blockIdx.y;
@@ -137,12 +135,11 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
         r[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
         r[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
         r[3] = make_float4(__int_as_float((int)(kp & 1023u)), __int_as_float((int)((kp >> 10) & 1023u)),
-                           __int_as_float(SORTED_OUT ? 0 : __ldg(&s.perm[si])), 0.f);
+                           0.f, 0.f);
     }
     __syncthreads();
     const int K0 = g.K[0], K1 = g.K[1];
     const float2* __restrict__ G = grid_il + (int64_t)grp * g.cells * kIL + lane;
-    const int b = grp * kIL + lane;
     // the warps of a CTA interleave over consecutive sorted samples: their stencils overlap, so the CTA's working set in
     // L1 is one moving window of a few rows instead of one window per warp
     for (int sidx = warp; sidx < cnt; sidx += kInterpWarps) {
@@ -181,30 +178,59 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
                 acc.y = fmaf(w0[j0], r.y, acc.y);
             }
         }
-        if (SORTED_OUT) y[((int64_t)grp * g.M + s0 + sidx) * kIL + lane] = acc;
-        else if (b < batch) y[(int64_t)b * g.M + __float_as_int(rd.z)] = acc;
+        y_il[((int64_t)grp * g.M + s0 + sidx) * kIL + lane] = acc;
     }
 }
 
-// y (caller's order, [batch][M]) -> y_il[group][sorted sample][32]; idle lanes of the last group get zeros.
+// Layout changes of the sample vectors, coalesced on both sides (a warp moves a 32 samples x 32 images tile through
+// shared memory): the caller's y[batch][M] <-> y_il[group][sorted position][32].  pos[m] = sorted position of caller
+// sample m.  Idle lanes of the last group are written as zeros.
 __global__ void __launch_bounds__(128)
-y_gather_il_kernel(const int32_t* __restrict__ perm, const float2* __restrict__ y, float2* __restrict__ y_il, int64_t M,
-                   int batch) {
+y_to_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y, float2* __restrict__ y_il, int64_t M,
+               int batch) {
     __shared__ float2 tile[4][32][33];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = blockIdx.y;
-    const int64_t s0 = ((int64_t)blockIdx.x * 4 + warp) * 32;
-    if (s0 >= M) return;
-    const int cnt = (int)min((int64_t)32, M - s0);
-    const int64_t pm = (lane < cnt) ? (int64_t)__ldg(&perm[s0 + lane]) : -1;
-#pragma unroll 4
+    const int64_t m0 = ((int64_t)blockIdx.x * 4 + warp) * 32;
+    if (m0 >= M) return;
+    const int cnt = (int)min((int64_t)32, M - m0);
+    const int my = (lane < cnt) ? __ldg(&pos[m0 + lane]) : 0;
+#pragma unroll 8
     for (int l = 0; l < kIL; ++l) {
         const int b = grp * kIL + l;
-        tile[warp][lane][l] = (pm >= 0 && b < batch) ? __ldg(&y[(int64_t)b * M + pm]) : make_float2(0.f, 0.f);
+        tile[warp][lane][l] = (lane < cnt && b < batch) ? __ldg(&y[(int64_t)b * M + m0 + lane]) : make_float2(0.f, 0.f);
     }
     __syncwarp();
-    float2* __restrict__ dst = y_il + ((int64_t)grp * M + s0) * kIL + lane;
-    for (int sidx = 0; sidx < cnt; ++sidx) dst[(int64_t)sidx * kIL] = tile[warp][sidx][lane];
+    float2* __restrict__ dst = y_il + (int64_t)grp * M * kIL + lane;
+    for (int k = 0; k < cnt; ++k) {
+        const int i = __shfl_sync(0xffffffffu, my, k);
+        dst[(int64_t)i * kIL] = tile[warp][k][lane];
+    }
+}
+
+__global__ void __launch_bounds__(128)
+y_from_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y_il, float2* __restrict__ y, int64_t M,
+                 int batch) {
+    __shared__ float2 tile[4][32][33];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = blockIdx.y;
+    const int64_t m0 = ((int64_t)blockIdx.x * 4 + warp) * 32;
+    if (m0 >= M) return;
+    const int cnt = (int)min((int64_t)32, M - m0);
+    const int my = (lane < cnt) ? __ldg(&pos[m0 + lane]) : 0;
+    const float2* __restrict__ src = y_il + (int64_t)grp * M * kIL + lane;
+#pragma unroll 8
+    for (int k = 0; k < cnt; ++k) {
+        const int i = __shfl_sync(0xffffffffu, my, k);
+        tile[warp][k][lane] = __ldg(&src[(int64_t)i * kIL]);
+    }
+    __syncwarp();
+    if (lane >= cnt) return;
+#pragma unroll 8
+    for (int l = 0; l < kIL; ++l) {
+        const int b = grp * kIL + l;
+        if (b < batch) y[(int64_t)b * M + m0 + lane] = tile[warp][lane][l];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------

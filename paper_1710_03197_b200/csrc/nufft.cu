@@ -76,7 +76,7 @@ struct nufft_plan_s {
     int batch_pad = 1;              // max_batch rounded up to whole groups of 32 when il_ok
     uint32_t* d_il_kpack = nullptr;
     float* d_il_delta = nullptr;
-    int32_t* d_il_perm = nullptr;
+    int32_t* d_il_pos = nullptr;     // caller sample -> sorted position
     float* d_il_wtab = nullptr;
     int32_t* d_il_rowptr = nullptr;
     int32_t* d_il_rowsplit = nullptr;
@@ -396,7 +396,7 @@ static ColPassParams il_col_params(nufft_plan_t p, int batch, float2* grid) {
 }
 static IlPlan il_plan(nufft_plan_t p) {
     IlPlan s{};
-    s.kpack = p->d_il_kpack; s.delta = p->d_il_delta; s.perm = p->d_il_perm; s.wtab = p->d_il_wtab;
+    s.kpack = p->d_il_kpack; s.delta = p->d_il_delta; s.pos = p->d_il_pos; s.wtab = p->d_il_wtab;
     s.rowptr = p->d_il_rowptr; s.rowsplit = p->d_il_rowsplit;
     return s;
 }
@@ -418,25 +418,34 @@ static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, 
     p->launches += 2;
     return NUFFT_OK;
 }
-// a3: sorted_out = false: y[batch][M] in the caller's order; true: y_il[group][sorted sample][32]
-static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* y, bool sorted_out, cudaStream_t st) {
+// a3: y_il[group][sorted sample][32] = V grid_il
+static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* y_il, cudaStream_t st) {
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + kInterpChunk - 1) / kInterpChunk), (unsigned)il_groups(batch));
     ProfScope ps(p, "interp", st);
-    if (sorted_out) interp_il_kernel<true><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
-    else            interp_il_kernel<false><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
+    interp_il_kernel<<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, p->poly);
     CU_TRY(cudaGetLastError());
     p->launches++;
     return NUFFT_OK;
 }
-// caller's y -> y_il
-static int run_y_gather_il(nufft_plan_t p, int batch, const float2* y, cudaStream_t st) {
+// caller's y[batch][M] -> d_yil
+static int run_y_to_il(nufft_plan_t p, int batch, const float2* y, cudaStream_t st) {
     if (p->M == 0) return NUFFT_OK;
     if (!p->d_yil)
         NU_TRY(dev_alloc((void**)&p->d_yil, (size_t)p->batch_pad * p->M * sizeof(float2), &p->bytes_work));
     const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)il_groups(batch));
-    ProfScope ps(p, "y_gather", st);
-    y_gather_il_kernel<<<blocks, 128, 0, st>>>(p->d_il_perm, y, p->d_yil, p->M, batch);
+    ProfScope ps(p, "y_to_il", st);
+    y_to_il_kernel<<<blocks, 128, 0, st>>>(p->d_il_pos, y, p->d_yil, p->M, batch);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+// y_il -> caller's y[batch][M]
+static int run_y_from_il(nufft_plan_t p, int batch, const float2* y_il, float2* y, cudaStream_t st) {
+    if (p->M == 0) return NUFFT_OK;
+    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)il_groups(batch));
+    ProfScope ps(p, "y_from_il", st);
+    y_from_il_kernel<<<blocks, 128, 0, st>>>(p->d_il_pos, y_il, y, p->M, batch);
     CU_TRY(cudaGetLastError());
     p->launches++;
     return NUFFT_OK;
@@ -571,7 +580,11 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
     p->n_il_items = (int)items.size();
     NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_delta, dl_s, &p->bytes_plan));
-    NU_TRY(dev_upload(&p->d_il_perm, perm, &p->bytes_plan));
+    {
+        std::vector<int32_t> pos(M);
+        for (int64_t i = 0; i < M; ++i) pos[perm[i]] = (int32_t)i;
+        NU_TRY(dev_upload(&p->d_il_pos, pos, &p->bytes_plan));
+    }
     NU_TRY(dev_upload(&p->d_il_wtab, wtab, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_rowptr, rowptr, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_rowsplit, rowsplit, &p->bytes_plan));
@@ -744,7 +757,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_grid); cudaFree(p->d_ywork); cudaFree(p->d_imgwork); cudaFree(p->d_solver);
     cudaFree(p->d_scal); cudaFree(p->d_hist);
     cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
-    cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_perm); cudaFree(p->d_il_wtab);
+    cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_rowsplit); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     (void)cudaGetLastError();
     delete p;
@@ -828,7 +841,8 @@ extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nuff
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, batch)) {
         NU_TRY(run_scale_fft_il(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
-        return run_interp_il(p, batch, p->d_grid, (float2*)y, false, st);
+        NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, st));
+        return run_y_from_il(p, batch, p->d_ywork, (float2*)y, st);
     }
     NU_TRY(run_scale_fft(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
     return run_interp(p, batch, p->d_grid, (float2*)y, st);
@@ -838,7 +852,7 @@ extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nuff
     if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, batch)) {
-        NU_TRY(run_y_gather_il(p, batch, (const float2*)y, st));
+        NU_TRY(run_y_to_il(p, batch, (const float2*)y, st));
         NU_TRY(run_gridding_il(p, batch, p->d_yil, p->d_grid, st));
         return run_fft_scale_il(p, batch, p->d_grid, (float2*)x, nullptr, st);
     }
@@ -851,7 +865,7 @@ extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_i
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, batch)) {     // the intermediate samples stay sorted and interleaved: no scatter, no gather
         NU_TRY(run_scale_fft_il(p, batch, (const float2*)x_in, p->d_grid, nullptr, false, st));
-        NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, true, st));
+        NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, st));
         NU_TRY(run_gridding_il(p, batch, p->d_ywork, p->d_grid, st));
         return run_fft_scale_il(p, batch, p->d_grid, (float2*)x_out, nullptr, st);
     }
@@ -887,7 +901,8 @@ extern "C" int nufft_forward_coils(nufft_plan_t p, const nufft_c64* x, nufft_c64
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
         NU_TRY(run_scale_fft_il(p, p->ncoil, (const float2*)x, p->d_grid, p->d_coils, true, st));
-        return run_interp_il(p, p->ncoil, p->d_grid, (float2*)y, false, st);
+        NU_TRY(run_interp_il(p, p->ncoil, p->d_grid, p->d_ywork, st));
+        return run_y_from_il(p, p->ncoil, p->d_ywork, (float2*)y, st);
     }
     NU_TRY(run_scale_fft(p, p->ncoil, (const float2*)x, p->d_grid, p->d_coils, true, st));
     return run_interp(p, p->ncoil, p->d_grid, (float2*)y, st);
@@ -898,7 +913,7 @@ extern "C" int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64* y, nufft_c64
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
-        NU_TRY(run_y_gather_il(p, p->ncoil, (const float2*)y, st));
+        NU_TRY(run_y_to_il(p, p->ncoil, (const float2*)y, st));
         NU_TRY(run_gridding_il(p, p->ncoil, p->d_yil, p->d_grid, st));
         NU_TRY(run_fft_scale_il(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
         return coil_reduce(p, (float2*)x, st);
@@ -914,7 +929,7 @@ extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nu
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
         NU_TRY(run_scale_fft_il(p, p->ncoil, (const float2*)x_in, p->d_grid, p->d_coils, true, st));
-        NU_TRY(run_interp_il(p, p->ncoil, p->d_grid, p->d_ywork, true, st));
+        NU_TRY(run_interp_il(p, p->ncoil, p->d_grid, p->d_ywork, st));
         NU_TRY(run_gridding_il(p, p->ncoil, p->d_ywork, p->d_grid, st));
         NU_TRY(run_fft_scale_il(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
         return coil_reduce(p, (float2*)x_out, st);
