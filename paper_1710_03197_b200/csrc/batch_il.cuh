@@ -100,15 +100,18 @@ fft_il_rows_adj_kernel(IlRowParams p) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// plan data of the interleaved path: samples in CELL-SORTED order, key = (column band, row k0_0, 7 - (k0_1 mod 8))
+// plan data of the interleaved path (built by plan_build_il in nufft.cu).  Two sample orders:
+//   V order    key (column band, row k0_0, column):  kpack, delta, v2h
+//   V^H order  key (column band, class, row k0_0, column), class 0 = column offset in the band >= 3 (the stencil
+//              reaches into the next band), class 1 = the rest:  wtab, rowptr, pos, and every y_il array
 // ------------------------------------------------------------------------------------------------------------
 struct IlPlan {
-    const uint32_t* kpack;    // stencil base index per axis (10 bits each), sorted order
-    const float* delta;       // [2][M]
-    const int32_t* pos;       // caller's sample index -> sorted position
-    const float* wtab;        // [M][kTabW] V^H weight table (float64-built)
-    const int32_t* rowptr;    // [K1/8][K0 + 1]: first sorted sample of (band, row)
-    const int32_t* rowsplit;  // [K1/8][K0]: samples of (band, row) whose stencil reaches into the next band (they come first)
+    const uint32_t* kpack;    // V order: stencil base index per axis (10 bits each)
+    const float* delta;       // V order: [2][M]
+    const int32_t* v2h;       // V-order position -> V^H-order position
+    const int32_t* pos;       // caller's sample index -> V^H-order position
+    const float* wtab;        // V^H order: [M][kTabW] = w0[6], k0_0 (int bits), pad, w1 part A[8], w1 part B[8] (float64-built)
+    const int32_t* rowptr;    // [(band * 2 + class) * K0 + row]: first V^H-order sample of (band, class, row); + 1 entry
 };
 
 // a3: y = V grid.  One warp = 32 consecutive sorted samples x the 32 images of group blockIdx.y.
@@ -135,7 +138,7 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
         r[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
         r[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
         r[3] = make_float4(__int_as_float((int)(kp & 1023u)), __int_as_float((int)((kp >> 10) & 1023u)),
-                           0.f, 0.f);
+                           __int_as_float(__ldg(&s.v2h[si])), 0.f);
     }
     __syncthreads();
     const int K0 = g.K[0], K1 = g.K[1];
@@ -178,7 +181,7 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
                 acc.y = fmaf(w0[j0], r.y, acc.y);
             }
         }
-        y_il[((int64_t)grp * g.M + s0 + sidx) * kIL + lane] = acc;
+        y_il[((int64_t)grp * g.M + __float_as_int(rd.z)) * kIL + lane] = acc;
     }
 }
 
@@ -243,16 +246,20 @@ struct IlItem {
     int32_t load;     // row-sample interactions of the item (plan-time cost estimate; sort key)
 };
 
+// Adds the samples [b, e) of the V^H order to the 8 accumulators of output row `row`.  OFF = 8: the samples lie in this
+// band (table part A), OFF = 16: in the previous band (part B).  The samples of a range span up to 6 stencil base rows;
+// each one looks up its own row weight w0[row - k0_0].
 template <int OFF>
 __device__ __forceinline__ void il_accumulate(float2 (&acc)[kBandW], const float* __restrict__ wtab,
-                                              const float2* __restrict__ Y, int j0, int b, int e) {
-    const float* __restrict__ rec = wtab + (int64_t)b * kTabW + j0;
+                                              const float2* __restrict__ Y, int row, int kmask, int b, int e) {
+    const float* __restrict__ rec = wtab + (int64_t)b * kTabW;
     const float2* __restrict__ yp = Y + (int64_t)b * kIL;
 #pragma unroll 4
     for (int i = b; i < e; ++i, rec += kTabW, yp += kIL) {
-        const float w0 = __ldg(rec);
-        const float4 pa = __ldg(reinterpret_cast<const float4*>(rec - j0 + OFF));
-        const float4 pb = __ldg(reinterpret_cast<const float4*>(rec - j0 + OFF + 4));
+        const int j0 = (row - __float_as_int(__ldg(rec + 6))) & kmask;
+        const float w0 = __ldg(rec + j0);
+        const float4 pa = __ldg(reinterpret_cast<const float4*>(rec + OFF));
+        const float4 pb = __ldg(reinterpret_cast<const float4*>(rec + OFF + 4));
         const float2 yv = __ldg(yp);
         const float tx = w0 * yv.x, ty = w0 * yv.y;
         acc[0].x = fmaf(pa.x, tx, acc[0].x); acc[0].y = fmaf(pa.x, ty, acc[0].y);
@@ -281,16 +288,19 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
     float2 acc[kBandW];
 #pragma unroll
     for (int c = 0; c < kBandW; ++c) acc[c] = make_float2(0.f, 0.f);
+    // stencil base rows row-5 .. row (mod K0): one row segment, or two at the periodic seam
+    const int nseg = (row >= kJ - 1) ? 1 : 2;
 #pragma unroll 1
-    for (int j0 = 0; j0 < kJ; ++j0) {
-        const int r = (row - j0) & (K0 - 1);
-        {   // samples of this band: columns relative to the band start, table part A
-            const int b = __ldg(&s.rowptr[it.cb * (K0 + 1) + r]), n = __ldg(&s.rowptr[it.cb * (K0 + 1) + r + 1]) - b;
-            il_accumulate<8>(acc, s.wtab, Y, j0, b + ((n * part) >> lsplit), b + ((n * (part + 1)) >> lsplit));
-        }
-        {   // samples of the previous band whose stencil reaches into this one: table part B
-            const int b = __ldg(&s.rowptr[cbp * (K0 + 1) + r]), n = __ldg(&s.rowsplit[cbp * K0 + r]);
-            il_accumulate<16>(acc, s.wtab, Y, j0, b + ((n * part) >> lsplit), b + ((n * (part + 1)) >> lsplit));
+    for (int sg = 0; sg < nseg; ++sg) {
+        const int lo = (nseg == 1) ? row - (kJ - 1) : (sg == 0 ? 0 : K0 - (kJ - 1) + row);
+        const int hi = (nseg == 1 || sg == 0) ? row : K0 - 1;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {     // this band class 0, this band class 1 (part A); previous band class 0 (part B)
+            const int base = ((q == 2 ? cbp : it.cb) * 2 + (q == 1 ? 1 : 0)) * K0;
+            const int b = __ldg(&s.rowptr[base + lo]), n = __ldg(&s.rowptr[base + hi + 1]) - b;
+            const int bb = b + ((n * part) >> lsplit), ee = b + ((n * (part + 1)) >> lsplit);
+            if (q == 2) il_accumulate<16>(acc, s.wtab, Y, row, K0 - 1, bb, ee);
+            else        il_accumulate<8>(acc, s.wtab, Y, row, K0 - 1, bb, ee);
         }
     }
     if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row

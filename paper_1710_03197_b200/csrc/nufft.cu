@@ -76,10 +76,10 @@ struct nufft_plan_s {
     int batch_pad = 1;              // max_batch rounded up to whole groups of 32 when il_ok
     uint32_t* d_il_kpack = nullptr;
     float* d_il_delta = nullptr;
-    int32_t* d_il_pos = nullptr;     // caller sample -> sorted position
+    int32_t* d_il_pos = nullptr;     // caller sample -> V^H-order position (the order of y_il)
     float* d_il_wtab = nullptr;
     int32_t* d_il_rowptr = nullptr;
-    int32_t* d_il_rowsplit = nullptr;
+    int32_t* d_il_v2h = nullptr;     // V-order position -> V^H-order position
     IlItem* d_il_items = nullptr;
     int n_il_items = 0;
     float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
@@ -397,7 +397,7 @@ static ColPassParams il_col_params(nufft_plan_t p, int batch, float2* grid) {
 static IlPlan il_plan(nufft_plan_t p) {
     IlPlan s{};
     s.kpack = p->d_il_kpack; s.delta = p->d_il_delta; s.pos = p->d_il_pos; s.wtab = p->d_il_wtab;
-    s.rowptr = p->d_il_rowptr; s.rowsplit = p->d_il_rowsplit;
+    s.rowptr = p->d_il_rowptr; s.v2h = p->d_il_v2h;
     return s;
 }
 
@@ -493,71 +493,85 @@ extern "C" int nufft_default_opts(nufft_opts* o) {
     return NUFFT_OK;
 }
 
-// Plan data of the batch-interleaved path (batch_il.cuh): cell-sorted sample order, V^H weight table (float64-built),
-// row pointers per column band, V^H work items.
+// Plan data of the batch-interleaved path (batch_il.cuh).  Two sample orders:
+//   V order   key (column band, row k0_0, column)          consecutive samples share stencil rows: L1 reuse in interp_il
+//   V^H order key (column band, class, row k0_0, column)   class 0 = column offset in the band >= 3 (stencil reaches into
+//             the next band), class 1 = the rest.  For one output row of one band the contributing samples are then
+//             three contiguous ranges (this band class 0, this band class 1, previous band class 0), each sorted by row.
+// y_il (the interleaved sample vectors) always uses the V^H order.
 static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, const std::vector<float>& delta,
                          const std::vector<double>& delta64) {
     const int64_t M = p->M;
     const int K0 = p->K[0], K1 = p->K[1], nb = K1 / kBandW;
     const double J = (double)kJ, beta = host::kb_beta(J, 2.0);
-    // counting sort, key = ((band * K0 + row) * 8 + (7 - column offset in the band))
-    const int64_t nbins = (int64_t)nb * K0 * kBandW;
-    std::vector<int32_t> binstart(nbins + 1, 0);
-    auto key_of = [&](uint32_t kp) -> int64_t {
-        const int r = kp & 1023u, c = (kp >> 10) & 1023u;
-        return ((int64_t)(c / kBandW) * K0 + r) * kBandW + (kBandW - 1 - (c % kBandW));
-    };
-    for (int64_t m = 0; m < M; ++m) binstart[key_of(kpack[m]) + 1]++;
-    for (int64_t b = 0; b < nbins; ++b) binstart[b + 1] += binstart[b];
-    std::vector<int32_t> perm(M);
-    {
+    auto row_of = [](uint32_t kp) { return (int)(kp & 1023u); };
+    auto col_of = [](uint32_t kp) { return (int)((kp >> 10) & 1023u); };
+    // counting sort by a key function over nbins bins; returns perm (sorted position -> caller sample) and bin starts
+    auto sort_by = [&](auto key_of, int64_t nbins, std::vector<int32_t>& perm, std::vector<int32_t>& binstart) {
+        binstart.assign(nbins + 1, 0);
+        for (int64_t m = 0; m < M; ++m) binstart[key_of(kpack[m]) + 1]++;
+        for (int64_t b = 0; b < nbins; ++b) binstart[b + 1] += binstart[b];
+        perm.resize(M);
         std::vector<int32_t> cur(binstart.begin(), binstart.end() - 1);
         for (int64_t m = 0; m < M; ++m) perm[cur[key_of(kpack[m])]++] = (int32_t)m;
-    }
+    };
+    // ---- V order
+    std::vector<int32_t> perm_v, bins_v;
+    sort_by([&](uint32_t kp) -> int64_t {
+        const int r = row_of(kp), c = col_of(kp);
+        return ((int64_t)(c / kBandW) * K0 + r) * kBandW + (c % kBandW);
+    }, (int64_t)nb * K0 * kBandW, perm_v, bins_v);
+    // ---- V^H order: bins (band, class, row)
+    std::vector<int32_t> perm_h, rowptr;
+    sort_by([&](uint32_t kp) -> int64_t {
+        const int r = row_of(kp), c = col_of(kp);
+        return ((int64_t)(c / kBandW) * 2 + ((c % kBandW) >= 3 ? 0 : 1)) * K0 + r;
+    }, (int64_t)nb * 2 * K0, perm_h, rowptr);
+    // rowptr[(band*2 + class) * K0 + r] .. [.. + r + 1]: samples of (band, class, row r); classes are adjacent, so the entry
+    // one past the last row of a class is the start of the next class / band.
+    std::vector<int32_t> pos_h(M);
+    for (int64_t i = 0; i < M; ++i) pos_h[perm_h[i]] = (int32_t)i;
     std::vector<uint32_t> kp_s(M);
     std::vector<float> dl_s((size_t)2 * M);
-    std::vector<float> wtab((size_t)M * kTabW, 0.f);
+    std::vector<int32_t> v2h(M);
     for (int64_t i = 0; i < M; ++i) {
-        const int64_t m = perm[i];
+        const int64_t m = perm_v[i];
         kp_s[i] = kpack[m];
         dl_s[i] = delta[m];
         dl_s[M + i] = delta[M + m];
+        v2h[i] = pos_h[m];
+    }
+    std::vector<float> wtab((size_t)M * kTabW, 0.f);
+    for (int64_t i = 0; i < M; ++i) {
+        const int64_t m = perm_h[i];
         double w0[kJ], w1[kJ];
         host::kb_weights_f64(delta64[m], J, beta, w0);
         host::kb_weights_f64(delta64[M + m], J, beta, w1);
         float* rec = &wtab[(size_t)i * kTabW];
         for (int j = 0; j < kJ; ++j) rec[j] = (float)w0[j];
-        const int off = ((kpack[m] >> 10) & 1023u) % kBandW;
+        const int32_t r = row_of(kpack[m]);
+        std::memcpy(&rec[6], &r, sizeof(r));             // stencil base row k0_0 (int bits)
+        const int off = col_of(kpack[m]) % kBandW;
         for (int j = 0; j < kJ; ++j) {
             const int c = off + j;                       // column relative to the start of the sample's own band
             if (c < kBandW) rec[8 + c] = (float)w1[j];   // part A: this band
             else rec[16 + c - kBandW] = (float)w1[j];    // part B: the next band
         }
     }
-    // row pointers; rowsplit = samples of (band, row) with column offset >= 3 (stencil reaches the next band)
-    std::vector<int32_t> rowptr((size_t)nb * (K0 + 1)), rowsplit((size_t)nb * K0);
-    for (int cb = 0; cb < nb; ++cb) {
-        for (int r = 0; r <= K0; ++r) {
-            const int64_t bin = ((int64_t)cb * K0 + std::min(r, K0 - 1)) * kBandW + (r == K0 ? kBandW : 0);
-            rowptr[(size_t)cb * (K0 + 1) + r] = binstart[bin];
-        }
-        for (int r = 0; r < K0; ++r) {
-            const int64_t bin = ((int64_t)cb * K0 + r) * kBandW;
-            rowsplit[(size_t)cb * K0 + r] = binstart[bin + (kBandW - 3)] - binstart[bin];   // offsets 7,6,5,4,3
-        }
-    }
     // work items: blocks of 8 rows; rows whose interaction count is far above the mean are split among warps
+    auto cnt_rows = [&](int cb, int cls, int r_lo, int r_hi) -> int64_t {      // rows r_lo..r_hi inclusive, no wrap
+        const size_t base = ((size_t)cb * 2 + cls) * K0;
+        return rowptr[base + r_hi + 1] - rowptr[base + r_lo];
+    };
     std::vector<int64_t> rowload((size_t)nb * K0);
     int64_t total = 0;
     for (int cb = 0; cb < nb; ++cb) {
         const int cbp = (cb + nb - 1) % nb;
         for (int r = 0; r < K0; ++r) {
             int64_t l = 0;
-            for (int j0 = 0; j0 < kJ; ++j0) {
-                const int rr = (r - j0 + K0) % K0;
-                l += rowptr[(size_t)cb * (K0 + 1) + rr + 1] - rowptr[(size_t)cb * (K0 + 1) + rr];
-                l += rowsplit[(size_t)cbp * K0 + rr];
-            }
+            auto add = [&](int lo, int hi) { l += cnt_rows(cb, 0, lo, hi) + cnt_rows(cb, 1, lo, hi) + cnt_rows(cbp, 0, lo, hi); };
+            if (r >= kJ - 1) add(r - (kJ - 1), r);
+            else { add(0, r); add(K0 - (kJ - 1) + r, K0 - 1); }
             rowload[(size_t)cb * K0 + r] = l;
             total += l;
         }
@@ -580,14 +594,10 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
     p->n_il_items = (int)items.size();
     NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_delta, dl_s, &p->bytes_plan));
-    {
-        std::vector<int32_t> pos(M);
-        for (int64_t i = 0; i < M; ++i) pos[perm[i]] = (int32_t)i;
-        NU_TRY(dev_upload(&p->d_il_pos, pos, &p->bytes_plan));
-    }
+    NU_TRY(dev_upload(&p->d_il_v2h, v2h, &p->bytes_plan));
+    NU_TRY(dev_upload(&p->d_il_pos, pos_h, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_wtab, wtab, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_rowptr, rowptr, &p->bytes_plan));
-    NU_TRY(dev_upload(&p->d_il_rowsplit, rowsplit, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_items, items, &p->bytes_plan));
     return NUFFT_OK;
 }
@@ -758,7 +768,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_scal); cudaFree(p->d_hist);
     cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
-    cudaFree(p->d_il_rowptr); cudaFree(p->d_il_rowsplit); cudaFree(p->d_il_items); cudaFree(p->d_yil);
+    cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     (void)cudaGetLastError();
     delete p;
     return NUFFT_OK;
