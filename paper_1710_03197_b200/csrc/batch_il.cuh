@@ -14,7 +14,8 @@
 //                            it walks the samples whose stencil covers that row (contiguous ranges of the
 //                            cell-sorted order, found through rowptr) and adds w0 * w1 * y.  No atomics, no
 //                            shared-memory read-modify-write, no zero-fill; every grid cell is written exactly once,
-//                            in a fixed summation order (bit-reproducible).
+//                            in a fixed summation order (bit-reproducible).  The contiguous table / sample ranges
+//                            of a CTA are staged in shared memory by bulk copies (cp.async.bulk + mbarrier).
 #pragma once
 #include "common.cuh"
 #include "fft.cuh"
@@ -273,10 +274,68 @@ __device__ __forceinline__ void il_accumulate(float2 (&acc)[kBandW], const float
     }
 }
 
+// ---- bulk-copy staging helpers (cp.async.bulk + mbarrier: the TMA engine moves contiguous plan / sample ranges into
+// shared memory; SASS: UBLKCP, SYNCS) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+constexpr int kStageCap = 48;      // samples per list per staging round
+constexpr int kGridSmemBytes = 3 * kStageCap * (kTabW * 4 + kIL * 8) + 16;
+
+// Adds staged samples [i0, i1) (indices into one staged list) to the 8 accumulators of output row `row`.
+template <int OFF>
+__device__ __forceinline__ void il_accumulate_smem(float2 (&acc)[kBandW], const float* __restrict__ rec_s,
+                                                   const float2* __restrict__ y_s, int row, int kmask, int i0, int i1) {
+#pragma unroll 4
+    for (int i = i0; i < i1; ++i) {
+        const float* rec = rec_s + i * kTabW;
+        const int j0 = (row - __float_as_int(rec[6])) & kmask;
+        const float w0 = rec[j0];
+        const float4 pa = *reinterpret_cast<const float4*>(rec + OFF);
+        const float4 pb = *reinterpret_cast<const float4*>(rec + OFF + 4);
+        const float2 yv = y_s[i * kIL];
+        const float tx = w0 * yv.x, ty = w0 * yv.y;
+        acc[0].x = fmaf(pa.x, tx, acc[0].x); acc[0].y = fmaf(pa.x, ty, acc[0].y);
+        acc[1].x = fmaf(pa.y, tx, acc[1].x); acc[1].y = fmaf(pa.y, ty, acc[1].y);
+        acc[2].x = fmaf(pa.z, tx, acc[2].x); acc[2].y = fmaf(pa.z, ty, acc[2].y);
+        acc[3].x = fmaf(pa.w, tx, acc[3].x); acc[3].y = fmaf(pa.w, ty, acc[3].y);
+        acc[4].x = fmaf(pb.x, tx, acc[4].x); acc[4].y = fmaf(pb.x, ty, acc[4].y);
+        acc[5].x = fmaf(pb.y, tx, acc[5].x); acc[5].y = fmaf(pb.y, ty, acc[5].y);
+        acc[6].x = fmaf(pb.z, tx, acc[6].x); acc[6].y = fmaf(pb.z, ty, acc[6].y);
+        acc[7].x = fmaf(pb.w, tx, acc[7].x); acc[7].y = fmaf(pb.w, ty, acc[7].y);
+    }
+}
+
+// CTA = one work item (band, nrows rows).  The samples that touch the item's rows are, per list (this band class 0,
+// this band class 1, previous band class 0), ONE contiguous range of the V^H order (two at the periodic row seam), so
+// their table records (96 B each) and their y_il rows (256 B each) are contiguous in global memory: one elected
+// thread issues bulk copies of up to kStageCap samples per list into shared memory, all warps wait on the mbarrier,
+// and every warp then accumulates its own row from shared memory.  Global-memory latency is paid once per round per
+// CTA instead of once per warp per four samples.
 __global__ void __launch_bounds__(256)
 gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const float2* __restrict__ y_il,
                    float2* __restrict__ grid_il) {
-    __shared__ float2 red[8][kBandW][kIL];
+    extern __shared__ __align__(128) unsigned char gsm[];
+    float2* y_s = reinterpret_cast<float2*>(gsm);                                           // [3][cap][32]
+    float* rec_s = reinterpret_cast<float*>(gsm + 3 * kStageCap * kIL * 8);                 // [3][cap][24]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(gsm + 3 * kStageCap * (kIL * 8 + kTabW * 4));
     const IlItem it = items[blockIdx.x];
     const int grp = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -284,33 +343,77 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
     const int row = it.r0 + (warp >> lsplit), part = warp & (nsplit - 1);
     const int K0 = g.K[0], K1 = g.K[1], nb = K1 / kBandW;
     const int cbp = (it.cb + nb - 1) % nb;
-    const float2* __restrict__ Y = y_il + (int64_t)grp * g.M * kIL + lane;
+    const float2* __restrict__ Y = y_il + (int64_t)grp * g.M * kIL;
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+    uint32_t phase = 0;
     float2 acc[kBandW];
 #pragma unroll
     for (int c = 0; c < kBandW; ++c) acc[c] = make_float2(0.f, 0.f);
-    // stencil base rows row-5 .. row (mod K0): one row segment, or two at the periodic seam
-    const int nseg = (row >= kJ - 1) ? 1 : 2;
+    // stencil base rows that touch the item: r0-5 .. r0+nrows-1 (mod K0): one row segment, or two at the seam
+    const int nseg = (it.r0 >= kJ - 1) ? 1 : 2;
 #pragma unroll 1
     for (int sg = 0; sg < nseg; ++sg) {
-        const int lo = (nseg == 1) ? row - (kJ - 1) : (sg == 0 ? 0 : K0 - (kJ - 1) + row);
-        const int hi = (nseg == 1 || sg == 0) ? row : K0 - 1;
+        const int slo = (sg == 0) ? max(it.r0 - (kJ - 1), 0) : K0 - (kJ - 1) + it.r0;
+        const int shi = (sg == 0) ? it.r0 + it.nrows - 1 : K0 - 1;
+        const int shift = (sg == 0) ? 0 : K0;
+        // CTA ranges (cb_, ce_) and this warp's ranges (wb_, we_) per list
+        int cbeg[3], cend[3], wbeg[3], wend[3];
+        const int wlo = max(slo, row + shift - (kJ - 1)), whi = min(shi, row + shift);
+        int rounds = 0;
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {     // this band class 0, this band class 1 (part A); previous band class 0 (part B)
+        for (int q = 0; q < 3; ++q) {
             const int base = ((q == 2 ? cbp : it.cb) * 2 + (q == 1 ? 1 : 0)) * K0;
-            const int b = __ldg(&s.rowptr[base + lo]), n = __ldg(&s.rowptr[base + hi + 1]) - b;
-            const int bb = b + ((n * part) >> lsplit), ee = b + ((n * (part + 1)) >> lsplit);
-            if (q == 2) il_accumulate<16>(acc, s.wtab, Y, row, K0 - 1, bb, ee);
-            else        il_accumulate<8>(acc, s.wtab, Y, row, K0 - 1, bb, ee);
+            cbeg[q] = __ldg(&s.rowptr[base + slo]);
+            cend[q] = __ldg(&s.rowptr[base + shi + 1]);
+            if (wlo <= whi) { wbeg[q] = __ldg(&s.rowptr[base + wlo]); wend[q] = __ldg(&s.rowptr[base + whi + 1]); }
+            else { wbeg[q] = 0; wend[q] = 0; }
+            rounds = max(rounds, (cend[q] - cbeg[q] + kStageCap - 1) / kStageCap);
+        }
+#pragma unroll 1
+        for (int k = 0; k < rounds; ++k) {
+            if (threadIdx.x == 0) {
+                uint32_t bytes = 0;
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    const int c0 = cbeg[q] + k * kStageCap, n = min(kStageCap, cend[q] - c0);
+                    if (n > 0) bytes += (uint32_t)n * (kTabW * 4 + kIL * 8);
+                }
+                mbar_expect_tx(bar, bytes);
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    const int c0 = cbeg[q] + k * kStageCap, n = min(kStageCap, cend[q] - c0);
+                    if (n > 0) {
+                        bulk_g2s(rec_s + q * kStageCap * kTabW, s.wtab + (int64_t)c0 * kTabW, (uint32_t)n * kTabW * 4, bar);
+                        bulk_g2s(y_s + q * kStageCap * kIL, Y + (int64_t)c0 * kIL, (uint32_t)n * kIL * 8, bar);
+                    }
+                }
+            }
+            mbar_wait(bar, phase);
+            phase ^= 1;
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                const int c0 = cbeg[q] + k * kStageCap, c1 = min(c0 + kStageCap, cend[q]);
+                const int x0 = max(wbeg[q], c0), x1 = min(wend[q], c1);       // my row's samples within the staged chunk
+                if (x1 > x0) {
+                    const int n = x1 - x0;
+                    const int i0 = x0 - c0 + ((n * part) >> lsplit), i1 = x0 - c0 + ((n * (part + 1)) >> lsplit);
+                    if (q == 2) il_accumulate_smem<16>(acc, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
+                    else        il_accumulate_smem<8>(acc, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
+                }
+            }
+            __syncthreads();      // every warp is done with the staged chunk before the next round overwrites it
         }
     }
-    if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row
+    if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row (staging area reused)
+        float2* red = y_s;  // [8][kBandW][32]
 #pragma unroll
-        for (int c = 0; c < kBandW; ++c) red[warp][c][lane] = acc[c];
+        for (int c = 0; c < kBandW; ++c) red[(warp * kBandW + c) * kIL + lane] = acc[c];
         __syncthreads();
         if (part != 0) return;
         for (int q = 1; q < nsplit; ++q)
 #pragma unroll
-            for (int c = 0; c < kBandW; ++c) acc[c] = cadd(acc[c], red[warp + q][c][lane]);
+            for (int c = 0; c < kBandW; ++c) acc[c] = cadd(acc[c], red[((warp + q) * kBandW + c) * kIL + lane]);
     }
     float2* __restrict__ dst = grid_il + (((int64_t)grp * K0 + row) * K1 + it.cb * kBandW) * kIL + lane;
 #pragma unroll

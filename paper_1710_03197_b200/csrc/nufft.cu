@@ -150,6 +150,7 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(gridding_il_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGridSmemBytes)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     return cudaSuccess;
 }
@@ -458,7 +459,7 @@ static int run_gridding_il(nufft_plan_t p, int batch, const float2* y_il, float2
     }
     const dim3 blocks((unsigned)p->n_il_items, (unsigned)il_groups(batch));
     ProfScope ps(p, "gridding", st);
-    gridding_il_kernel<<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid);
+    gridding_il_kernel<<<blocks, 256, kGridSmemBytes, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid);
     CU_TRY(cudaGetLastError());
     p->launches++;
     return NUFFT_OK;
