@@ -404,6 +404,47 @@ def extra_legs(nb, torch, peak, args):
     rows = kernel_table(p.profile(), algorithmic_bytes(3, N, K, M, 1, cov=0.55), peak)
     info = p.info()
     p.destroy()
+    # config 3: 2-D variable-density spiral 512^2, 50 CG iterations on A^H A x = A^H y (batch 1, planar path)
+    cfg = wl.config(2)
+    p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1)
+    xt = torch.from_numpy(wl.phantom(cfg["Nd"])).cuda().reshape(1, *cfg["Nd"])
+    y3 = p.forward(xt)
+    y3 = y3 + 0.01 * y3.abs().pow(2).mean().sqrt() * torch.randn_like(y3)
+    xs = p.solve_cg(y3, 3)
+    cg_ms = time_calls(lambda: p.solve_cg(y3, 50, x=xs), 3, flush)
+    sa_ms = time_calls(lambda: p.selfadjoint(xt, xt.clone()), 10, flush)
+    out["cfg3_2d_spiral_cg50"] = {"workload": "Nd=512^2 Kd=1024^2 M=262144 VD spiral, batch 1", "cg50_ms": cg_ms,
+                                  "ms_per_iteration": cg_ms / 50, "selfadjoint_ms": sa_ms,
+                                  "note": "linear CG on A^H A x = A^H y, x0 = 0, scalars float64 on device (R12)"}
+    p.destroy()
+    # config 5: 32-coil 2-D radial, multi-coil A^H A and 20 split-Bregman L1TV-OLS iterations (interleaved path)
+    cfg = wl.config(4)
+    nc = cfg["ncoil"]
+    p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=nc)
+    c = torch.from_numpy(wl.coil_maps(nc, cfg["Nd"])).cuda()
+    p.set_coils(c)
+    xt = torch.from_numpy(wl.phantom(cfg["Nd"])).cuda()
+    y5 = p.forward_coils(xt)
+    y5 = y5 + 0.01 * y5.abs().pow(2).mean().sqrt() * torch.randn_like(y5)
+    xo5 = p.selfadjoint_coils(xt)
+    xs = p.solve_l1tv_ols(y5, 1.0, 0.02, 1, 1, 1, use_coils=True)
+    sac_ms = time_calls(lambda: p.selfadjoint_coils(xt, xo5), 10, flush)
+    fwc_ms = time_calls(lambda: p.forward_coils(xt, y5), 10, flush)
+    adc_ms = time_calls(lambda: p.adjoint_coils(y5, xo5), 10, flush)
+    tv_ms = time_calls(lambda: p.solve_l1tv_ols(y5, 1.0, 0.02, 4, 5, 3, use_coils=True, x=xs), 3, flush)
+    out["cfg5_2d_multicoil_l1tv"] = {
+        "workload": "Nd=256^2 Kd=512^2 M=65536 radial 128x512, 32 coils", "forward_coils_ms": fwc_ms,
+        "adjoint_coils_ms": adc_ms, "selfadjoint_coils_ms": sac_ms, "l1tv_ols_20it_ms": tv_ms,
+        "coil_pairs_per_s": 32 * 1e3 / (fwc_ms + adc_ms),
+        "note": "n_outer=4, n_inner=5, n_cg=3, mu=1, lam=0.02 (R17); 32-coil batch on the interleaved grid"}
+    p.destroy()
+    # cuFFT reference point for F alone (never linked into the product): full 512^2 FFT of 64 grids via torch.fft
+    gref = torch.randn(64, 512, 512, dtype=torch.complex64, device="cuda")
+    torch.fft.fftn(gref, dim=(1, 2))
+    out["cufft_reference"] = {"what": "torch.fft.fftn (cuFFT) on [64][512][512] complex64, unpruned, no scaling/pad fused",
+                              "ms": time_calls(lambda: torch.fft.fftn(gref, dim=(1, 2)), 10, flush),
+                              "ours_F_ms": "roofline.stages_ms['F (S+pad+FFT)'] (pruned, S and zero-pad fused)"}
+    del gref
     out["cfg4_3d_kooshball"] = {
         "workload": "Nd=128^3 Kd=256^3 Jd=6^3 M=2097152 kooshball, batch 1", "forward_ms": f_ms, "adjoint_ms": a_ms,
         "pairs_per_s": 1e3 / (f_ms + a_ms), "kernels": rows, "plan": info,

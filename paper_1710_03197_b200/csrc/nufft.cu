@@ -680,7 +680,13 @@ static int plan_build(nufft_plan_t p, const double* om) {
     NU_TRY(dev_upload(&p->d_perm, perm, &p->bytes_plan));
     // V^H work items: (tile, sample range), hot tiles split into chunks of at most max_subtile samples
     {
-        int cap = p->opts.max_subtile > 0 ? p->opts.max_subtile : (d == 2 ? 1024 : 512);
+        // default: enough work items to fill the machine at this plan's batch size (148 SMs x ~16 resident warps), but
+        // at least 128 samples per item so that the tile flush stays a small share
+        int cap = p->opts.max_subtile;
+        if (cap <= 0) {
+            const int64_t fill = M * (int64_t)p->max_batch / (148 * 16);
+            cap = (d == 2) ? (int)std::max<int64_t>(128, std::min<int64_t>(1024, fill)) : 512;
+        }
         std::vector<WorkItem> items;
         std::vector<int32_t> tstart(p->n_tiles + 1, 0);
         for (int64_t t = 0; t < p->n_tiles; ++t) {
