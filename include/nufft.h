@@ -61,7 +61,8 @@ typedef struct {
                                (summation order across tiles free: reproducible to rounding only);
                            1 = deterministic: tiles flushed to private slabs and summed in fixed order
                                (bit-reproducible run to run)                                                      */
-    int interp_mode;    /* 0 = V gathers straight from the grid through L1/L2; 1 = tile staged in shared memory */
+    int interp_mode;    /* 0 = library default: 3-D planar V stages the padded tile of a work item in shared memory
+                               (half-warp per sample), 2-D planar V gathers through L1/L2; 1 = always direct gather */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
     int use_graphs;     /* 1 = capture forward/adjoint/selfadjoint into CUDA graphs on first use (default 0)     */

@@ -150,6 +150,7 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(interp_tiled_3d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kInterp3dSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_il_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGridSmemBytes)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     return cudaSuccess;
@@ -302,8 +303,16 @@ static SampleData sample_data(nufft_plan_t p) {
 // a3: y = V grid
 static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, cudaStream_t st) {
     if (p->M == 0) return NUFFT_OK;
-    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
     ProfScope ps(p, "interp", st);
+    if (p->d == 3 && p->opts.interp_mode == 0 && p->tile[0] == k3T0 && p->tile[1] == k3T1 && p->tile[2] == k3T2 && p->n_items > 0) {
+        // tile-staged V (default tile only); interp_mode = 1 keeps the direct gather
+        const dim3 tb((unsigned)p->n_items, (unsigned)batch);
+        interp_tiled_3d_kernel<<<tb, 256, kInterp3dSmem, st>>>(sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+        return NUFFT_OK;
+    }
+    const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
     if (p->d == 2) interp_direct_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     else           interp_direct_kernel<3><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     CU_TRY(cudaGetLastError());

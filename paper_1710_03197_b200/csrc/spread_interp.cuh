@@ -354,3 +354,103 @@ gridding_merge_kernel(GridGeom g, TileGeom tg, int nt0, int nt1, int nt2, const 
     grid[(int64_t)b * g.cells + cell] = acc;
 }
 }  // namespace nufft
+
+namespace nufft {
+// ============================================================================================================
+// Tiled V, 3-D (step a3), batch 1.  profiles/r01b + the 3-D capture: with one thread per sample every load
+// instruction of a warp touches ~16 sectors in as many lines and the L1 data pipe saturates (l1tex 98 %).  Here a CTA
+// owns one work item (tile 8 x 8 x 16 cells + halo, sample range): it stages the padded tile (13 x 13 x 24 cells,
+// 32 KB) in shared memory with coalesced 16-byte loads and then every HALF-WARP interpolates one sample: lane
+// (rr, cc) reads cell (row 2g + rr, column cc) of an 8-cell window of stencil plane p -- two 64-byte row segments per
+// half-warp load, bank-conflict free because the row pitch is 8 (mod 16) cells -- 18 loads per sample pair instead
+// of 216 per sample, then a 4-step shuffle reduction.  Weights: one thread per sample evaluates kb_weights and parks
+// w0[6], w1[6], w2[6] (zero-padded to 8) in shared memory.
+// ============================================================================================================
+constexpr int k3T0 = 8, k3T1 = 8, k3T2 = 16;
+constexpr int k3P0 = k3T0 + kJ - 1, k3P1 = k3T1 + kJ - 1;      // 13 x 13 padded rows
+constexpr int k3Pitch = 24;                                    // cells per padded row (8 mod 16), >= 16 + 5 + 2
+constexpr int k3Plane = k3P1 * k3Pitch;
+constexpr int k3Cells = k3P0 * k3Plane;                        // 4056 cells = 32448 B
+constexpr int k3Chunk = 128;                                   // samples whose weights are staged at a time
+constexpr int k3RecW = 28;                                     // floats per staged sample record
+constexpr int kInterp3dSmem = k3Cells * 8 + k3Chunk * k3RecW * 4;
+
+__global__ void __launch_bounds__(256)
+interp_tiled_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ items, const float2* __restrict__ grid,
+                       float2* __restrict__ y, KernelPoly P) {
+    extern __shared__ float4 smem4[];
+    float2* tile = reinterpret_cast<float2*>(smem4);
+    float* recs = reinterpret_cast<float*>(tile + k3Cells);
+    const WorkItem wi = items[blockIdx.x];
+    const int b = blockIdx.y;
+    int o[3];
+    unpack_k0(wi.origin, o);
+    const int K0 = g.K[0], K1 = g.K[1], K2 = g.K[2];
+    const float2* __restrict__ G = grid + (int64_t)b * g.cells;
+    // stage the padded tile: 169 rows x 12 float4 (24 cells); rows and the 16-byte pairs wrap periodically
+    for (int idx = threadIdx.x; idx < k3P0 * k3P1 * (k3Pitch / 2); idx += blockDim.x) {
+        const int row = idx / (k3Pitch / 2), c4 = idx - row * (k3Pitch / 2);
+        const int lx = row / k3P1, ly = row - lx * k3P1;
+        const int gx = (o[0] + lx) & (K0 - 1), gy = (o[1] + ly) & (K1 - 1), gz = (o[2] + 2 * c4) & (K2 - 1);
+        reinterpret_cast<float4*>(tile)[idx] =
+            __ldg(reinterpret_cast<const float4*>(G + ((int64_t)gx * K1 + gy) * K2 + gz));
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int half = lane >> 4, rr = (lane >> 3) & 1, cc = lane & 7;
+    const int lane_off = rr * k3Pitch + cc;
+    float2* __restrict__ yb = y + (int64_t)b * g.M;
+    for (int c0 = wi.s_begin; c0 < wi.s_end; c0 += k3Chunk) {
+        const int cnt = min(k3Chunk, wi.s_end - c0);
+        __syncthreads();          // tile staged (first pass) / previous chunk's records consumed
+        for (int t = threadIdx.x; t < cnt; t += blockDim.x) {
+            const int si = c0 + t;
+            int k0[3];
+            unpack_k0(__ldg(&s.kpack[si]), k0);
+            float w0[kJ], w1[kJ], w2[kJ];
+            kb_weights(P, __ldg(&s.delta[si]), w0);
+            kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
+            kb_weights(P, __ldg(&s.delta[2 * g.M + si]), w2);
+            float4* r = reinterpret_cast<float4*>(recs + t * k3RecW);
+            r[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
+            r[1] = make_float4(w0[4], w0[5], 0.f, 0.f);
+            r[2] = make_float4(w1[0], w1[1], w1[2], w1[3]);
+            r[3] = make_float4(w1[4], w1[5], 0.f, 0.f);
+            r[4] = make_float4(w2[0], w2[1], w2[2], w2[3]);
+            r[5] = make_float4(w2[4], w2[5], 0.f, 0.f);
+            const int l0 = (k0[0] - o[0]) & (K0 - 1), l1 = (k0[1] - o[1]) & (K1 - 1), l2 = (k0[2] - o[2]) & (K2 - 1);
+            r[6] = make_float4(__int_as_float(l0 * k3Plane + l1 * k3Pitch + l2), __int_as_float(__ldg(&s.perm[si])), 0.f, 0.f);
+        }
+        __syncthreads();
+        // half-warp per sample; a warp handles sample pairs warp*2 + half, + 16, ...
+        for (int t0 = warp * 2; t0 < cnt; t0 += 16) {
+            const int t = t0 + half;
+            const bool valid = t < cnt;
+            const float* rec = recs + (valid ? t : t0) * k3RecW;
+            const float4 wa = *reinterpret_cast<const float4*>(rec), wb = *reinterpret_cast<const float4*>(rec + 4);
+            const float w0[kJ] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y};
+            const float wc = rec[16 + cc];
+            const float w12[3] = {rec[8 + rr] * wc, rec[10 + rr] * wc, rec[12 + rr] * wc};
+            const float2* __restrict__ tp = tile + __float_as_int(rec[24]) + lane_off;
+            float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int p = 0; p < kJ; ++p) {
+                float2 tsum = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int gq = 0; gq < 3; ++gq) {
+                    const float2 v = tp[p * k3Plane + 2 * gq * k3Pitch];
+                    tsum.x = fmaf(w12[gq], v.x, tsum.x);
+                    tsum.y = fmaf(w12[gq], v.y, tsum.y);
+                }
+                acc.x = fmaf(w0[p], tsum.x, acc.x);
+                acc.y = fmaf(w0[p], tsum.y, acc.y);
+            }
+#pragma unroll
+            for (int off = 8; off > 0; off >>= 1) {
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, off);
+                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, off);
+            }
+            if (valid && (lane & 15) == 0) yb[__float_as_int(rec[25])] = acc;
+        }
+    }
+}
+}  // namespace nufft
