@@ -103,12 +103,12 @@ __device__ __forceinline__ void twiddle_powers(float2* v, float2 w) {
 //   interleaved (element stride T);  TS: lines per CTA of the strided kernels;  LC: lines per CTA, contiguous kernels
 // ------------------------------------------------------------------------------------------------------------
 template <int K> struct Rad;
-template <> struct Rad<32>   { static constexpr int R1 = 8,  R2 = 4,  R3 = 1, E = 8,  PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32; };
-template <> struct Rad<64>   { static constexpr int R1 = 8,  R2 = 8,  R3 = 1, E = 8,  PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32; };
-template <> struct Rad<128>  { static constexpr int R1 = 16, R2 = 8,  R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32; };
-template <> struct Rad<256>  { static constexpr int R1 = 16, R2 = 16, R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 16; };
-template <> struct Rad<512>  { static constexpr int R1 = 8,  R2 = 8,  R3 = 8, E = 8,  PC1 = 8, PC2 = 1, PS1 = 0, PS2 = 1, TS = 8,  LC = 4;  };
-template <> struct Rad<1024> { static constexpr int R1 = 16, R2 = 8,  R3 = 8, E = 16, PC1 = 8, PC2 = 1, PS1 = 0, PS2 = 1, TS = 8,  LC = 4;  };
+template <> struct Rad<32>   { static constexpr int R1 = 8,  R2 = 4,  R3 = 1, E = 8,  PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32, MBS = 1; };
+template <> struct Rad<64>   { static constexpr int R1 = 8,  R2 = 8,  R3 = 1, E = 8,  PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32, MBS = 1; };
+template <> struct Rad<128>  { static constexpr int R1 = 16, R2 = 8,  R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32, MBS = 1; };
+template <> struct Rad<256>  { static constexpr int R1 = 16, R2 = 16, R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 16, MBS = 1; };
+template <> struct Rad<512>  { static constexpr int R1 = 8,  R2 = 8,  R3 = 8, E = 8,  PC1 = 8, PC2 = 1, PS1 = 0, PS2 = 1, TS = 8,  LC = 4, MBS = 3;  };
+template <> struct Rad<1024> { static constexpr int R1 = 16, R2 = 8,  R3 = 8, E = 16, PC1 = 8, PC2 = 1, PS1 = 0, PS2 = 1, TS = 8,  LC = 4, MBS = 1;  };
 
 template <int K> struct FftGeom {
     using C = Rad<K>;
@@ -323,7 +323,7 @@ struct ColPassParams {
 };
 
 template <int K, bool ADJ>
-__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS, Rad<K>::MBS)
 fft_cols_kernel(ColPassParams p) {
     using G = FftGeom<K>;
     constexpr int T = Rad<K>::TS, TPL = G::TPL;
