@@ -236,10 +236,9 @@ def run_ours(args):
         plan.adjoint(y, xo)
 
     def step_e2e():
-        xd = x_host.to("cuda", non_blocking=True)
-        plan.forward(xd, y)
-        plan.adjoint(y, xo)
-        xo_host.copy_(xo, non_blocking=True)
+        # the pair through the host-buffer C-ABI call: pinned x -> H2D -> A -> A^H -> D2H x' (y stays on the device),
+        # chunked copy/compute pipeline inside the library (nufft_selfadjoint_host)
+        plan.selfadjoint_host(x_host, xo_host)
 
     def timed(fn, nsteps):
         evs = []
@@ -332,7 +331,9 @@ def run_ours(args):
             "clocks": clocks,
             "e2e": {"value": world * B / (e2e_ms / K_steps * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": int(x_host.numel() * 8), "d2h_bytes_per_step": int(xo_host.numel() * 8),
-                    "ms_per_step": e2e_ms / K_steps},
+                    "ms_per_step": e2e_ms / K_steps,
+                    "call": "nufft_selfadjoint_host: A^H(A x) per image, y kept on the device, 32-image chunks pipelined "
+                            "H2D / kernels / D2H"},
             "gpu_launches": int(l1 - l0),
             "roofline": roofline,
             "cpu_baseline": {"value": 1.0 / cpu_s, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",

@@ -92,6 +92,16 @@ int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64 *y, nufft_c64 *x, v
 /* x_out[b] = A^H A x_in[b], the intermediate samples stay in the plan's workspace.   eq.(5), R8 */
 int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
 
+/* The same three transforms on HOST buffers (bench.py's end-to-end leg).  x / y are host pointers, read / written
+ * asynchronously: they must stay valid until `stream` has passed this call, and should be page-locked (pinned) --
+ * pageable memory works but serialises the copies.  The batch is cut into chunks (32 images on the interleaved path);
+ * chunk c+1 is copied in on an internal copy stream while the kernels of chunk c run on `stream` and chunk c-1 is
+ * copied back on a second copy stream; `stream` is made to wait for the last copy back before the call's work counts
+ * as finished.  Device staging buffers (2 x 2 chunks) belong to the plan. */
+int nufft_forward_host(nufft_plan_t p, int batch, const nufft_c64 *x_host, nufft_c64 *y_host, void *stream);
+int nufft_adjoint_host(nufft_plan_t p, int batch, const nufft_c64 *y_host, nufft_c64 *x_host, void *stream);
+int nufft_selfadjoint_host(nufft_plan_t p, int batch, const nufft_c64 *x_in_host, nufft_c64 *x_out_host, void *stream);
+
 /* The four stages on their own (used by the per-stage parity tests and the per-stage timings).
  * grid: device [batch][prod Kd] complex64 in natural FFT order (k = 0 is index 0), caller-owned.
  *   scale_fft:  grid = F S x          (a1+a2)      fft_scale: x = S^H F^H grid   (a5+a6; grid is DESTROYED)

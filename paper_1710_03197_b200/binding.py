@@ -16,6 +16,7 @@ _I64P = _c.POINTER(_c.c_int64)
 
 EXPORTED_SYMBOLS = [
     "nufft_default_opts", "nufft_plan", "nufft_forward", "nufft_adjoint", "nufft_selfadjoint",
+    "nufft_forward_host", "nufft_adjoint_host", "nufft_selfadjoint_host",
     "nufft_stage_scale_fft", "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale",
     "nufft_set_coils", "nufft_forward_coils", "nufft_adjoint_coils", "nufft_selfadjoint_coils",
     "nufft_solve_cg", "nufft_solve_l1tv_ols", "nufft_plan_info", "nufft_launch_count", "nufft_destroy",
@@ -55,7 +56,8 @@ def lib():
     L.nufft_default_opts.argtypes = [_c.POINTER(NufftOpts)]
     L.nufft_plan.argtypes = [_c.c_int, _I64P, _I64P, _c.POINTER(_c.c_int), _c.c_int64, _c.POINTER(_c.c_double),
                              _c.c_int, _c.POINTER(NufftOpts), _c.POINTER(_PLAN)]
-    for name in ("nufft_forward", "nufft_adjoint", "nufft_selfadjoint", "nufft_stage_scale_fft",
+    for name in ("nufft_forward", "nufft_adjoint", "nufft_selfadjoint", "nufft_forward_host", "nufft_adjoint_host",
+                 "nufft_selfadjoint_host", "nufft_stage_scale_fft",
                  "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale"):
         getattr(L, name).argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR]
     L.nufft_set_coils.argtypes = [_PLAN, _c.c_int, _PTR]
@@ -300,22 +302,39 @@ class NufftPlan:
             out[name.value.decode()] = (float(ms.value), int(n.value))
         return out
 
-    # -- host-buffer convenience (the e2e path) ---------------------------------------------------------------
-    def forward_host(self, x_host, y_host=None):
-        """x_host: pinned (or pageable) CPU complex64 tensor [b][Nd] -> y_host CPU tensor [b][M]."""
+    # -- host-buffer transforms (the e2e path): marshalling only, the chunked copy/compute pipeline is in the library --
+    @staticmethod
+    def _hostptr(t, what, numel):
         import torch
-        xd = x_host.to("cuda", non_blocking=True)
-        yd = self.forward(xd)
-        if y_host is None:
-            y_host = torch.empty(yd.shape, dtype=torch.complex64, pin_memory=True)
-        y_host.copy_(yd, non_blocking=True)
+        if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.complex64 or not t.is_contiguous():
+            raise TypeError("%s must be a contiguous complex64 CPU tensor (pinned for overlap)" % what)
+        if t.numel() != numel:
+            raise ValueError("%s has %d elements, expected %d" % (what, t.numel(), numel))
+        return _c.c_void_p(t.data_ptr())
+
+    def _new_host(self, *shape):
+        import torch
+        return torch.empty(shape, dtype=torch.complex64, pin_memory=True)
+
+    def forward_host(self, x_host, y_host=None):
+        """x_host: pinned CPU complex64 [b][Nd] -> y_host pinned CPU [b][M].  Asynchronous on the current stream."""
+        b = self._batch_of(x_host, self.nimg)
+        y_host = self._new_host(b, self.M) if y_host is None else y_host
+        _check(lib().nufft_forward_host(self._h, b, self._hostptr(x_host, "x_host", b * self.nimg),
+                                        self._hostptr(y_host, "y_host", b * self.M), _stream()), "nufft_forward_host")
         return y_host
 
     def adjoint_host(self, y_host, x_host=None):
-        import torch
-        yd = y_host.to("cuda", non_blocking=True)
-        xd = self.adjoint(yd)
-        if x_host is None:
-            x_host = torch.empty(xd.shape, dtype=torch.complex64, pin_memory=True)
-        x_host.copy_(xd, non_blocking=True)
+        b = self._batch_of(y_host, self.M)
+        x_host = self._new_host(b, *self.Nd) if x_host is None else x_host
+        _check(lib().nufft_adjoint_host(self._h, b, self._hostptr(y_host, "y_host", b * self.M),
+                                        self._hostptr(x_host, "x_host", b * self.nimg), _stream()), "nufft_adjoint_host")
         return x_host
+
+    def selfadjoint_host(self, x_host, out_host=None):
+        b = self._batch_of(x_host, self.nimg)
+        out_host = self._new_host(b, *self.Nd) if out_host is None else out_host
+        _check(lib().nufft_selfadjoint_host(self._h, b, self._hostptr(x_host, "x_host", b * self.nimg),
+                                            self._hostptr(out_host, "out_host", b * self.nimg), _stream()),
+               "nufft_selfadjoint_host")
+        return out_host

@@ -83,6 +83,13 @@ struct nufft_plan_s {
     IlItem* d_il_items = nullptr;
     int n_il_items = 0;
     float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
+    // host-buffer pipeline (nufft_*_host): copy streams, events, double-buffered device staging, lazy
+    bool hp_ready = false;
+    int hp_chunk = 1;
+    cudaStream_t hp_h2d = nullptr, hp_d2h = nullptr;
+    cudaEvent_t hp_in[2] = {nullptr, nullptr}, hp_cmp[2] = {nullptr, nullptr}, hp_out[2] = {nullptr, nullptr}, hp_start = nullptr;
+    float2* hp_din[2] = {nullptr, nullptr};
+    float2* hp_dout[2] = {nullptr, nullptr};
     // optional per-kernel event timing (nufft_profile_*)
     bool prof_on = false;
     struct ProfRec { int label; cudaEvent_t a, b; };
@@ -785,6 +792,15 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
+    if (p->hp_h2d) cudaStreamDestroy(p->hp_h2d);
+    if (p->hp_d2h) cudaStreamDestroy(p->hp_d2h);
+    for (int i = 0; i < 2; ++i) {
+        if (p->hp_in[i]) cudaEventDestroy(p->hp_in[i]);
+        if (p->hp_cmp[i]) cudaEventDestroy(p->hp_cmp[i]);
+        if (p->hp_out[i]) cudaEventDestroy(p->hp_out[i]);
+        cudaFree(p->hp_din[i]); cudaFree(p->hp_dout[i]);
+    }
+    if (p->hp_start) cudaEventDestroy(p->hp_start);
     (void)cudaGetLastError();
     delete p;
     return NUFFT_OK;
@@ -899,6 +915,80 @@ extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_i
     NU_TRY(run_interp(p, batch, p->d_grid, p->d_ywork, st));
     NU_TRY(run_gridding(p, batch, p->d_ywork, p->d_grid, st));
     return run_fft_scale(p, batch, p->d_grid, (float2*)x_out, nullptr, st);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host-buffer transforms: chunked pipeline  H2D (copy stream) -> kernels (caller's stream) -> D2H (second copy stream)
+// ------------------------------------------------------------------------------------------------------------
+static int host_pipe_init(nufft_plan_t p) {
+    if (p->hp_ready) return NUFFT_OK;
+    CU_TRY(cudaStreamCreateWithFlags(&p->hp_h2d, cudaStreamNonBlocking));
+    CU_TRY(cudaStreamCreateWithFlags(&p->hp_d2h, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        CU_TRY(cudaEventCreateWithFlags(&p->hp_in[i], cudaEventDisableTiming));
+        CU_TRY(cudaEventCreateWithFlags(&p->hp_cmp[i], cudaEventDisableTiming));
+        CU_TRY(cudaEventCreateWithFlags(&p->hp_out[i], cudaEventDisableTiming));
+    }
+    CU_TRY(cudaEventCreateWithFlags(&p->hp_start, cudaEventDisableTiming));
+    p->hp_chunk = std::min(p->max_batch, p->il_ok ? kIL : 8);
+    const size_t per = (size_t)std::max<int64_t>(p->nimg, std::max<int64_t>(p->M, 1)) * sizeof(float2);
+    for (int i = 0; i < 2; ++i) {
+        NU_TRY(dev_alloc((void**)&p->hp_din[i], (size_t)p->hp_chunk * per, &p->bytes_work));
+        NU_TRY(dev_alloc((void**)&p->hp_dout[i], (size_t)p->hp_chunk * per, &p->bytes_work));
+    }
+    p->hp_ready = true;
+    return NUFFT_OK;
+}
+
+// kind: 0 = forward (in: images, out: samples), 1 = adjoint (in: samples, out: images), 2 = selfadjoint (images both)
+static int host_pipeline(nufft_plan_t p, int kind, int batch, const nufft_c64* in_host, nufft_c64* out_host,
+                         cudaStream_t st) {
+    NU_TRY(host_pipe_init(p));
+    const int64_t n_in = (kind == 1) ? p->M : p->nimg, n_out = (kind == 0) ? p->M : p->nimg;
+    const int CH = p->hp_chunk;
+    CU_TRY(cudaEventRecord(p->hp_start, st));
+    CU_TRY(cudaStreamWaitEvent(p->hp_h2d, p->hp_start, 0));
+    CU_TRY(cudaStreamWaitEvent(p->hp_d2h, p->hp_start, 0));
+    int c = 0;
+    for (int b0 = 0; b0 < batch; b0 += CH, ++c) {
+        const int n = std::min(CH, batch - b0), buf = c & 1;
+        if (c >= 2) CU_TRY(cudaStreamWaitEvent(p->hp_h2d, p->hp_cmp[buf], 0));      // kernels of chunk c-2 have read din[buf]
+        if (n_in > 0)
+            CU_TRY(cudaMemcpyAsync(p->hp_din[buf], (const float2*)in_host + (int64_t)b0 * n_in,
+                                   (size_t)n * n_in * sizeof(float2), cudaMemcpyHostToDevice, p->hp_h2d));
+        CU_TRY(cudaEventRecord(p->hp_in[buf], p->hp_h2d));
+        CU_TRY(cudaStreamWaitEvent(st, p->hp_in[buf], 0));
+        if (c >= 2) CU_TRY(cudaStreamWaitEvent(st, p->hp_out[buf], 0));             // D2H of chunk c-2 has read dout[buf]
+        int rc;
+        if (kind == 0) rc = nufft_forward(p, n, (const nufft_c64*)p->hp_din[buf], (nufft_c64*)p->hp_dout[buf], st);
+        else if (kind == 1) rc = nufft_adjoint(p, n, (const nufft_c64*)p->hp_din[buf], (nufft_c64*)p->hp_dout[buf], st);
+        else rc = nufft_selfadjoint(p, n, (const nufft_c64*)p->hp_din[buf], (nufft_c64*)p->hp_dout[buf], st);
+        NU_TRY(rc);
+        CU_TRY(cudaEventRecord(p->hp_cmp[buf], st));
+        CU_TRY(cudaStreamWaitEvent(p->hp_d2h, p->hp_cmp[buf], 0));
+        if (n_out > 0)
+            CU_TRY(cudaMemcpyAsync((float2*)out_host + (int64_t)b0 * n_out, p->hp_dout[buf],
+                                   (size_t)n * n_out * sizeof(float2), cudaMemcpyDeviceToHost, p->hp_d2h));
+        CU_TRY(cudaEventRecord(p->hp_out[buf], p->hp_d2h));
+    }
+    // join: the caller's stream continues only after the last copies back
+    CU_TRY(cudaStreamWaitEvent(st, p->hp_out[0], 0));
+    if (c >= 2) CU_TRY(cudaStreamWaitEvent(st, p->hp_out[1], 0));
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_forward_host(nufft_plan_t p, int batch, const nufft_c64* x_host, nufft_c64* y_host, void* stream) {
+    if (bad_batch(p, batch) || !x_host || (!y_host && p->M > 0)) return NUFFT_EINVAL;
+    return host_pipeline(p, 0, batch, x_host, y_host, (cudaStream_t)stream);
+}
+extern "C" int nufft_adjoint_host(nufft_plan_t p, int batch, const nufft_c64* y_host, nufft_c64* x_host, void* stream) {
+    if (bad_batch(p, batch) || !x_host || (!y_host && p->M > 0)) return NUFFT_EINVAL;
+    return host_pipeline(p, 1, batch, y_host, x_host, (cudaStream_t)stream);
+}
+extern "C" int nufft_selfadjoint_host(nufft_plan_t p, int batch, const nufft_c64* x_in_host, nufft_c64* x_out_host,
+                                      void* stream) {
+    if (bad_batch(p, batch) || !x_in_host || !x_out_host) return NUFFT_EINVAL;
+    return host_pipeline(p, 2, batch, x_in_host, x_out_host, (cudaStream_t)stream);
 }
 
 // ------------------------------------------------------------------------------------------------------------
