@@ -75,6 +75,23 @@ def algorithmic_bytes(d, N, K, M, B, cov=1.0):
     }
 
 
+def max_over_ranks(values, world, device):
+    """Replicas-only multi-GPU timing rule: every rank times its own replica on its device, the job's time is the MAX
+    over ranks (one all-reduce of a few scalars, outside the timed region; no collective in the data path)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_pairs_per_s(world, batch, ms_per_step):
+    """Whole-job throughput of `world` independent replicas that each process `batch` pairs per step (weak scaling)."""
+    return world * batch / (ms_per_step * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -277,10 +294,7 @@ def run_ours(args):
     e2e_ms = timed(step_e2e, K_steps)
     barrier()
 
-    if world > 1:
-        t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_ms = float(t[0]), float(t[1])
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, "cuda")
 
     # per-kernel device times of the same step (library-side CUDA events on the launch stream)
     peak, peak_src = measured_peak()
@@ -293,7 +307,7 @@ def run_ours(args):
     result = None
     if rank == 0:
         ms_per_step = total_ms / K_steps
-        value = world * B / (ms_per_step * 1e-3)
+        value = aggregate_pairs_per_s(world, B, ms_per_step)
         timed_kernels = {k: v for k, v in rows.items() if "alg_bytes" in v}
         dom = max(timed_kernels, key=lambda k: timed_kernels[k]["ms_per_launch"])
         traffic = None
