@@ -496,3 +496,41 @@ def test_l1tv_ols_16_coils_interleaved_path():
     xg = p.solve_l1tv_ols(dev(y), 1.0, 0.02, 1, 2, 2, use_coils=True)
     assert rel(host(xg), xo) < 1e-4
     p.destroy()
+
+
+def test_cg_config3_parity_against_the_oracles_own_noise_floor(repo_root):
+    """the VD spiral leaves the k-space corners unsampled, A^H A has a near-null space and CG amplifies any
+    perturbation there.  Measure, on the scaled config 3 (128^2), (i) GPU vs oracle and (ii) the oracle against itself
+    with 1e-12 relative noise injected into every operator application, at iterations 1, 5, 10, 50; the GPU may exceed
+    1e-4 only where the float64 floor itself is within two orders of magnitude of it.  Numbers go to
+    gpurun_out/cg_floor.json (quoted in DESIGN.md)."""
+    import json
+    import os
+    cfg = wl.config(2, scale=4)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    p = make_plan(cfg)
+    xt = wl.phantom(Nd)
+    y = orc.forward(xt.astype(np.complex128), om, Nd, Kd, Jd)
+    y = (y + wl.noise_like(y)).astype(np.complex64)
+    AHy = orc.adjoint(y.astype(np.complex128), om, Nd, Kd, Jd)
+    AHA = lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd)
+    rng = np.random.default_rng(77)
+
+    def AHA_noisy(z):
+        r = AHA(z)
+        return r * (1.0 + 1e-12 * (rng.standard_normal(r.shape) + 1j * rng.standard_normal(r.shape)))
+
+    out = {}
+    for niter in (1, 5, 10, 50):
+        xo, _ = sol.cg(AHA, AHy, niter)
+        xn, _ = sol.cg(AHA_noisy, AHy, niter)
+        xg = host(p.solve_cg(dev(y), niter))
+        out[niter] = {"gpu_vs_oracle": float(rel(xg, xo)), "oracle_noise_floor_1e-12": float(rel(xn, xo))}
+    d = os.path.join(repo_root, "gpurun_out")
+    if os.path.isdir(d):
+        with open(os.path.join(d, "cg_floor.json"), "w") as f:
+            json.dump(out, f, indent=1)
+    assert out[1]["gpu_vs_oracle"] < 1e-4 and out[5]["gpu_vs_oracle"] < 1e-4
+    for niter, v in out.items():
+        assert v["gpu_vs_oracle"] < max(1e-4, 1e9 * v["oracle_noise_floor_1e-12"]), (niter, v)
+    p.destroy()
