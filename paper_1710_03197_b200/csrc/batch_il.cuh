@@ -299,10 +299,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 constexpr int kStageCap = 48;      // samples per list per staging round
 constexpr int kGridSmemBytes = 3 * kStageCap * (kTabW * 4 + kIL * 8) + 16;
 
-// Adds staged samples [i0, i1) (indices into one staged list) to the 8 accumulators of output row `row`.
+// Adds staged samples [i0, i1) (indices into one staged list) to the accumulators of output row `row`.
+// Accumulators are kept as packed pairs for Blackwell's two-wide FP32 FMA (fma.rn.f32x2, SASS FFMA2):
+// ax[k] = (re of cell 2k, re of cell 2k+1), ay[k] = the imaginary parts; the weight pair of two adjacent cells is one
+// aligned register pair straight out of the 128-bit table load, so one FFMA2 updates two cells.
 template <int OFF>
-__device__ __forceinline__ void il_accumulate_smem(float2 (&acc)[kBandW], const float* __restrict__ rec_s,
-                                                   const float2* __restrict__ y_s, int row, int kmask, int i0, int i1) {
+__device__ __forceinline__ void il_accumulate_smem(float2 (&ax)[kBandW / 2], float2 (&ay)[kBandW / 2],
+                                                   const float* __restrict__ rec_s, const float2* __restrict__ y_s,
+                                                   int row, int kmask, int i0, int i1) {
 #pragma unroll 4
     for (int i = i0; i < i1; ++i) {
         const float* rec = rec_s + i * kTabW;
@@ -312,14 +316,11 @@ __device__ __forceinline__ void il_accumulate_smem(float2 (&acc)[kBandW], const 
         const float4 pb = *reinterpret_cast<const float4*>(rec + OFF + 4);
         const float2 yv = y_s[i * kIL];
         const float tx = w0 * yv.x, ty = w0 * yv.y;
-        acc[0].x = fmaf(pa.x, tx, acc[0].x); acc[0].y = fmaf(pa.x, ty, acc[0].y);
-        acc[1].x = fmaf(pa.y, tx, acc[1].x); acc[1].y = fmaf(pa.y, ty, acc[1].y);
-        acc[2].x = fmaf(pa.z, tx, acc[2].x); acc[2].y = fmaf(pa.z, ty, acc[2].y);
-        acc[3].x = fmaf(pa.w, tx, acc[3].x); acc[3].y = fmaf(pa.w, ty, acc[3].y);
-        acc[4].x = fmaf(pb.x, tx, acc[4].x); acc[4].y = fmaf(pb.x, ty, acc[4].y);
-        acc[5].x = fmaf(pb.y, tx, acc[5].x); acc[5].y = fmaf(pb.y, ty, acc[5].y);
-        acc[6].x = fmaf(pb.z, tx, acc[6].x); acc[6].y = fmaf(pb.z, ty, acc[6].y);
-        acc[7].x = fmaf(pb.w, tx, acc[7].x); acc[7].y = fmaf(pb.w, ty, acc[7].y);
+        const float2 txx = make_float2(tx, tx), tyy = make_float2(ty, ty);
+        ax[0] = __ffma2_rn(make_float2(pa.x, pa.y), txx, ax[0]); ay[0] = __ffma2_rn(make_float2(pa.x, pa.y), tyy, ay[0]);
+        ax[1] = __ffma2_rn(make_float2(pa.z, pa.w), txx, ax[1]); ay[1] = __ffma2_rn(make_float2(pa.z, pa.w), tyy, ay[1]);
+        ax[2] = __ffma2_rn(make_float2(pb.x, pb.y), txx, ax[2]); ay[2] = __ffma2_rn(make_float2(pb.x, pb.y), tyy, ay[2]);
+        ax[3] = __ffma2_rn(make_float2(pb.z, pb.w), txx, ax[3]); ay[3] = __ffma2_rn(make_float2(pb.z, pb.w), tyy, ay[3]);
     }
 }
 
@@ -347,9 +348,9 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
     if (threadIdx.x == 0) mbar_init(bar, 1);
     __syncthreads();
     uint32_t phase = 0;
-    float2 acc[kBandW];
+    float2 ax[kBandW / 2], ay[kBandW / 2];
 #pragma unroll
-    for (int c = 0; c < kBandW; ++c) acc[c] = make_float2(0.f, 0.f);
+    for (int c = 0; c < kBandW / 2; ++c) { ax[c] = make_float2(0.f, 0.f); ay[c] = make_float2(0.f, 0.f); }
     // stencil base rows that touch the item: r0-5 .. r0+nrows-1 (mod K0): one row segment, or two at the seam
     const int nseg = (it.r0 >= kJ - 1) ? 1 : 2;
 #pragma unroll 1
@@ -398,12 +399,18 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
                 if (x1 > x0) {
                     const int n = x1 - x0;
                     const int i0 = x0 - c0 + ((n * part) >> lsplit), i1 = x0 - c0 + ((n * (part + 1)) >> lsplit);
-                    if (q == 2) il_accumulate_smem<16>(acc, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
-                    else        il_accumulate_smem<8>(acc, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
+                    if (q == 2) il_accumulate_smem<16>(ax, ay, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
+                    else        il_accumulate_smem<8>(ax, ay, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
                 }
             }
             __syncthreads();      // every warp is done with the staged chunk before the next round overwrites it
         }
+    }
+    float2 acc[kBandW];
+#pragma unroll
+    for (int c = 0; c < kBandW / 2; ++c) {
+        acc[2 * c] = make_float2(ax[c].x, ay[c].x);
+        acc[2 * c + 1] = make_float2(ax[c].y, ay[c].y);
     }
     if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row (staging area reused)
         float2* red = y_s;  // [8][kBandW][32]
