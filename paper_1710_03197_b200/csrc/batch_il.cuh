@@ -119,7 +119,7 @@ struct IlPlan {
 // Each lane prepares the weights of one sample (kb_weights) and stages them in shared memory; the warp then walks
 // the samples one by one with warp-uniform weights: 36 loads of 256 contiguous bytes and 72 + 12 FMAs per lane.
 constexpr int kInterpWarps = 8;
-constexpr int kInterpChunk = 128;    // consecutive sorted samples per CTA
+constexpr int kInterpChunk = 64;     // consecutive sorted samples per CTA
 // Output: y_il[group][sorted sample][32] (coalesced); y_from_il_kernel restores the caller's order when needed.
 __global__ void __launch_bounds__(256)
 interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y_il, KernelPoly P) {
