@@ -311,9 +311,12 @@ def run_ours(args):
         timed_kernels = {k: v for k, v in rows.items() if "alg_bytes" in v}
         dom = max(timed_kernels, key=lambda k: timed_kernels[k]["ms_per_launch"])
         traffic = None
-        try:
-            with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
-                traffic = json.load(f).get("cfg2_batch%d" % B, {}).get(dom)
+        try:    # DRAM bytes per launch of the dominant kernel, from the committed ncu --set full capture
+            import csv
+            with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
+                for row in csv.DictReader(f):
+                    if row["config"] == "cfg2_batch%d" % B and row["kernel"] == dom:
+                        traffic = int(row["dram_bytes_per_launch"])
         except Exception:
             pass
         step_bytes = sum(v["alg_bytes"] for v in timed_kernels.values())
