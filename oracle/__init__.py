@@ -16,6 +16,7 @@ Modules:
   nufft_oracle.py    kernel, scaling factors, stencil, V, V^H, forward, adjoint, selfadjoint, direct NDFT,
                      multi-coil
   solvers_oracle.py  gradient, shrink, CG, L1TV-OLS
+  next_oracle.py     density compensation (eqs. 6-7), Toeplitz A^H A
 
 Parity status of every function is listed in each module's header.
 """

@@ -1,0 +1,76 @@
+"""Float64 CPU oracle of the rows SURVEY.md 8(f) marks "next".   TEST INFRASTRUCTURE.
+
+    density_weights / adjoint_dcf   sampling density compensation, eqs. (6)-(7)
+    toeplitz_kernel / selfadjoint_toeplitz   "precomputing A^H A" (Toeplitz, ref. [6])   PAPER.md:86-98, Fig. 3 :114
+
+Built on oracle/nufft_oracle.py (forward, adjoint); numpy float64 / complex128; numpy.fft as a library step.
+
+Readings of the paper taken here (R21-R22):
+    R21  eq. (6) w_{i+1} = w_i / (A A^H w_i): the paper gives neither w_0, nor the iteration count, nor how a complex
+         A A^H w is divided into a real density function.  Taken: w_0 = 1, w real, w_{i+1} = w_i / |A A^H w_i|
+         (elementwise magnitude, as in ref. [7]'s iteration), a fixed iteration count given by the caller.
+    R22  the paper's own "Toeplitz" precomputes the sparse V^H V; SURVEY 8(f)-1 asks for the true
+         Toeplitz embedding of ref. [6]: A^H A x = crop(F^H(T^ . F(pad x))) on the 2N grid, T^ = F(T),
+         T[d] = sum_m w_m e^{i om_m . d}, d in [-N, N)^dim, obtained by ONE adjoint NUFFT of the weights onto a 2N image
+         (4N grid).  It equals the back-to-back operator up to the interpolation-kernel error (~1e-5), not to rounding.
+
+Parity pins (tests/test_oracle_next.py):
+    density_weights        Cartesian full sampling: fixed point w = 1 / prod(N) (closed form, A A^H = prod(N) I);
+                           every location duplicated: the weights halve; invariance to the scale of w_0 after one step
+    adjoint_dcf            = adjoint(y * w) by definition; Cartesian case inverts the DFT: A^H(w . A x) = x
+    toeplitz_kernel        T[d] against the brute-force sum over samples on tiny sizes (rel. <= 1e-4); Hermitian symmetry
+                           T[-d] = conj(T[d])
+    selfadjoint_toeplitz   against the dense matrix A_exact^H A_exact built from the plain non-uniform DFT definition
+                           (rel. <= 1e-4) and against adjoint(forward(x)) (same bound)
+No function here is "parity unpinned".
+"""
+import numpy as np
+
+from . import nufft_oracle as orc
+
+__all__ = ["density_weights", "adjoint_dcf", "toeplitz_kernel", "selfadjoint_toeplitz"]
+
+
+def density_weights(om, Nd, Kd, Jd, niter):
+    """Sampling density compensation function, eq. (6) PAPER.md:118 with reading R21:
+    w_0 = 1;  w_{i+1} = w_i / |A A^H w_i|.   Returns real float64 w[M]."""
+    M = np.asarray(om).shape[0]
+    w = np.ones(M, dtype=np.float64)
+    for _ in range(int(niter)):
+        t = orc.forward(orc.adjoint(w.astype(np.complex128), om, Nd, Kd, Jd), om, Nd, Kd, Jd)
+        w = w / np.abs(t)
+    return w
+
+
+def adjoint_dcf(y, w, om, Nd, Kd, Jd):
+    """x = A^H (y . w), eq. (7) PAPER.md:122."""
+    return orc.adjoint(np.asarray(y, dtype=np.complex128) * np.asarray(w), om, Nd, Kd, Jd)
+
+
+def toeplitz_kernel(om, Nd, Kd, Jd, w=None):
+    """T^ = FFT over the 2N grid of the point-spread function T[d] = sum_m w_m e^{i om_m . d}, d in [-N, N)^dim (R22).
+    T comes from one adjoint NUFFT of the weights onto an image of size 2N (grid 4N): its pixel n sits at position
+    n - N = d.  Returns (T^ complex128 of shape 2N, T of shape 2N with d = n - N)."""
+    Nd = tuple(int(n) for n in Nd)
+    N2 = tuple(2 * n for n in Nd)
+    K2 = tuple(4 * n for n in Nd)
+    M = np.asarray(om).shape[0]
+    wv = np.ones(M, dtype=np.complex128) if w is None else np.asarray(w, dtype=np.complex128)
+    T = orc.adjoint(wv, om, N2, K2, Jd)
+    # d = -N (pixel 0 on every axis) is never used by a linear convolution of two length-N supports; drop it
+    for a in range(len(Nd)):
+        sl = [slice(None)] * len(Nd)
+        sl[a] = 0
+        T[tuple(sl)] = 0.0
+    That = np.fft.fftn(np.fft.ifftshift(T))          # index d mod 2N
+    return That, T
+
+
+def selfadjoint_toeplitz(x, That, Nd):
+    """A^H A x by Toeplitz embedding (R22): zero-pad x to 2N, multiply the spectra, crop.
+    (T * x)[n] = sum_n' T[n - n'] x[n'] for n in [0, N): the circular convolution of size 2N is alias-free."""
+    Nd = tuple(int(n) for n in Nd)
+    z = np.zeros(That.shape, dtype=np.complex128)
+    z[tuple(slice(0, n) for n in Nd)] = x
+    r = np.fft.ifftn(np.fft.fftn(z) * That)
+    return r[tuple(slice(0, n) for n in Nd)]
