@@ -139,6 +139,25 @@ int nufft_solve_cg(nufft_plan_t p, int use_coils, const nufft_c64 *y, nufft_c64 
 int nufft_solve_l1tv_ols(nufft_plan_t p, int use_coils, const nufft_c64 *y, nufft_c64 *x,
                          double mu, double lam, int n_outer, int n_inner, int n_cg, void *stream);
 
+/* ---- rows SURVEY.md 8(f) marks "next", built on the same kernels -------------------------------------------------
+ * Density compensation, eqs.(6)-(7) PAPER.md:118-122 with reading R21 (w_0 = 1, w real, w <- w / |A A^H w|, exactly
+ * niter iterations).  w: device complex64 [M] (output; imaginary parts are 0).
+ *   nufft_adjoint_dcf: x[b] = A^H (y_b . w), y device [batch][M], w device [M], x device [batch][prod Nd]. */
+int nufft_density_weights(nufft_plan_t p, int niter, nufft_c64 *w, void *stream);
+int nufft_adjoint_dcf(nufft_plan_t p, int batch, const nufft_c64 *y, const nufft_c64 *w, nufft_c64 *x, void *stream);
+
+/* Toeplitz form of A^H A ("precomputing A^H A", ref.[6]; reading R22):
+ *   A^H A x = crop(F^H(T^ . F(pad x))) on the same K = 2N grid, T^ = F(T), T[d] = sum_m w_m e^{i om_m . d}.
+ * nufft_toeplitz_build computes T^ once per plan with ONE adjoint NUFFT of the weights w (device complex64 [M], or NULL
+ * = all ones) onto a 2N image through a temporary second plan (4N grid: needs 2*Kd[a] <= 1024, else NUFFT_EINVAL);
+ * synchronises the stream.  The result differs from the back-to-back nufft_selfadjoint by the interpolation-kernel
+ * error (~1e-5 relative), not by rounding; V and V^H no longer run.  nufft_toeplitz_enable(p, 1) makes nufft_solve_cg
+ * and nufft_solve_l1tv_ols apply A^H A this way (NUFFT_ESTATE before a build). */
+int nufft_toeplitz_build(nufft_plan_t p, const nufft_c64 *w, void *stream);
+int nufft_toeplitz_enable(nufft_plan_t p, int on);
+int nufft_selfadjoint_toeplitz(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
+int nufft_selfadjoint_toeplitz_coils(nufft_plan_t p, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
+
 /* Plan facts.  Any pointer may be NULL.  bytes_plan = device bytes of per-sample plan data; bytes_work = device
  * bytes of workspace (grids, sample buffers, solver vectors); n_tiles / n_work = V^H tiles and work items (after
  * hot-tile splitting); max_tile_samples = the largest tile's sample count. */

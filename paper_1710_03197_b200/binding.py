@@ -17,6 +17,8 @@ _I64P = _c.POINTER(_c.c_int64)
 EXPORTED_SYMBOLS = [
     "nufft_default_opts", "nufft_plan", "nufft_forward", "nufft_adjoint", "nufft_selfadjoint",
     "nufft_forward_host", "nufft_adjoint_host", "nufft_selfadjoint_host",
+    "nufft_density_weights", "nufft_adjoint_dcf", "nufft_toeplitz_build", "nufft_toeplitz_enable",
+    "nufft_selfadjoint_toeplitz", "nufft_selfadjoint_toeplitz_coils",
     "nufft_stage_scale_fft", "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale",
     "nufft_set_coils", "nufft_forward_coils", "nufft_adjoint_coils", "nufft_selfadjoint_coils",
     "nufft_solve_cg", "nufft_solve_l1tv_ols", "nufft_plan_info", "nufft_launch_count", "nufft_destroy",
@@ -60,6 +62,12 @@ def lib():
                  "nufft_selfadjoint_host", "nufft_stage_scale_fft",
                  "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale"):
         getattr(L, name).argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR]
+    L.nufft_density_weights.argtypes = [_PLAN, _c.c_int, _PTR, _PTR]
+    L.nufft_adjoint_dcf.argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR, _PTR]
+    L.nufft_toeplitz_build.argtypes = [_PLAN, _PTR, _PTR]
+    L.nufft_toeplitz_enable.argtypes = [_PLAN, _c.c_int]
+    L.nufft_selfadjoint_toeplitz.argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR]
+    L.nufft_selfadjoint_toeplitz_coils.argtypes = [_PLAN, _PTR, _PTR, _PTR]
     L.nufft_set_coils.argtypes = [_PLAN, _c.c_int, _PTR]
     for name in ("nufft_forward_coils", "nufft_adjoint_coils", "nufft_selfadjoint_coils"):
         getattr(L, name).argtypes = [_PLAN, _PTR, _PTR, _PTR]
@@ -260,6 +268,39 @@ class NufftPlan:
         out = self._new(*self.Nd) if out is None else out
         _check(lib().nufft_selfadjoint_coils(self._h, _dev(x, "x", self.nimg), _dev(out, "out", self.nimg), _stream()),
                "nufft_selfadjoint_coils")
+        return out
+
+    # -- "next" rows: density compensation, Toeplitz A^H A -------------------------------------------------------
+    def density_weights(self, niter, w=None):
+        w = self._new(self.M) if w is None else w
+        _check(lib().nufft_density_weights(self._h, int(niter), _dev(w, "w", self.M), _stream()), "nufft_density_weights")
+        return w
+
+    def adjoint_dcf(self, y, w, x=None):
+        b = self._batch_of(y, self.M)
+        x = self._new(b, *self.Nd) if x is None else x
+        _check(lib().nufft_adjoint_dcf(self._h, b, _dev(y, "y"), _dev(w, "w", self.M), _dev(x, "x", b * self.nimg),
+                                       _stream()), "nufft_adjoint_dcf")
+        return x
+
+    def toeplitz_build(self, w=None):
+        _check(lib().nufft_toeplitz_build(self._h, None if w is None else _dev(w, "w", self.M), _stream()),
+               "nufft_toeplitz_build")
+
+    def toeplitz_enable(self, on=True):
+        _check(lib().nufft_toeplitz_enable(self._h, int(bool(on))), "nufft_toeplitz_enable")
+
+    def selfadjoint_toeplitz(self, x, out=None):
+        b = self._batch_of(x, self.nimg)
+        out = self._new(b, *self.Nd) if out is None else out
+        _check(lib().nufft_selfadjoint_toeplitz(self._h, b, _dev(x, "x"), _dev(out, "out", b * self.nimg), _stream()),
+               "nufft_selfadjoint_toeplitz")
+        return out
+
+    def selfadjoint_toeplitz_coils(self, x, out=None):
+        out = self._new(*self.Nd) if out is None else out
+        _check(lib().nufft_selfadjoint_toeplitz_coils(self._h, _dev(x, "x", self.nimg), _dev(out, "out", self.nimg),
+                                                      _stream()), "nufft_selfadjoint_toeplitz_coils")
         return out
 
     # -- solvers ----------------------------------------------------------------------------------------------

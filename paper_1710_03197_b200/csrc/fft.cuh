@@ -320,13 +320,17 @@ struct ColPassParams {
     int n_outer, k_outer;      // number of outer slabs visited and K of that axis (k_outer = 0: identity map)
     int inner;                 // contiguous extent (multiple of T)
     int ngroups;               // batch * n_outer * inner / T
+    const float2* mult;        // ADJ only, optional: every loaded element is first multiplied by mult[(offset within one
+    int mult_shift;            //   batch item) >> mult_shift]  (Toeplitz spectrum; shift 5 on the interleaved grid)
 };
 
-template <int K, bool ADJ>
+// FULL: no pruning (every input is loaded, every output stored): used once per plan to transform the Toeplitz
+// point-spread function, which fills the whole grid.
+template <int K, bool ADJ, bool FULL = false>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS, Rad<K>::MBS)
 fft_cols_kernel(ColPassParams p) {
     using G = FftGeom<K>;
-    constexpr int T = Rad<K>::TS, TPL = G::TPL;
+    constexpr int T = Rad<K>::TS;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x % T, q0 = threadIdx.x / T;
     const int g = blockIdx.x;
@@ -334,18 +338,46 @@ fft_cols_kernel(ColPassParams p) {
     const int i0 = (g % per_slab) * T;
     const int o = (g / per_slab) % p.n_outer, b = g / (per_slab * p.n_outer);
     const int om = p.k_outer ? ((o - p.n_outer / 2) & (p.k_outer - 1)) : o;
-    float2* __restrict__ base = p.grid + (int64_t)b * p.batch_stride + (int64_t)om * p.outer_stride + i0 + t;
+    const int64_t off = (int64_t)om * p.outer_stride + i0 + t;
+    float2* __restrict__ base = p.grid + (int64_t)b * p.batch_stride + off;
     const int64_t ls = p.line_stride;
     LayStrided<K, T> lay{smem + t};
-    if (!ADJ) {
+    if (FULL) {
+        auto ld = [&](int i) -> float2 { return base[i * ls]; };
+        auto st = [&](int i, float2 v) { base[i * ls] = v; };
+        fft_line<K, false, false>(q0, true, lay, p.tw, ld, st);
+    } else if (!ADJ) {
         auto ld = [&](int i) -> float2 { return base[i * ls]; };
         auto st = [&](int i, float2 v) { base[i * ls] = v; };
         fft_line<K, true, false>(q0, true, lay, p.tw, ld, st);
     } else {
-        auto ld = [&](int i) -> float2 { return cconj(base[i * ls]); };
+        const float2* __restrict__ mult = p.mult;
+        const int ms = p.mult_shift;
+        auto ld = [&](int i) -> float2 {
+            float2 v = base[i * ls];
+            if (mult) v = cmul(v, __ldg(&mult[(off + i * ls) >> ms]));
+            return cconj(v);
+        };
         auto st = [&](int i, float2 v) { base[i * ls] = cconj(v); };
         fft_line<K, false, true>(q0, true, lay, p.tw, ld, st);
     }
+}
+
+// Unpruned in-place forward FFT along the last (contiguous) axis of a planar array: nlines lines of K elements.
+template <int K>
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::LC)
+fft_rows_full_kernel(float2* __restrict__ data, const float2* __restrict__ tw, int nlines) {
+    using G = FftGeom<K>;
+    constexpr int TPL = G::TPL, LC = Rad<K>::LC;
+    extern __shared__ float2 smem[];
+    const int lt = threadIdx.x / TPL, q0 = threadIdx.x % TPL;
+    const int line = blockIdx.x * LC + lt;
+    const bool active = line < nlines;
+    float2* __restrict__ row = data + (int64_t)(active ? line : 0) * K;
+    LayContig<K> lay{smem + lt * G::PITCH_C};
+    auto ld = [&](int i) -> float2 { return row[i]; };
+    auto st = [&](int i, float2 v) { row[i] = v; };
+    fft_line<K, false, false>(q0, active, lay, tw, ld, st);
 }
 
 }  // namespace nufft

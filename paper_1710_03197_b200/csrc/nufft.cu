@@ -83,6 +83,15 @@ struct nufft_plan_s {
     IlItem* d_il_items = nullptr;
     int n_il_items = 0;
     float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
+    // "next" rows: density compensation and Toeplitz A^H A
+    std::vector<double> om_host;    // copy of the trajectory (the Toeplitz build plans a second, 2N transform)
+    float* d_ones = nullptr;        // unit scaling vector (max N), used instead of d_scale by the Toeplitz passes
+    float2* d_that = nullptr;       // Toeplitz spectrum T^ on the K grid, planar [K0][K1]([K2])
+    bool toep_on = false;           // solvers and selfadjoint calls use the Toeplitz operator
+    bool unit_scale = false;        // transient: FFT row passes use d_ones
+    const float2* cur_mult = nullptr;   // transient: the first adjoint column pass multiplies by this spectrum
+    float2* d_dcf_img = nullptr;
+    float2* d_dcf_t = nullptr;
     // host-buffer pipeline (nufft_*_host): copy streams, events, double-buffered device staging, lazy
     bool hp_ready = false;
     int hp_chunk = 1;
@@ -142,6 +151,10 @@ template <int K> static cudaError_t configure_fft() {
     e = cudaFuncSetAttribute(fft_il_rows_fwd_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_il_rows_adj_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_cols_kernel<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_rows_full_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
     return e;
 }
 
@@ -216,13 +229,13 @@ static RowPassParams row_params(nufft_plan_t p, int batch, const float2* img_in,
     RowPassParams r{};
     r.img_in = img_in; r.img_out = img_out; r.grid = grid; r.coil = coil;
     const int d = p->d;
-    r.s_line = p->d_scale[d - 1];
+    r.s_line = p->unit_scale ? p->d_ones : p->d_scale[d - 1];
     r.tw = p->d_tw[d - 1];
     if (d == 2) {
-        r.s_outer0 = p->d_scale[0]; r.s_outer1 = nullptr;
+        r.s_outer0 = p->unit_scale ? p->d_ones : p->d_scale[0]; r.s_outer1 = nullptr;
         r.n_outer0 = p->N[0]; r.n_outer1 = 1; r.k_outer0 = p->K[0]; r.k_outer1 = 1;
     } else {
-        r.s_outer0 = p->d_scale[0]; r.s_outer1 = p->d_scale[1];
+        r.s_outer0 = p->unit_scale ? p->d_ones : p->d_scale[0]; r.s_outer1 = p->unit_scale ? p->d_ones : p->d_scale[1];
         r.n_outer0 = p->N[0]; r.n_outer1 = p->N[1]; r.k_outer0 = p->K[0]; r.k_outer1 = p->K[1];
     }
     r.nlines = batch * r.n_outer0 * r.n_outer1;
@@ -272,6 +285,7 @@ static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, con
         c.batch_stride = p->cells; c.outer_stride = 0; c.line_stride = p->K[1];
         c.n_outer = 1; c.k_outer = 0; c.inner = p->K[1];
         c.ngroups = batch * (c.inner / tile_T(p->K[0]));
+        c.mult = p->cur_mult; c.mult_shift = 0;
         { ProfScope ps(p, "fft_cols_adj", st); NU_TRY(dispatch_cols(p->K[0], true, c, st)); }
         p->launches++;
     } else {
@@ -280,6 +294,7 @@ static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, con
         c0.batch_stride = p->cells; c0.outer_stride = 0; c0.line_stride = (int64_t)p->K[1] * p->K[2];
         c0.n_outer = 1; c0.k_outer = 0; c0.inner = p->K[1] * p->K[2];
         c0.ngroups = batch * (c0.inner / tile_T(p->K[0]));
+        c0.mult = p->cur_mult; c0.mult_shift = 0;
         { ProfScope ps(p, "fft_cols_adj_axis0", st); NU_TRY(dispatch_cols(p->K[0], true, c0, st)); }
         ColPassParams c{};
         c.grid = grid; c.tw = p->d_tw[1];
@@ -399,7 +414,8 @@ static IlRowParams il_row_params(nufft_plan_t p, int batch, const float2* img_in
                                  const float2* coil, bool same_image) {
     IlRowParams r{};
     r.img_in = img_in; r.img_out = img_out; r.grid = grid; r.coil = coil;
-    r.s_outer = p->d_scale[0]; r.s_line = p->d_scale[1]; r.tw = p->d_tw[1];
+    r.s_outer = p->unit_scale ? p->d_ones : p->d_scale[0]; r.s_line = p->unit_scale ? p->d_ones : p->d_scale[1];
+    r.tw = p->d_tw[1];
     r.n_outer = p->N[0]; r.k_outer = p->K[0]; r.batch = batch; r.same_image = same_image ? 1 : 0;
     return r;
 }
@@ -429,7 +445,12 @@ static int run_scale_fft_il(nufft_plan_t p, int batch, const float2* x, float2* 
 }
 // a5 + a6 on the interleaved grid
 static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
-    { ProfScope ps(p, "fft_cols_adj", st); NU_TRY(dispatch_cols(p->K[0], true, il_col_params(p, batch, grid), st)); }
+    {
+        ColPassParams c = il_col_params(p, batch, grid);
+        c.mult = p->cur_mult; c.mult_shift = 5;
+        ProfScope ps(p, "fft_cols_adj", st);
+        NU_TRY(dispatch_cols(p->K[0], true, c, st));
+    }
     IlRowParams r = il_row_params(p, batch, nullptr, x, grid, coil, false);
     { ProfScope ps(p, "fft_rows_adj", st); NU_TRY(dispatch_il_rows(p->K[1], true, r, st)); }
     p->launches += 2;
@@ -628,6 +649,11 @@ static int plan_build(nufft_plan_t p, const double* om) {
         NU_TRY(dev_upload(&p->d_scale[a], host::scaling_vector(p->N[a], p->K[a], J), &p->bytes_plan));
         NU_TRY(dev_upload(&p->d_tw[a], host::twiddle_table(p->K[a]), &p->bytes_plan));
     }
+    {
+        int nmax = 1;
+        for (int a = 0; a < d; ++a) nmax = std::max(nmax, p->N[a]);
+        NU_TRY(dev_upload(&p->d_ones, std::vector<float>((size_t)nmax, 1.0f), &p->bytes_plan));
+    }
     // tiles
     const int def2[3] = {16, 32, 1}, def3[3] = {8, 8, 16};
     for (int a = 0; a < 3; ++a) {
@@ -772,6 +798,7 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     }
     int rc = NUFFT_OK;
     try {
+        if (M > 0) p->om_host.assign(om, om + (size_t)M * d);
         rc = plan_build(p, om);
     } catch (const std::bad_alloc&) {
         rc = NUFFT_ENOMEM;
@@ -790,6 +817,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_grid); cudaFree(p->d_ywork); cudaFree(p->d_imgwork); cudaFree(p->d_solver);
     cudaFree(p->d_scal); cudaFree(p->d_hist);
     cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
+    cudaFree(p->d_ones); cudaFree(p->d_that); cudaFree(p->d_dcf_img); cudaFree(p->d_dcf_t);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     if (p->hp_h2d) cudaStreamDestroy(p->hp_h2d);
@@ -1058,6 +1086,155 @@ extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nu
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// "next" rows of SURVEY 8(f): density compensation (eqs. 6-7) and Toeplitz A^H A
+// ------------------------------------------------------------------------------------------------------------
+static int ew_blocks(int64_t n);
+
+extern "C" int nufft_density_weights(nufft_plan_t p, int niter, nufft_c64* w, void* stream) {
+    if (!p || niter < 0 || (!w && p->M > 0)) return NUFFT_EINVAL;
+    if (p->M == 0) return NUFFT_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!p->d_dcf_img) NU_TRY(dev_alloc((void**)&p->d_dcf_img, (size_t)p->nimg * sizeof(float2), &p->bytes_work));
+    if (!p->d_dcf_t) NU_TRY(dev_alloc((void**)&p->d_dcf_t, (size_t)p->M * sizeof(float2), &p->bytes_work));
+    const int nb = ew_blocks(p->M);
+    dcf_init_kernel<<<nb, 256, 0, st>>>((float2*)w, p->M);
+    p->launches++;
+    for (int i = 0; i < niter; ++i) {          // w <- w / |A A^H w|   (eq. 6, R21)
+        NU_TRY(nufft_adjoint(p, 1, w, (nufft_c64*)p->d_dcf_img, st));
+        NU_TRY(nufft_forward(p, 1, (const nufft_c64*)p->d_dcf_img, (nufft_c64*)p->d_dcf_t, st));
+        dcf_update_kernel<<<nb, 256, 0, st>>>((float2*)w, p->d_dcf_t, p->M);
+        p->launches++;
+    }
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_adjoint_dcf(nufft_plan_t p, int batch, const nufft_c64* y, const nufft_c64* w, nufft_c64* x,
+                                 void* stream) {
+    if (bad_batch(p, batch) || !x || ((!y || !w) && p->M > 0)) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p->M > 0) {       // x = A^H (y . w)   (eq. 7); d_ywork is free during an adjoint
+        weight_mul_kernel<<<ew_blocks(p->M * batch), 256, 0, st>>>(p->d_ywork, (const float2*)y, (const float2*)w, p->M, batch);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+    }
+    return nufft_adjoint(p, batch, (const nufft_c64*)p->d_ywork, x, st);
+}
+
+template <int K> static void launch_rows_full(float2* data, const float2* tw, int nlines, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::LC;
+    fft_rows_full_kernel<K><<<(nlines + Rad<K>::LC - 1) / Rad<K>::LC, threads, smem_rows<K>(), st>>>(data, tw, nlines);
+}
+template <int K> static void launch_cols_full(const ColPassParams& c, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
+    fft_cols_kernel<K, false, true><<<c.ngroups, threads, smem_cols<K>(), st>>>(c);
+}
+#define NUFFT_K_SWITCH(K, CALL)                                                                                \
+    switch (K) {                                                                                               \
+        case 32: CALL(32); break; case 64: CALL(64); break; case 128: CALL(128); break;                        \
+        case 256: CALL(256); break; case 512: CALL(512); break; case 1024: CALL(1024); break;                  \
+        default: return NUFFT_EINVAL;                                                                          \
+    }
+
+// in-place unpruned forward FFT of a planar K^d array (used once per plan for the Toeplitz spectrum)
+static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st) {
+    const int d = p->d;
+    const int64_t cells = p->cells;
+    {
+        const int Kl = p->K[d - 1];
+        const int nlines = (int)(cells / Kl);
+#define CALL_ROWS(KK) launch_rows_full<KK>(data, p->d_tw[d - 1], nlines, st)
+        NUFFT_K_SWITCH(Kl, CALL_ROWS)
+#undef CALL_ROWS
+    }
+    for (int a = d - 2; a >= 0; --a) {
+        ColPassParams c{};
+        c.grid = data; c.tw = p->d_tw[a];
+        c.batch_stride = cells;
+        int64_t inner = 1;
+        for (int b = a + 1; b < d; ++b) inner *= p->K[b];
+        c.line_stride = inner; c.inner = (int)inner;
+        c.n_outer = (a == 0) ? 1 : p->K[0]; c.k_outer = 0;
+        c.outer_stride = (a == 0) ? 0 : (int64_t)p->K[1] * p->K[2];
+        c.ngroups = c.n_outer * (c.inner / tile_T(p->K[a]));
+#define CALL_COLS(KK) launch_cols_full<KK>(c, st)
+        NUFFT_K_SWITCH(p->K[a], CALL_COLS)
+#undef CALL_COLS
+    }
+    CU_TRY(cudaGetLastError());
+    p->launches += d;
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_toeplitz_build(nufft_plan_t p, const nufft_c64* w, void* stream) {
+    if (!p) return NUFFT_EINVAL;
+    for (int a = 0; a < p->d; ++a)
+        if (2 * p->K[a] > 1024) return NUFFT_EINVAL;         // the point-spread function needs a 4N grid
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!p->d_that) NU_TRY(dev_alloc((void**)&p->d_that, (size_t)p->cells * sizeof(float2), &p->bytes_plan));
+    // T[d] = sum_m w_m e^{i om_m . d}: one adjoint NUFFT of the weights onto the 2N image (R22)
+    int64_t N2[3], K2[3];
+    int J[3] = {kJ, kJ, kJ};
+    for (int a = 0; a < p->d; ++a) { N2[a] = p->K[a]; K2[a] = 2 * p->K[a]; }
+    nufft_opts o2;
+    nufft_default_opts(&o2);
+    o2.batch_layout = 1;
+    nufft_plan_t p2 = nullptr;
+    NU_TRY(nufft_plan(p->d, N2, K2, J, p->M, p->om_host.data(), 1, &o2, &p2));
+    int rc = NUFFT_OK;
+    float2* ones = nullptr;
+    if (!w && p->M > 0) {
+        rc = dev_alloc((void**)&ones, (size_t)p->M * sizeof(float2), nullptr);
+        if (rc == NUFFT_OK) dcf_init_kernel<<<ew_blocks(p->M), 256, 0, st>>>(ones, p->M);
+    }
+    if (rc == NUFFT_OK) rc = nufft_adjoint(p2, 1, w ? w : (const nufft_c64*)ones, (nufft_c64*)p->d_that, st);
+    if (rc == NUFFT_OK) {
+        const int nb = ew_blocks(p->cells);
+        psf_zero_planes_kernel<<<nb, 256, 0, st>>>(p->d_that, p->K[0], p->K[1], p->d == 3 ? p->K[2] : 1);
+        rc = fft_full_inplace(p, p->d_that, st);
+        if (rc == NUFFT_OK) psf_sign_kernel<<<nb, 256, 0, st>>>(p->d_that, p->K[0], p->K[1], p->d == 3 ? p->K[2] : 1,
+                                                                   (float)(1.0 / (double)p->cells));
+        p->launches += 2;
+    }
+    cudaError_t e = cudaStreamSynchronize(st);      // the temporary plan and `ones` are released below
+    nufft_destroy(p2);
+    cudaFree(ones);
+    if (rc == NUFFT_OK && e != cudaSuccess) { g_last_cuda_error = (int)e; rc = NUFFT_ECUDA; }
+    return rc;
+}
+
+extern "C" int nufft_toeplitz_enable(nufft_plan_t p, int on) {
+    if (!p) return NUFFT_EINVAL;
+    if (on && !p->d_that) return NUFFT_ESTATE;
+    p->toep_on = on != 0;
+    return NUFFT_OK;
+}
+
+// x_out = crop(F^H(T^ . F(pad x_in))); coils: sum_i conj(c_i) crop(F^H(T^ . F(pad c_i x_in)))
+static int run_toeplitz(nufft_plan_t p, int batch, const float2* x_in, float2* x_out, const float2* coil, bool same_image,
+                        cudaStream_t st) {
+    p->unit_scale = true;
+    p->cur_mult = p->d_that;
+    int rc;
+    if (use_il(p, batch)) {
+        rc = run_scale_fft_il(p, batch, x_in, p->d_grid, coil, same_image, st);
+        if (rc == NUFFT_OK) rc = run_fft_scale_il(p, batch, p->d_grid, x_out, coil, st);
+    } else {
+        rc = run_scale_fft(p, batch, x_in, p->d_grid, coil, same_image, st);
+        if (rc == NUFFT_OK) rc = run_fft_scale(p, batch, p->d_grid, x_out, coil, st);
+    }
+    p->unit_scale = false;
+    p->cur_mult = nullptr;
+    return rc;
+}
+
+extern "C" int nufft_selfadjoint_toeplitz(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
+    if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
+    if (!p->d_that) return NUFFT_ESTATE;
+    return run_toeplitz(p, batch, (const float2*)x_in, (float2*)x_out, nullptr, false, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // solvers
 // ------------------------------------------------------------------------------------------------------------
 static int ew_blocks(int64_t n) { return (int)std::max<int64_t>(1, std::min<int64_t>((n + 255) / 256, 148 * 8)); }
@@ -1080,7 +1257,20 @@ static int ensure_solver(nufft_plan_t p, int64_t nvec, int hist) {
     return NUFFT_OK;
 }
 
+static int coil_reduce(nufft_plan_t p, float2* x, cudaStream_t st);
+extern "C" int nufft_selfadjoint_toeplitz_coils(nufft_plan_t p, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
+    if (!p || !x_in || !x_out) return NUFFT_EINVAL;
+    if (p->ncoil < 1 || !p->d_that) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_toeplitz(p, p->ncoil, (const float2*)x_in, p->d_imgwork, p->d_coils, true, st));
+    return coil_reduce(p, (float2*)x_out, st);
+}
+
 static int apply_aha(nufft_plan_t p, bool coils, const float2* in, float2* out, cudaStream_t st) {
+    if (p->toep_on) {
+        if (coils) return nufft_selfadjoint_toeplitz_coils(p, (const nufft_c64*)in, (nufft_c64*)out, st);
+        return nufft_selfadjoint_toeplitz(p, 1, (const nufft_c64*)in, (nufft_c64*)out, st);
+    }
     if (coils) return nufft_selfadjoint_coils(p, (const nufft_c64*)in, (nufft_c64*)out, st);
     return nufft_selfadjoint(p, 1, (const nufft_c64*)in, (nufft_c64*)out, st);
 }

@@ -209,4 +209,46 @@ tv_outer_kernel(float2* __restrict__ ahy_k, const float2* __restrict__ ahy_s, co
         ahy_k[i] = cadd(ahy_k[i], csub(ahy_s[i], ahax[i]));
 }
 
+// ---- density compensation, eqs. (6)-(7) PAPER.md:118-122 (reading R21) ----
+// w = 1 (complex64 with zero imaginary part)
+__global__ void __launch_bounds__(256) dcf_init_kernel(float2* __restrict__ w, int64_t M) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < M; i += (int64_t)gridDim.x * blockDim.x)
+        w[i] = make_float2(1.f, 0.f);
+}
+// w <- w / |t|,  t = A A^H w
+__global__ void __launch_bounds__(256) dcf_update_kernel(float2* __restrict__ w, const float2* __restrict__ t, int64_t M) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < M; i += (int64_t)gridDim.x * blockDim.x) {
+        const float2 tv = t[i];
+        w[i] = make_float2(w[i].x / sqrtf(tv.x * tv.x + tv.y * tv.y), 0.f);
+    }
+}
+// out[b][m] = y[b][m] * w[m].re
+__global__ void __launch_bounds__(256)
+weight_mul_kernel(float2* __restrict__ out, const float2* __restrict__ y, const float2* __restrict__ w, int64_t M, int batch) {
+    const int64_t n = M * batch;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        out[i] = cscale(y[i], __ldg(&w[i % M].x));
+}
+
+// ---- Toeplitz point-spread function (reading R22) ----
+// T2 is the adjoint NUFFT of the weights onto the 2N image (pixel n <-> displacement d = n - N).  Zero the d = -N
+// hyperplanes (pixel 0 of every axis), which a linear convolution of two length-N supports never uses.
+__global__ void __launch_bounds__(256) psf_zero_planes_kernel(float2* __restrict__ T, int K0, int K1, int K2) {
+    const int64_t n = (int64_t)K0 * K1 * K2;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c2 = (int)(i % K2), c1 = (int)((i / K2) % K1), c0 = (int)(i / ((int64_t)K1 * K2));
+        if (c0 == 0 || c1 == 0 || (K2 > 1 && c2 == 0)) T[i] = make_float2(0.f, 0.f);
+    }
+}
+// T^[k] = sum_d T[d] e^{-2 pi i k d / K} = (-1)^{sum k_a} FFT(T2)[k]   (d = n - K/2 per axis), times `scale` = 1/prod(K):
+// the path's F^H is the unnormalised conjugate transpose (R5), so F^H(T^ . F z) carries a factor prod(K).
+__global__ void __launch_bounds__(256) psf_sign_kernel(float2* __restrict__ T, int K0, int K1, int K2, float scale) {
+    const int64_t n = (int64_t)K0 * K1 * K2;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c2 = (int)(i % K2), c1 = (int)((i / K2) % K1), c0 = (int)(i / ((int64_t)K1 * K2));
+        const float sgn = ((c0 + c1 + c2) & 1) ? -scale : scale;
+        T[i] = make_float2(sgn * T[i].x, sgn * T[i].y);
+    }
+}
+
 }  // namespace nufft
