@@ -450,6 +450,20 @@ def extra_legs(nb, torch, peak, args):
     fwc_ms = time_calls(lambda: p.forward_coils(xt, y5), 10, flush)
     adc_ms = time_calls(lambda: p.adjoint_coils(y5, xo5), 10, flush)
     tv_ms = time_calls(lambda: p.solve_l1tv_ols(y5, 1.0, 0.02, 4, 5, 3, use_coils=True, x=xs), 3, flush)
+    # next row 8(f)-1: Toeplitz A^H A (no V / V^H per application) on the same 32-coil problem
+    p.toeplitz_build()
+    toep_ms = time_calls(lambda: p.selfadjoint_toeplitz_coils(xt, xo5), 10, flush)
+    p.toeplitz_enable(True)
+    xs = p.solve_l1tv_ols(y5, 1.0, 0.02, 1, 1, 1, use_coils=True, x=xs)
+    tv_toep_ms = time_calls(lambda: p.solve_l1tv_ols(y5, 1.0, 0.02, 4, 5, 3, use_coils=True, x=xs), 3, flush)
+    p.toeplitz_enable(False)
+    # next row 8(f)-3: density compensation, 4 iterations of eq. (6) + the weighted adjoint of eq. (7)
+    wdc = p.density_weights(1)
+    dcf_ms = time_calls(lambda: p.density_weights(4, wdc), 5, flush)
+    out["next_rows"] = {
+        "toeplitz_selfadjoint_coils_ms": toep_ms, "l1tv_ols_20it_toeplitz_ms": tv_toep_ms,
+        "density_weights_4it_ms": dcf_ms,
+        "note": "cfg5 problem; Toeplitz: crop(F^H(T^ . F(pad c_i x))) summed over 32 coils, T^ built once per plan"}
     out["cfg5_2d_multicoil_l1tv"] = {
         "workload": "Nd=256^2 Kd=512^2 M=65536 radial 128x512, 32 coils", "forward_coils_ms": fwc_ms,
         "adjoint_coils_ms": adc_ms, "selfadjoint_coils_ms": sac_ms, "l1tv_ols_20it_ms": tv_ms,
