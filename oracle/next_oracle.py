@@ -2,6 +2,7 @@
 
     density_weights / adjoint_dcf   sampling density compensation, eqs. (6)-(7)
     toeplitz_kernel / selfadjoint_toeplitz   "precomputing A^H A" (Toeplitz, ref. [6])   PAPER.md:86-98, Fig. 3 :114
+    l1tv_lad                        split-Bregman L1TV-LAD, eqs. (23)-(33)
 
 Built on oracle/nufft_oracle.py (forward, adjoint); numpy float64 / complex128; numpy.fft as a library step.
 
@@ -22,13 +23,15 @@ Parity pins (tests/test_oracle_next.py):
                            T[-d] = conj(T[d])
     selfadjoint_toeplitz   against the dense matrix A_exact^H A_exact built from the plain non-uniform DFT definition
                            (rel. <= 1e-4) and against adjoint(forward(x)) (same bound)
-No function here is "parity unpinned".
+    l1tv_lad               PARITY UNPINNED by the paper (eqs. (23)-(33), garbled; reading R23 in its docstring).  Sanity
+                           pins: first inner iteration = L1TV-OLS's, scale equivariance, consistent-data fixed point.
+No other function here is "parity unpinned".
 """
 import numpy as np
 
 from . import nufft_oracle as orc
 
-__all__ = ["density_weights", "adjoint_dcf", "toeplitz_kernel", "selfadjoint_toeplitz"]
+__all__ = ["density_weights", "adjoint_dcf", "toeplitz_kernel", "selfadjoint_toeplitz", "l1tv_lad"]
 
 
 def density_weights(om, Nd, Kd, Jd, niter):
@@ -74,3 +77,52 @@ def selfadjoint_toeplitz(x, That, Nd):
     z[tuple(slice(0, n) for n in Nd)] = x
     r = np.fft.ifftn(np.fft.fftn(z) * That)
     return r[tuple(slice(0, n) for n in Nd)]
+
+
+def l1tv_lad(AHA, AHy, mu, lam, n_outer, n_inner, n_cg):
+    """Split-Bregman L1TV-LAD, eqs. (23)-(33), with the readings of L1TV-OLS (R13-R18: two gradient
+    splits, complex soft threshold, periodic gradient, n_cg warm-started CG steps for eq. (26), scaling by
+    1/max|A^H y|) and, for the data-term split (R23): eq. (29) prints `b_y^k` where the pattern of eqs. (25), (32)
+    requires b_f^k; the `A^H y` of eqs. (29) and (32) is the (scaled) A^H y itself, not the Bregman-updated A^H y^k:
+        rhs  = mu (A^H y^k + d_f - b_f) + lam sum_a grad_a^T (d_a - b_a)                      (25)
+        x    = K^{-1} rhs,   K = mu A^H A + lam sum_a grad_a^T grad_a                          (24), (26)
+        d_a  = shrink(grad_a x + b_a, 1/lam);   b_a += grad_a x - d_a                         (27)-(28), (30)-(31)
+        r    = A^H A x - A^H y;   d_f = shrink(r + b_f, 1/mu);   b_f += r - d_f               (29), (32)
+        outer: A^H y^{k+1} = A^H y^k + A^H y - A^H A x                                        (33)
+    PARITY UNPINNED by the paper (iterate values are defined only by this code).  Sanity pins: the first inner iteration
+    equals L1TV-OLS's (d_f = b_f = 0); scale equivariance; d_f = b_f = 0 forever when A^H A x = A^H y already holds."""
+    from .solvers_oracle import cg_steps, grad, grad_T, shrink
+    AHy = np.asarray(AHy, dtype=np.complex128)
+    assert AHy.ndim == 2
+    c = 1.0 / np.max(np.abs(AHy))
+    AHy_s = AHy * c
+    AHy_k = AHy_s.copy()
+    x = np.zeros_like(AHy_s)
+    d = [np.zeros_like(AHy_s) for _ in range(2)]
+    b = [np.zeros_like(AHy_s) for _ in range(2)]
+    d_f = np.zeros_like(AHy_s)
+    b_f = np.zeros_like(AHy_s)
+
+    def K(z):                                         # eq. (24)
+        out = mu * AHA(z)
+        for a in range(2):
+            out = out + lam * grad_T(grad(z, a), a)
+        return out
+
+    thr = 1.0 / lam if lam > 0.0 else np.inf
+    thr_f = 1.0 / mu if mu > 0.0 else np.inf
+    for _ in range(int(n_outer)):
+        for _ in range(int(n_inner)):
+            rhs = mu * (AHy_k + d_f - b_f)            # eq. (25)
+            for a in range(2):
+                rhs = rhs + lam * grad_T(d[a] - b[a], a)
+            x, _ = cg_steps(K, rhs, x, n_cg)          # eq. (26)
+            for a in range(2):
+                g = grad(x, a)
+                d[a] = shrink(g + b[a], thr)          # eqs. (27)-(28)
+                b[a] = b[a] + (g - d[a])              # eqs. (30)-(31)
+            r = AHA(x) - AHy_s
+            d_f = shrink(r + b_f, thr_f)              # eq. (29)
+            b_f = b_f + (r - d_f)                     # eq. (32)
+        AHy_k = AHy_k + AHy_s - AHA(x)                # eq. (33)
+    return x / c

@@ -108,3 +108,36 @@ def test_selfadjoint_toeplitz_3d_tiny():
     A = dense_ndft(om, Nd)
     exact = (A.conj().T @ (A @ x.ravel())).reshape(Nd)
     assert rel(nxt.selfadjoint_toeplitz(x, That, Nd), exact) < 1e-4
+
+
+# ---- L1TV-LAD (parity unpinned by the paper: sanity pins only) ----
+def _lad_problem(seed=11, N=12, M=500):
+    from oracle import solvers_oracle as sol  # noqa: F401
+    rng = np.random.default_rng(seed)
+    Nd, Kd, Jd = (N, N), (2 * N, 2 * N), (6, 6)
+    om = rng.uniform(-np.pi, np.pi, (M, 2))
+    xt = np.zeros(Nd, dtype=np.complex128)
+    xt[3:8, 4:9] = 1.0 + 0.5j
+    y = orc.forward(xt, om, Nd, Kd, Jd)
+    AHA = lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd)
+    return AHA, orc.adjoint(y, om, Nd, Kd, Jd), xt
+
+
+def test_lad_first_inner_iteration_equals_ols():
+    from oracle import solvers_oracle as sol
+    AHA, AHy, _ = _lad_problem()
+    a = nxt.l1tv_lad(AHA, AHy, 1.0, 0.05, 1, 1, 4)
+    b = sol.l1tv_ols(AHA, AHy, 1.0, 0.05, 1, 1, 4)
+    assert np.array_equal(a, b)          # d_f = b_f = 0 before the first data-term shrink
+    a2 = nxt.l1tv_lad(AHA, AHy, 1.0, 0.05, 1, 3, 4)
+    b2 = sol.l1tv_ols(AHA, AHy, 1.0, 0.05, 1, 3, 4)
+    assert rel(a2, b2) > 1e-6            # and the data-term split does act afterwards
+
+
+def test_lad_scale_equivariance_and_progress():
+    AHA, AHy, xt = _lad_problem()
+    x1 = nxt.l1tv_lad(AHA, AHy, 1.0, 0.05, 2, 3, 4)
+    x2 = nxt.l1tv_lad(AHA, 7.5 * AHy, 1.0, 0.05, 2, 3, 4)
+    assert rel(x2, 7.5 * x1) < 1e-12
+    x0 = nxt.l1tv_lad(AHA, AHy, 1.0, 0.05, 1, 1, 1)
+    assert rel(x1, xt) < rel(x0, xt)     # more iterations move towards the piecewise-constant truth
