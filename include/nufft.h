@@ -158,6 +158,14 @@ int nufft_toeplitz_enable(nufft_plan_t p, int on);
 int nufft_selfadjoint_toeplitz(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
 int nufft_selfadjoint_toeplitz_coils(nufft_plan_t p, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
 
+/* Split-Bregman L1TV-LAD, eqs.(23)-(33) PAPER.md:204-249: L1TV-OLS plus a split of the data term (reading R23: the
+ * `b_y^k` printed in eq.(29) is b_f^k; the A^H y of eqs.(29),(32) is the scaled A^H y, not the Bregman-updated one):
+ *   rhs = mu (A^H y^k + d_f - b_f) + lam sum_a grad_a^T(d_a - b_a) (25);  x <- n_cg warm-started CG steps on K x = rhs (24),(26);
+ *   d_a, b_a as in L1TV-OLS (27)-(28),(30)-(31);  r = A^H A x - A^H y;  d_f = shrink(r + b_f, 1/mu) (29);  b_f += r - d_f (32);
+ *   outer: A^H y^{k+1} = A^H y^k + A^H y - A^H A x (33).  Arguments and synchronisation as nufft_solve_l1tv_ols. */
+int nufft_solve_l1tv_lad(nufft_plan_t p, int use_coils, const nufft_c64 *y, nufft_c64 *x,
+                         double mu, double lam, int n_outer, int n_inner, int n_cg, void *stream);
+
 /* Plan facts.  Any pointer may be NULL.  bytes_plan = device bytes of per-sample plan data; bytes_work = device
  * bytes of workspace (grids, sample buffers, solver vectors); n_tiles / n_work = V^H tiles and work items (after
  * hot-tile splitting); max_tile_samples = the largest tile's sample count. */

@@ -1396,6 +1396,58 @@ extern "C" int nufft_solve_l1tv_ols(nufft_plan_t p, int use_coils, const nufft_c
     return NUFFT_OK;
 }
 
+extern "C" int nufft_solve_l1tv_lad(nufft_plan_t p, int use_coils, const nufft_c64* y, nufft_c64* x, double mu,
+                                    double lam, int n_outer, int n_inner, int n_cg, void* stream) {
+    if (!p || !y || !x || n_outer < 0 || n_inner < 0 || n_cg < 0 || p->d != 2 || lam < 0.0 || mu < 0.0) return NUFFT_EINVAL;
+    const bool coils = use_coils != 0;
+    if (coils && p->ncoil < 1) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n = p->nimg;
+    NU_TRY(ensure_solver(p, 15, 1));
+    float2* v = p->d_solver;
+    float2 *ahy_s = v, *ahy_k = v + n, *rhs = v + 2 * n, *r = v + 3 * n, *pv = v + 4 * n, *Ap = v + 5 * n;
+    float2 *d0 = v + 6 * n, *b0 = v + 7 * n, *d1 = v + 8 * n, *b1 = v + 9 * n, *df = v + 10 * n, *bf = v + 11 * n;
+    float2 *xs = v + 12 * n, *tmp = v + 13 * n, *prep = v + 14 * n;
+    const int nb = ew_blocks(n);
+    NU_TRY(adjoint_any(p, coils, (const float2*)y, tmp, st));
+    scalars_clear_kernel<<<1, 1, 0, st>>>(p->d_scal);
+    maxabs_kernel<<<nb, 256, 0, st>>>(tmp, n, p->d_scal);
+    p->launches += 2;
+    double mx = 0.0;
+    CU_TRY(cudaMemcpyAsync(&mx, &p->d_scal->maxabs, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    if (!(mx > 0.0)) {
+        CU_TRY(cudaMemsetAsync(x, 0, (size_t)n * sizeof(float2), st));
+        return NUFFT_OK;
+    }
+    scale_kernel<<<nb, 256, 0, st>>>(ahy_s, tmp, (float)(1.0 / mx), n);
+    CU_TRY(cudaMemcpyAsync(ahy_k, ahy_s, (size_t)n * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    CU_TRY(cudaMemsetAsync(d0, 0, (size_t)7 * n * sizeof(float2), st));     // d0, b0, d1, b1, df, bf, xs are contiguous
+    p->launches += 1;
+    const float fmu = (float)mu, flam = (float)lam;
+    const float thr = (lam > 0.0) ? (float)(1.0 / lam) : -1.0f;
+    const float thr_f = (mu > 0.0) ? (float)(1.0 / mu) : -1.0f;
+    NormalOp op{coils, true, fmu, flam};
+    for (int o = 0; o < n_outer; ++o) {
+        for (int i = 0; i < n_inner; ++i) {
+            lad_prep_kernel<<<nb, 256, 0, st>>>(prep, ahy_k, df, bf, n);                                   // eq. (25)
+            tv_rhs_kernel<<<nb, 256, 0, st>>>(rhs, prep, d0, b0, d1, b1, fmu, flam, p->N[0], p->N[1]);
+            NU_TRY(cg_run(p, op, rhs, xs, true, n_cg, r, pv, Ap, nullptr, st));                            // eq. (26)
+            tv_shrink_kernel<<<nb, 256, 0, st>>>(xs, d0, b0, d1, b1, thr, p->N[0], p->N[1]);               // (27)-(28), (30)-(31)
+            NU_TRY(apply_aha(p, coils, xs, tmp, st));
+            lad_data_kernel<<<nb, 256, 0, st>>>(tmp, ahy_s, df, bf, thr_f, n);                             // (29), (32)
+            p->launches += 4;
+        }
+        if (n_inner == 0) NU_TRY(apply_aha(p, coils, xs, tmp, st));
+        tv_outer_kernel<<<nb, 256, 0, st>>>(ahy_k, ahy_s, tmp, n);                                         // eq. (33)
+        p->launches++;
+    }
+    scale_kernel<<<nb, 256, 0, st>>>((float2*)x, xs, (float)mx, n);
+    p->launches++;
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 extern "C" const char* nufft_strerror(int code) {
     switch (code) {

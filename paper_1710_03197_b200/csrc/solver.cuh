@@ -209,6 +209,29 @@ tv_outer_kernel(float2* __restrict__ ahy_k, const float2* __restrict__ ahy_s, co
         ahy_k[i] = cadd(ahy_k[i], csub(ahy_s[i], ahax[i]));
 }
 
+// ---- L1TV-LAD data-term split, eqs. (25), (29), (32) PAPER.md:224-243 (reading R23) ----
+// out = ahy_k + d_f - b_f      (the bracket of eq. 25)
+__global__ void __launch_bounds__(256)
+lad_prep_kernel(float2* __restrict__ out, const float2* __restrict__ ahy_k, const float2* __restrict__ df,
+                const float2* __restrict__ bf, int64_t n) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        out[i] = cadd(ahy_k[i], csub(df[i], bf[i]));
+}
+// r = A^H A x - A^H y;  d_f = shrink(r + b_f, thr);  b_f += r - d_f.   thr < 0 encodes +infinity (mu = 0): d_f = 0.
+__global__ void __launch_bounds__(256)
+lad_data_kernel(const float2* __restrict__ ahax, const float2* __restrict__ ahy_s, float2* __restrict__ df,
+                float2* __restrict__ bf, float thr, int64_t n) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float2 r = csub(ahax[i], ahy_s[i]);
+        const float2 b = bf[i], t = cadd(r, b);
+        const float mag = sqrtf(t.x * t.x + t.y * t.y);
+        const float f = (thr < 0.f || mag <= 0.f) ? 0.f : fmaxf(mag - thr, 0.f) / mag;
+        const float2 dn = cscale(t, f);
+        df[i] = dn;
+        bf[i] = cadd(b, csub(r, dn));
+    }
+}
+
 // ---- density compensation, eqs. (6)-(7) PAPER.md:118-122 (reading R21) ----
 // w = 1 (complex64 with zero imaginary part)
 __global__ void __launch_bounds__(256) dcf_init_kernel(float2* __restrict__ w, int64_t M) {

@@ -135,3 +135,28 @@ def test_cg_and_multicoil_with_toeplitz_operator():
     assert rel(host(p.solve_l1tv_ols(dev(y), 1.0, 0.02, 1, 2, 2, use_coils=True)), xo) < 1e-4
     p.toeplitz_enable(False)
     p.destroy()
+
+
+@pytest.mark.parametrize("ncoil", [0, 16])
+def test_l1tv_lad(ncoil):
+    cfg = wl.config(4, scale=4)            # 64^2 radial
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    xt = wl.phantom(Nd)
+    if ncoil:
+        c = wl.coil_maps(ncoil, Nd)
+        c128 = c.astype(np.complex128)
+        y = orc.forward_coils(xt.astype(np.complex128), c128, om, Nd, Kd, Jd)
+        AHA = lambda z: orc.selfadjoint_coils(z, c128, om, Nd, Kd, Jd)
+        adj = lambda v: orc.adjoint_coils(v, c128, om, Nd, Kd, Jd)
+    else:
+        y = orc.forward(xt.astype(np.complex128), om, Nd, Kd, Jd)
+        AHA = lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd)
+        adj = lambda v: orc.adjoint(v, om, Nd, Kd, Jd)
+    y = (y + wl.noise_like(y)).astype(np.complex64)
+    p = make_plan(cfg, max_batch=max(ncoil, 1))
+    if ncoil:
+        p.set_coils(dev(c))
+    xo = nxt.l1tv_lad(AHA, adj(y.astype(np.complex128)), 1.0, 0.02, 2, 2, 2)
+    xg = p.solve_l1tv_lad(dev(y), 1.0, 0.02, 2, 2, 2, use_coils=bool(ncoil))
+    assert rel(host(xg), xo) < 1e-4
+    p.destroy()
