@@ -46,7 +46,7 @@ struct IlRowParams {
 // a1 + first pass of a2: x (scaled, circularly zero-padded) -> FFT along axis 1 -> grid_il rows
 // CTA = T images of one image row; thread (t, q0) works on image t.
 template <int K>
-__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS, (K == 512) ? 4 : 1)
 fft_il_rows_fwd_kernel(IlRowParams p) {
     constexpr int N = K / 2, T = Rad<K>::TS;
     extern __shared__ float2 smem[];

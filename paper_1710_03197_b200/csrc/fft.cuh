@@ -326,7 +326,7 @@ struct ColPassParams {
 
 // FULL: no pruning (every input is loaded, every output stored): used once per plan to transform the Toeplitz
 // point-spread function, which fills the whole grid.
-template <int K, bool ADJ, bool FULL = false>
+template <int K, bool ADJ, bool FULL = false, bool MULT = false>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS, Rad<K>::MBS)
 fft_cols_kernel(ColPassParams p) {
     using G = FftGeom<K>;
@@ -355,7 +355,7 @@ fft_cols_kernel(ColPassParams p) {
         const int ms = p.mult_shift;
         auto ld = [&](int i) -> float2 {
             float2 v = base[i * ls];
-            if (mult) v = cmul(v, __ldg(&mult[(off + i * ls) >> ms]));
+            if (MULT) v = cmul(v, __ldg(&mult[(off + i * ls) >> ms]));
             return cconj(v);
         };
         auto st = [&](int i, float2 v) { base[i * ls] = cconj(v); };

@@ -152,6 +152,8 @@ template <int K> static cudaError_t configure_fft() {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_il_rows_adj_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_cols_kernel<K, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_cols_kernel<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_rows_full_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
@@ -187,7 +189,8 @@ template <int K> static void launch_rows(bool adj, const RowPassParams& p, cudaS
 }
 template <int K> static void launch_cols(bool adj, const ColPassParams& p, cudaStream_t st) {
     constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
-    if (adj) fft_cols_kernel<K, true><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
+    if (adj && p.mult) fft_cols_kernel<K, true, false, true><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
+    else if (adj) fft_cols_kernel<K, true><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
     else     fft_cols_kernel<K, false><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
 }
 static int tile_T(int K) {
