@@ -435,6 +435,24 @@ def extra_legs(nb, torch, peak, args):
                                   "ms_per_iteration": cg_ms / 50, "selfadjoint_ms": sa_ms,
                                   "note": "linear CG on A^H A x = A^H y, x0 = 0, scalars float64 on device (R12)"}
     p.destroy()
+    # the same 50 iterations with opts.use_graphs (one CUDA graph per CG iteration), on a non-default stream
+    pg = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1, use_graphs=1)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        xs = pg.solve_cg(y3, 5)
+        evs = []
+        for _ in range(3):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(side)
+            pg.solve_cg(y3, 50, x=xs)
+            b.record(side)
+            evs.append((a, b))
+    side.synchronize()
+    out["cfg3_2d_spiral_cg50"]["cg50_graph_ms"] = float(np.median([a.elapsed_time(b) for a, b in evs]))
+    torch.cuda.current_stream().wait_stream(side)
+    pg.destroy()
     # config 5: 32-coil 2-D radial, multi-coil A^H A and 20 split-Bregman L1TV-OLS iterations (interleaved path)
     cfg = wl.config(4)
     nc = cfg["ncoil"]

@@ -65,7 +65,10 @@ typedef struct {
                                (half-warp per sample), 2-D planar V gathers through L1/L2; 1 = always direct gather */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
-    int use_graphs;     /* 1 = capture forward/adjoint/selfadjoint into CUDA graphs on first use (default 0)     */
+    int use_graphs;     /* 1 = the CG iterations of nufft_solve_cg and of the L1TV solvers' inner solves are replayed as one
+                               CUDA graph per iteration (pointers are fixed and every scalar lives on the device); the
+                               first iteration of a call runs eagerly, the graph is cached in the plan.  Needs a
+                               non-default stream (the legacy stream cannot capture: eager launches are used).  Default 0 */
     int batch_layout;   /* workspace layout of batched 2-D transforms (PAPER.md:52 batch mode, :251-258 coils):
                            0 = auto: calls with batch >= 16 use the batch-interleaved grid [group][K0][K1][32]
                                (lanes = images; V^H in gather form with register accumulators, deterministic),

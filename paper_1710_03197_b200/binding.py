@@ -135,7 +135,7 @@ class NufftPlan:
     """
 
     def __init__(self, Nd, Kd, Jd, om, max_batch=1, adjoint_mode=0, interp_mode=0, tile=None, max_subtile=0,
-                 batch_layout=0):
+                 batch_layout=0, use_graphs=0):
         L = lib()
         self.Nd = tuple(int(n) for n in Nd)
         self.Kd = tuple(int(k) for k in Kd)
@@ -155,6 +155,7 @@ class NufftPlan:
         opts.interp_mode = int(interp_mode)
         opts.max_subtile = int(max_subtile)
         opts.batch_layout = int(batch_layout)
+        opts.use_graphs = int(use_graphs)
         if tile is not None:
             for a, t in enumerate(tile):
                 opts.tile[a] = int(t)

@@ -35,6 +35,14 @@ static thread_local int g_last_cuda_error = 0;
         if (r__ != NUFFT_OK) return r__; \
     } while (0)
 
+// identity of the captured CG iteration (operator configuration and every pointer baked into the graph)
+struct CgGraphKey {
+    bool coils, tv;
+    float mu, lam;
+    bool toep;
+    const void *x, *r, *pv, *Ap, *hist, *stream;
+};
+
 struct nufft_plan_s {
     int d = 0;
     int N[3] = {1, 1, 1}, K[3] = {1, 1, 1};
@@ -92,6 +100,9 @@ struct nufft_plan_s {
     const float2* cur_mult = nullptr;   // transient: the first adjoint column pass multiplies by this spectrum
     float2* d_dcf_img = nullptr;
     float2* d_dcf_t = nullptr;
+    cudaGraphExec_t cg_graph = nullptr;     // one CG iteration (opts.use_graphs)
+    CgGraphKey cg_key{};
+    int cg_iter_launches = 0;
     // host-buffer pipeline (nufft_*_host): copy streams, events, double-buffered device staging, lazy
     bool hp_ready = false;
     int hp_chunk = 1;
@@ -823,6 +834,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_ones); cudaFree(p->d_that); cudaFree(p->d_dcf_img); cudaFree(p->d_dcf_t);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
+    if (p->cg_graph) cudaGraphExecDestroy(p->cg_graph);
     if (p->hp_h2d) cudaStreamDestroy(p->hp_h2d);
     if (p->hp_d2h) cudaStreamDestroy(p->hp_d2h);
     for (int i = 0; i < 2; ++i) {
@@ -1310,13 +1322,57 @@ static int cg_run(nufft_plan_t p, const NormalOp& op, const float2* rhs, float2*
     }
     cg_shift_kernel<<<1, 1, 0, st>>>(p->d_scal, hist, 1);
     p->launches += 3;
-    for (int k = 0; k < niter; ++k) {
+    // One iteration has fixed pointers and scalars that live on the device, so it is one replayable CUDA graph
+    // (opts.use_graphs): the first iteration runs eagerly (lazy allocations happen there), the second is captured, the
+    // rest are replays.  Per-kernel event profiling needs eager launches.
+    auto iteration = [&]() -> int {
         NU_TRY(apply_op(p, op, pv, Ap, st));
         dot_real_kernel<<<nb, 256, 0, st>>>(pv, Ap, n, &p->d_scal->pAp);
         cg_update_xr_kernel<<<nb, 256, 0, st>>>(x, r, pv, Ap, n, p->d_scal);
         cg_update_p_kernel<<<nb, 256, 0, st>>>(pv, r, n, p->d_scal);
-        cg_shift_kernel<<<1, 1, 0, st>>>(p->d_scal, hist ? hist + k + 1 : nullptr, 0);
+        cg_shift_kernel<<<1, 1, 0, st>>>(p->d_scal, hist, 0);
         p->launches += 4;
+        return NUFFT_OK;
+    };
+    const bool graphs = p->opts.use_graphs && !p->prof_on && niter >= 3 && st != nullptr;   // the legacy stream cannot capture
+    int k = 0;
+    if (niter > 0) {
+        const int64_t l0 = p->launches;
+        NU_TRY(iteration());
+        p->cg_iter_launches = (int)(p->launches - l0);
+        k = 1;
+    }
+    if (graphs) {
+        CgGraphKey key;
+        std::memset(&key, 0, sizeof(key));
+        key.coils = op.coils; key.tv = op.tv; key.mu = op.mu; key.lam = op.lam; key.toep = p->toep_on;
+        key.x = x; key.r = r; key.pv = pv; key.Ap = Ap; key.hist = hist; key.stream = (void*)st;
+        if (!p->cg_graph || std::memcmp(&key, &p->cg_key, sizeof(key)) != 0) {
+            if (p->cg_graph) { cudaGraphExecDestroy(p->cg_graph); p->cg_graph = nullptr; }
+            const int64_t l0 = p->launches;
+            CU_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            const int rc = iteration();
+            cudaGraph_t g = nullptr;
+            const cudaError_t e = cudaStreamEndCapture(st, &g);
+            p->launches = l0;                       // the captured launches did not run
+            if (rc != NUFFT_OK || e != cudaSuccess || !g) {
+                if (g) cudaGraphDestroy(g);
+                (void)cudaGetLastError();
+                if (rc != NUFFT_OK) return rc;
+                g_last_cuda_error = (int)e;
+                return NUFFT_ECUDA;
+            }
+            const cudaError_t ei = cudaGraphInstantiate(&p->cg_graph, g, 0);
+            cudaGraphDestroy(g);
+            if (ei != cudaSuccess) { p->cg_graph = nullptr; g_last_cuda_error = (int)ei; (void)cudaGetLastError(); return NUFFT_ECUDA; }
+            p->cg_key = key;
+        }
+        for (; k < niter; ++k) {
+            CU_TRY(cudaGraphLaunch(p->cg_graph, st));
+            p->launches += p->cg_iter_launches;
+        }
+    } else {
+        for (; k < niter; ++k) NU_TRY(iteration());
     }
     CU_TRY(cudaGetLastError());
     return NUFFT_OK;

@@ -13,6 +13,7 @@ struct CgScalars {
     double pAp;       // accumulator: Re <p, A p>
     double rs_new;    // accumulator: <r, r> after the update
     double maxabs;    // scratch for max |.| reductions (bit pattern of a non-negative double, ordered as int64)
+    int hist_pos;     // next slot of the residual-norm history (kept on the device so that one iteration is one replayable graph)
 };
 
 __device__ __forceinline__ double block_reduce_sum(double v) {
@@ -93,14 +94,14 @@ cg_update_p_kernel(float2* __restrict__ p, const float2* __restrict__ r, int64_t
 }
 
 // rs <- rs_new, accumulators cleared, residual norm logged
-__global__ void cg_shift_kernel(CgScalars* s, double* hist_slot, int first) {
+__global__ void cg_shift_kernel(CgScalars* s, double* hist, int first) {
     if (!first) s->rs = s->rs_new;
     s->rs_new = 0.0;
     s->pAp = 0.0;
-    if (hist_slot) *hist_slot = sqrt(s->rs);
+    if (hist) hist[s->hist_pos++] = sqrt(s->rs);
 }
 
-__global__ void scalars_clear_kernel(CgScalars* s) { s->rs = 0.0; s->pAp = 0.0; s->rs_new = 0.0; s->maxabs = 0.0; }
+__global__ void scalars_clear_kernel(CgScalars* s) { s->rs = 0.0; s->pAp = 0.0; s->rs_new = 0.0; s->maxabs = 0.0; s->hist_pos = 0; }
 
 // max |a_i|  (non-negative doubles order like their bit patterns)
 __global__ void __launch_bounds__(256)

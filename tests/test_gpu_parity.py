@@ -534,3 +534,33 @@ def test_cg_config3_parity_against_the_oracles_own_noise_floor(repo_root):
     for niter, v in out.items():
         assert v["gpu_vs_oracle"] < max(1e-4, 1e9 * v["oracle_noise_floor_1e-12"]), (niter, v)
     p.destroy()
+
+
+def test_cg_iterations_replayed_as_cuda_graph_match_eager():
+    """opts.use_graphs: the CG iteration captured once and replayed (on a non-default stream) gives the bits of the eager
+    run in deterministic V^H mode, for CG and for the inner solves of L1TV-OLS, and survives repeated calls."""
+    cfg = wl.config(1, scale=2)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    y = dev(wl.data_gaussian(om.shape[0]))
+    pe = make_plan(cfg, adjoint_mode=1)
+    pg = make_plan(cfg, adjoint_mode=1, use_graphs=1)
+    xe, he = pe.solve_cg(y, 12, want_history=True)
+    xl = pe.solve_l1tv_ols(y, 1.0, 0.02, 2, 2, 3)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        for _ in range(2):
+            xg, hg = pg.solve_cg(y, 12, want_history=True)
+            xlg = pg.solve_l1tv_ols(y, 1.0, 0.02, 2, 2, 3)
+    side.synchronize()
+    assert np.array_equal(host(xe).view(np.uint32), host(xg).view(np.uint32))
+    assert np.allclose(he, hg, rtol=1e-10)      # float64 block sums are combined by atomics: order-free to ~1e-16
+    assert np.array_equal(host(xl).view(np.uint32), host(xlg).view(np.uint32))
+    xo, _ = sol.cg(lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd),
+                   orc.adjoint(host(y).astype(np.complex128), om, Nd, Kd, Jd), 3)
+    with torch.cuda.stream(side):
+        x3 = pg.solve_cg(y, 3)
+    side.synchronize()
+    assert rel(host(x3), xo) < 1e-4
+    pe.destroy()
+    pg.destroy()
