@@ -429,20 +429,17 @@ interp_tiled_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ it
             const float4 wa = *reinterpret_cast<const float4*>(rec), wb = *reinterpret_cast<const float4*>(rec + 4);
             const float w0[kJ] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y};
             const float wc = rec[16 + cc];
-            const float w12[3] = {rec[8 + rr] * wc, rec[10 + rr] * wc, rec[12 + rr] * wc};
+            // packed two-wide FP32 FMA (fma.rn.f32x2 / FFMA2): (re, im) of a cell travel as one register pair
+            const float wa0 = rec[8 + rr] * wc, wa1 = rec[10 + rr] * wc, wa2 = rec[12 + rr] * wc;
+            const float2 w12[3] = {make_float2(wa0, wa0), make_float2(wa1, wa1), make_float2(wa2, wa2)};
             const float2* __restrict__ tp = tile + __float_as_int(rec[24]) + lane_off;
             float2 acc = make_float2(0.f, 0.f);
 #pragma unroll
             for (int p = 0; p < kJ; ++p) {
-                float2 tsum = make_float2(0.f, 0.f);
-#pragma unroll
-                for (int gq = 0; gq < 3; ++gq) {
-                    const float2 v = tp[p * k3Plane + 2 * gq * k3Pitch];
-                    tsum.x = fmaf(w12[gq], v.x, tsum.x);
-                    tsum.y = fmaf(w12[gq], v.y, tsum.y);
-                }
-                acc.x = fmaf(w0[p], tsum.x, acc.x);
-                acc.y = fmaf(w0[p], tsum.y, acc.y);
+                float2 tsum = __fmul2_rn(w12[0], tp[p * k3Plane]);
+                tsum = __ffma2_rn(w12[1], tp[p * k3Plane + 2 * k3Pitch], tsum);
+                tsum = __ffma2_rn(w12[2], tp[p * k3Plane + 4 * k3Pitch], tsum);
+                acc = __ffma2_rn(make_float2(w0[p], w0[p]), tsum, acc);
             }
 #pragma unroll
             for (int off = 8; off > 0; off >>= 1) {
