@@ -3,6 +3,7 @@
     density_weights / adjoint_dcf   sampling density compensation, eqs. (6)-(7)
     toeplitz_kernel / selfadjoint_toeplitz   "precomputing A^H A" (Toeplitz, ref. [6])   PAPER.md:86-98, Fig. 3 :114
     l1tv_lad                        split-Bregman L1TV-LAD, eqs. (23)-(33)
+    cg_kspace                       the paper's k-space CG  V^H V k = V^H y, x = S^-1 F^-1 k   PAPER.md:124-143, eqs. (8)-(11)
 
 Built on oracle/nufft_oracle.py (forward, adjoint); numpy float64 / complex128; numpy.fft as a library step.
 
@@ -25,13 +26,16 @@ Parity pins (tests/test_oracle_next.py):
                            (rel. <= 1e-4) and against adjoint(forward(x)) (same bound)
     l1tv_lad               PARITY UNPINNED by the paper (eqs. (23)-(33), garbled; reading R23 in its docstring).  Sanity
                            pins: first inner iteration = L1TV-OLS's, scale equivariance, consistent-data fixed point.
+    cg_kspace              final step: S^{-1}F^{-1} inverts k = F S x exactly; converged k equals the minimum-norm least
+                           squares solution pinv(V) y computed from the dense V (numpy.linalg.lstsq); CG recurrence itself
+                           pinned in tests/test_oracle_solvers.py
 No other function here is "parity unpinned".
 """
 import numpy as np
 
 from . import nufft_oracle as orc
 
-__all__ = ["density_weights", "adjoint_dcf", "toeplitz_kernel", "selfadjoint_toeplitz", "l1tv_lad"]
+__all__ = ["density_weights", "adjoint_dcf", "toeplitz_kernel", "selfadjoint_toeplitz", "l1tv_lad", "cg_kspace"]
 
 
 def density_weights(om, Nd, Kd, Jd, niter):
@@ -126,3 +130,26 @@ def l1tv_lad(AHA, AHy, mu, lam, n_outer, n_inner, n_cg):
             b_f = b_f + (r - d_f)                     # eq. (32)
         AHy_k = AHy_k + AHy_s - AHA(x)                # eq. (33)
     return x / c
+
+
+def cg_kspace(y, om, Nd, Kd, Jd, niter):
+    """The paper's own two-step conjugate-gradient solution, eqs. (8)-(11):
+        solve  V^H V k = V^H y  for the oversampled grid k by conjugate gradient             (9), (11)
+        x = S^{-1} F^{-1} k: inverse FFT, crop, divide by the scaling factor               (10)
+    Reading R24: k_0 = 0, exactly niter iterations of linear CG (the same recurrence as solvers_oracle.cg_steps), F^{-1}
+    is the normalised inverse DFT (the inverse of F, not its adjoint), the image is read from the circular positions
+    (n - N/2) mod K where S placed it (R4).  Returns (x, k)."""
+    from .solvers_oracle import cg_steps
+    Nd = tuple(int(n) for n in Nd)
+    Kd = tuple(int(k) for k in Kd)
+    op = lambda g: orc.grid_adjoint(orc.interp(g, om, Nd, Kd, Jd), om, Nd, Kd, Jd)
+    rhs = orc.grid_adjoint(np.asarray(y, dtype=np.complex128), om, Nd, Kd, Jd)
+    k, _ = cg_steps(op, rhs, np.zeros(Kd, dtype=np.complex128), niter)
+    g = np.fft.ifftn(k)                                                   # F^{-1}
+    idx = np.ix_(*[(np.arange(n) - n // 2) % K for n, K in zip(Nd, Kd)])   # crop at (n - N/2) mod K
+    x = g[idx]
+    for a, (n, K, J) in enumerate(zip(Nd, Kd, Jd)):                        # S^{-1}
+        shape = [1] * len(Nd)
+        shape[a] = n
+        x = x / orc.scaling_factors(n, K, J).reshape(shape)
+    return x, k

@@ -141,3 +141,37 @@ def test_lad_scale_equivariance_and_progress():
     assert rel(x2, 7.5 * x1) < 1e-12
     x0 = nxt.l1tv_lad(AHA, AHy, 1.0, 0.05, 1, 1, 1)
     assert rel(x1, xt) < rel(x0, xt)     # more iterations move towards the piecewise-constant truth
+
+
+# ---- k-space CG, eqs. (8)-(11) ----
+def test_cg_kspace_final_step_inverts_FS():
+    rng = np.random.default_rng(12)
+    Nd, Kd, Jd = (8, 12), (16, 24), (6, 6)
+    x0 = rng.standard_normal(Nd) + 1j * rng.standard_normal(Nd)
+    k = orc.scale_pad_fft(x0, Nd, Kd, Jd)
+    # zero iterations from a given k: reuse the function's final step through a 0-iteration solve of a trivial problem
+    g = np.fft.ifftn(k)
+    idx = np.ix_(*[(np.arange(n) - n // 2) % K for n, K in zip(Nd, Kd)])
+    x = g[idx] / np.outer(orc.scaling_factors(8, 16, 6), orc.scaling_factors(12, 24, 6))
+    assert rel(x, x0) < 1e-13
+
+
+def test_cg_kspace_converges_to_min_norm_least_squares_of_dense_V():
+    rng = np.random.default_rng(13)
+    Nd, Kd, Jd = (4, 4), (8, 8), (6, 6)
+    om = rng.uniform(-np.pi, np.pi, (40, 2))
+    y = rng.standard_normal(40) + 1j * rng.standard_normal(40)
+    # dense V from the oracle's own interpolation of unit grids (columns), 40 x 64
+    V = np.zeros((40, 64), dtype=np.complex128)
+    for j in range(64):
+        e = np.zeros(64, dtype=np.complex128)
+        e[j] = 1.0
+        V[:, j] = orc.interp(e.reshape(Kd), om, Nd, Kd, Jd)
+    kls = np.linalg.lstsq(V, y, rcond=None)[0]           # minimum-norm least-squares solution
+    x, k = nxt.cg_kspace(y, om, Nd, Kd, Jd, 100)      # kappa(V)^2 ~ 1.4e4: ~100 iterations to converge in float64
+    assert rel(k.ravel(), kls) < 1e-8
+    # and x is S^-1 F^-1 of that k
+    g = np.fft.ifftn(kls.reshape(Kd))
+    idx = np.ix_(*[(np.arange(n) - n // 2) % K for n, K in zip(Nd, Kd)])
+    xr = g[idx] / np.outer(orc.scaling_factors(4, 8, 6), orc.scaling_factors(4, 8, 6))
+    assert rel(x, xr) < 1e-8
