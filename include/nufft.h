@@ -169,6 +169,12 @@ int nufft_selfadjoint_toeplitz_coils(nufft_plan_t p, const nufft_c64 *x_in, nuff
 int nufft_solve_l1tv_lad(nufft_plan_t p, int use_coils, const nufft_c64 *y, nufft_c64 *x,
                          double mu, double lam, int n_outer, int n_inner, int n_cg, void *stream);
 
+/* The paper's own conjugate-gradient solution, eqs.(8)-(11) (reading R24): CG on V^H V k = V^H y over the
+ * oversampled grid (k_0 = 0, exactly niter iterations, float64 scalars on the device), then x = S^-1 F^-1 k (normalised
+ * inverse FFT, crop, divide by the scaling factor; eq.(10)).  y: device [M]; x: device [prod Nd] (output).  Single image,
+ * planar path; 5 grid-sized work vectors are allocated on first use.  resnorm_host as in nufft_solve_cg. */
+int nufft_solve_cg_kspace(nufft_plan_t p, const nufft_c64 *y, nufft_c64 *x, int niter, double *resnorm_host, void *stream);
+
 /* Plan facts.  Any pointer may be NULL.  bytes_plan = device bytes of per-sample plan data; bytes_work = device
  * bytes of workspace (grids, sample buffers, solver vectors); n_tiles / n_work = V^H tiles and work items (after
  * hot-tile splitting); max_tile_samples = the largest tile's sample count. */

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "nufft_default_opts", "nufft_plan", "nufft_forward", "nufft_adjoint", "nufft_selfadjoint",
     "nufft_forward_host", "nufft_adjoint_host", "nufft_selfadjoint_host",
     "nufft_density_weights", "nufft_adjoint_dcf", "nufft_toeplitz_build", "nufft_toeplitz_enable",
-    "nufft_selfadjoint_toeplitz", "nufft_selfadjoint_toeplitz_coils", "nufft_solve_l1tv_lad",
+    "nufft_selfadjoint_toeplitz", "nufft_selfadjoint_toeplitz_coils", "nufft_solve_l1tv_lad", "nufft_solve_cg_kspace",
     "nufft_stage_scale_fft", "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale",
     "nufft_set_coils", "nufft_forward_coils", "nufft_adjoint_coils", "nufft_selfadjoint_coils",
     "nufft_solve_cg", "nufft_solve_l1tv_ols", "nufft_plan_info", "nufft_launch_count", "nufft_destroy",
@@ -75,6 +75,7 @@ def lib():
     L.nufft_solve_l1tv_ols.argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _c.c_double, _c.c_double, _c.c_int, _c.c_int,
                                        _c.c_int, _PTR]
     L.nufft_solve_l1tv_lad.argtypes = L.nufft_solve_l1tv_ols.argtypes
+    L.nufft_solve_cg_kspace.argtypes = [_PLAN, _PTR, _PTR, _c.c_int, _c.POINTER(_c.c_double), _PTR]
     L.nufft_plan_info.argtypes = [_PLAN, _I64P, _I64P, _I64P, _I64P, _I64P]
     L.nufft_launch_count.argtypes = [_PLAN]
     L.nufft_launch_count.restype = _c.c_int64
@@ -319,6 +320,13 @@ class NufftPlan:
                                           float(mu), float(lam), int(n_outer), int(n_inner), int(n_cg), _stream()),
                "nufft_solve_l1tv_ols")
         return x
+
+    def solve_cg_kspace(self, y, niter, x=None, want_history=False):
+        x = self._new(*self.Nd) if x is None else x
+        hist = (_c.c_double * (niter + 1))() if want_history else None
+        _check(lib().nufft_solve_cg_kspace(self._h, _dev(y, "y", self.M), _dev(x, "x", self.nimg), int(niter), hist,
+                                           _stream()), "nufft_solve_cg_kspace")
+        return (x, np.array(hist[:])) if want_history else x
 
     def solve_l1tv_lad(self, y, mu, lam, n_outer, n_inner, n_cg, use_coils=False, x=None):
         x = self._new(*self.Nd) if x is None else x

@@ -97,6 +97,9 @@ struct nufft_plan_s {
     float2* d_that = nullptr;       // Toeplitz spectrum T^ on the K grid, planar [K0][K1]([K2])
     bool toep_on = false;           // solvers and selfadjoint calls use the Toeplitz operator
     bool unit_scale = false;        // transient: FFT row passes use d_ones
+    bool inv_scale = false;         // transient: FFT row passes use d_sinv (1 / (s K)): x = S^-1 F^-1 k of eq. (10)
+    float* d_sinv[3] = {nullptr, nullptr, nullptr};
+    float2* d_kspace = nullptr;     // 5 grid-sized vectors of the k-space CG, lazy
     const float2* cur_mult = nullptr;   // transient: the first adjoint column pass multiplies by this spectrum
     float2* d_dcf_img = nullptr;
     float2* d_dcf_t = nullptr;
@@ -243,13 +246,14 @@ static RowPassParams row_params(nufft_plan_t p, int batch, const float2* img_in,
     RowPassParams r{};
     r.img_in = img_in; r.img_out = img_out; r.grid = grid; r.coil = coil;
     const int d = p->d;
-    r.s_line = p->unit_scale ? p->d_ones : p->d_scale[d - 1];
+    auto sc = [&](int a) -> const float* { return p->unit_scale ? p->d_ones : (p->inv_scale ? p->d_sinv[a] : p->d_scale[a]); };
+    r.s_line = sc(d - 1);
     r.tw = p->d_tw[d - 1];
     if (d == 2) {
-        r.s_outer0 = p->unit_scale ? p->d_ones : p->d_scale[0]; r.s_outer1 = nullptr;
+        r.s_outer0 = sc(0); r.s_outer1 = nullptr;
         r.n_outer0 = p->N[0]; r.n_outer1 = 1; r.k_outer0 = p->K[0]; r.k_outer1 = 1;
     } else {
-        r.s_outer0 = p->unit_scale ? p->d_ones : p->d_scale[0]; r.s_outer1 = p->unit_scale ? p->d_ones : p->d_scale[1];
+        r.s_outer0 = sc(0); r.s_outer1 = sc(1);
         r.n_outer0 = p->N[0]; r.n_outer1 = p->N[1]; r.k_outer0 = p->K[0]; r.k_outer1 = p->K[1];
     }
     r.nlines = batch * r.n_outer0 * r.n_outer1;
@@ -831,6 +835,8 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_grid); cudaFree(p->d_ywork); cudaFree(p->d_imgwork); cudaFree(p->d_solver);
     cudaFree(p->d_scal); cudaFree(p->d_hist);
     cudaFree(p->d_items); cudaFree(p->d_tile_item_start); cudaFree(p->d_slabs);
+    for (int a = 0; a < 3; ++a) cudaFree(p->d_sinv[a]);
+    cudaFree(p->d_kspace);
     cudaFree(p->d_ones); cudaFree(p->d_that); cudaFree(p->d_dcf_img); cudaFree(p->d_dcf_t);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
@@ -1295,8 +1301,13 @@ struct NormalOp {
     bool coils;
     bool tv;
     float mu, lam;
+    bool kspace = false;      // the operator is V^H V on the oversampled grid (the paper's k-space CG, eq. 11)
 };
 static int apply_op(nufft_plan_t p, const NormalOp& op, const float2* in, float2* out, cudaStream_t st) {
+    if (op.kspace) {          // out = V^H (V in), planar grid vectors of prod(K) cells
+        NU_TRY(run_interp(p, 1, in, p->d_ywork, st));
+        return run_gridding(p, 1, p->d_ywork, out, st);
+    }
     NU_TRY(apply_aha(p, op.coils, in, out, st));
     if (op.tv) {
         tv_normal_kernel<<<ew_blocks(p->nimg), 256, 0, st>>>(out, in, op.mu, op.lam, p->N[0], p->N[1]);
@@ -1310,7 +1321,7 @@ static int apply_op(nufft_plan_t p, const NormalOp& op, const float2* in, float2
 // r, pv, Ap: work vectors.  hist: device double[niter + 1] or nullptr.
 static int cg_run(nufft_plan_t p, const NormalOp& op, const float2* rhs, float2* x, bool warm, int niter, float2* r,
                   float2* pv, float2* Ap, double* hist, cudaStream_t st) {
-    const int64_t n = p->nimg;
+    const int64_t n = op.kspace ? p->cells : p->nimg;
     const int nb = ew_blocks(n);
     scalars_clear_kernel<<<1, 1, 0, st>>>(p->d_scal);
     if (warm) {
@@ -1345,7 +1356,7 @@ static int cg_run(nufft_plan_t p, const NormalOp& op, const float2* rhs, float2*
     if (graphs) {
         CgGraphKey key;
         std::memset(&key, 0, sizeof(key));
-        key.coils = op.coils; key.tv = op.tv; key.mu = op.mu; key.lam = op.lam; key.toep = p->toep_on;
+        key.coils = op.coils; key.tv = op.tv; key.mu = op.mu; key.lam = op.lam; key.toep = p->toep_on || op.kspace;
         key.x = x; key.r = r; key.pv = pv; key.Ap = Ap; key.hist = hist; key.stream = (void*)st;
         if (!p->cg_graph || std::memcmp(&key, &p->cg_key, sizeof(key)) != 0) {
             if (p->cg_graph) { cudaGraphExecDestroy(p->cg_graph); p->cg_graph = nullptr; }
@@ -1397,6 +1408,41 @@ extern "C" int nufft_solve_cg(nufft_plan_t p, int use_coils, const nufft_c64* y,
     NU_TRY(adjoint_any(p, coils, (const float2*)y, rhs, st));
     NormalOp op{coils, false, 1.f, 0.f};
     NU_TRY(cg_run(p, op, rhs, (float2*)x, false, niter, r, pv, Ap, p->d_hist, st));
+    if (resnorm_host) {
+        CU_TRY(cudaMemcpyAsync(resnorm_host, p->d_hist, (size_t)(niter + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+    }
+    return NUFFT_OK;
+}
+
+// The paper's own CG (eqs. 8-11; reading R24): conjugate gradient on V^H V k = V^H y over the
+// oversampled grid, k_0 = 0, exactly niter iterations; then x = S^-1 F^-1 k (normalised inverse FFT, crop, divide by the
+// scaling factor).
+extern "C" int nufft_solve_cg_kspace(nufft_plan_t p, const nufft_c64* y, nufft_c64* x, int niter, double* resnorm_host,
+                                     void* stream) {
+    if (!p || !x || (!y && p->M > 0) || niter < 0) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n = p->cells;
+    if (!p->d_kspace) NU_TRY(dev_alloc((void**)&p->d_kspace, (size_t)5 * n * sizeof(float2), &p->bytes_work));
+    if (!p->d_sinv[0]) {
+        for (int a = 0; a < p->d; ++a) {
+            std::vector<float> s = host::scaling_vector(p->N[a], p->K[a], (double)kJ);
+            // 1 / (s K): computed in float64 from the float64 scaling factor, rounded once
+            const double beta = host::kb_beta((double)kJ, (double)p->K[a] / (double)p->N[a]);
+            for (int i = 0; i < p->N[a]; ++i)
+                s[i] = (float)(host::kb_Phi(((double)i - 0.5 * p->N[a]) / (double)p->K[a], (double)kJ, beta) / (double)p->K[a]);
+            NU_TRY(dev_upload(&p->d_sinv[a], s, &p->bytes_plan));
+        }
+    }
+    NU_TRY(ensure_solver(p, 0, niter + 1));
+    float2 *rhs = p->d_kspace, *k = rhs + n, *r = k + n, *pv = r + n, *Ap = pv + n;
+    NU_TRY(run_gridding(p, 1, (const float2*)y, rhs, st));                 // V^H y
+    NormalOp op{false, false, 1.f, 0.f, true};
+    NU_TRY(cg_run(p, op, rhs, k, false, niter, r, pv, Ap, p->d_hist, st));
+    p->inv_scale = true;                                                     // x = S^-1 F^-1 k  (eq. 10); k is consumed
+    const int rc = run_fft_scale(p, 1, k, (float2*)x, nullptr, st);
+    p->inv_scale = false;
+    NU_TRY(rc);
     if (resnorm_host) {
         CU_TRY(cudaMemcpyAsync(resnorm_host, p->d_hist, (size_t)(niter + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
         CU_TRY(cudaStreamSynchronize(st));

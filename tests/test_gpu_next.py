@@ -160,3 +160,21 @@ def test_l1tv_lad(ncoil):
     xg = p.solve_l1tv_lad(dev(y), 1.0, 0.02, 2, 2, 2, use_coils=bool(ncoil))
     assert rel(host(xg), xo) < 1e-4
     p.destroy()
+
+
+@pytest.mark.parametrize("ci,scale", [(0, 1), (1, 4), (3, 8)])
+def test_cg_kspace(ci, scale):
+    """The paper's k-space CG (eqs. 8-11): iterates 1 and 4 against the oracle (<= 1e-4; V^H V is singular on the
+    oversampled grid, so late iterates amplify rounding like config 3's image-space CG)."""
+    cfg = wl.config(ci, scale=scale)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    y = wl.data_gaussian(om.shape[0])
+    p = make_plan(cfg, adjoint_mode=1)
+    for niter in (0, 1, 4):
+        xo, _ = nxt.cg_kspace(y.astype(np.complex128), om, Nd, Kd, Jd, niter)
+        xg = host(p.solve_cg_kspace(dev(y), niter))
+        if niter == 0:
+            assert float(np.abs(xg).max()) == 0.0 and float(np.abs(xo).max()) == 0.0
+        else:
+            assert rel(xg, xo) < 1e-4, (niter, rel(xg, xo))
+    p.destroy()
