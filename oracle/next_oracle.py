@@ -7,7 +7,7 @@
 
 Built on oracle/nufft_oracle.py (forward, adjoint); numpy float64 / complex128; numpy.fft as a library step.
 
-Readings of the paper taken here (R21-R22):
+Readings of the paper taken here (R21-R24; R23 and R24 are stated in the docstrings of l1tv_lad and cg_kspace):
     R21  eq. (6) w_{i+1} = w_i / (A A^H w_i): the paper gives neither w_0, nor the iteration count, nor how a complex
          A A^H w is divided into a real density function.  Taken: w_0 = 1, w real, w_{i+1} = w_i / |A A^H w_i|
          (elementwise magnitude, as in ref. [7]'s iteration), a fixed iteration count given by the caller.
