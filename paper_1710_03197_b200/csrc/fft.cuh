@@ -106,7 +106,7 @@ template <int K> struct Rad;
 template <> struct Rad<32>   { static constexpr int R1 = 8,  R2 = 4,  R3 = 1, E = 8,  PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32, MBS = 1; };
 template <> struct Rad<64>   { static constexpr int R1 = 8,  R2 = 8,  R3 = 1, E = 8,  PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32, MBS = 1; };
 template <> struct Rad<128>  { static constexpr int R1 = 16, R2 = 8,  R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 32, MBS = 1; };
-template <> struct Rad<256>  { static constexpr int R1 = 16, R2 = 16, R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 16, MBS = 1; };
+template <> struct Rad<256>  { static constexpr int R1 = 16, R2 = 16, R3 = 1, E = 16, PC1 = 1, PC2 = 0, PS1 = 0, PS2 = 0, TS = 16, LC = 16, MBS = 4; };
 template <> struct Rad<512>  { static constexpr int R1 = 8,  R2 = 8,  R3 = 8, E = 8,  PC1 = 8, PC2 = 1, PS1 = 0, PS2 = 1, TS = 8,  LC = 4, MBS = 3;  };
 template <> struct Rad<1024> { static constexpr int R1 = 16, R2 = 8,  R3 = 8, E = 16, PC1 = 8, PC2 = 1, PS1 = 0, PS2 = 1, TS = 8,  LC = 4, MBS = 1;  };
 
