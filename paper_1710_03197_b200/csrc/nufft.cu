@@ -363,7 +363,7 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
 // a4: grid = V^H y
 static constexpr int kGrid2dWarps = 8;
 static size_t smem_grid2d(nufft_plan_t p) { return (size_t)kGrid2dWarps * ((size_t)p->tg.tile_cells * 8 + kStageBytes); }
-static size_t smem_grid3d(nufft_plan_t p) { return (size_t)p->tg.tile_cells * 8 + 6 * (size_t)kStageBytes; }
+static size_t smem_grid3d(nufft_plan_t p) { return (size_t)p->tg.tile_cells * 8 + (size_t)kStage3dBytes; }
 
 static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid, cudaStream_t st) {
     const bool det = p->opts.adjoint_mode == 1;

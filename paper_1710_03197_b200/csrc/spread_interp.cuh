@@ -268,6 +268,13 @@ gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
 }
 
 // 3-D: one work item per CTA of 6 warps; warp w owns the tile-local planes = w (mod 6).
+// Staging is CTA-wide, 32 samples per round: warp 0 writes the part every warp needs (per stencil row r: the row weight
+// and the cell offset of the row's 8-cell window; per cell pair q: the two column weights), every warp writes its own
+// 16 bytes per sample (y times the plane weight of ITS plane of that sample, and the plane offset).  Per sample and
+// warp the apply loop then costs three small loads, one 16-byte read-modify-write and six FMAs per lane.
+constexpr int k3CommonF2 = 10;                                             // float2 slots per sample: 6 rows + 4 pairs
+constexpr int kStage3dBytes = 32 * k3CommonF2 * 8 + 6 * 32 * 16;           // 2560 + 3072
+
 template <bool DET>
 __global__ void __launch_bounds__(192)
 gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items, int n_items,
@@ -277,37 +284,64 @@ gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y;
     float2* tile = reinterpret_cast<float2*>(smem4);
-    float4* rowrec = reinterpret_cast<float4*>(tile + tg.tile_cells) + (size_t)warp * (kStageBytes / 16);
-    float2* colrec = reinterpret_cast<float2*>(rowrec + 32 * kStageRow);
+    float2* common = tile + tg.tile_cells;                                  // [32][k3CommonF2]
+    float4* perwarp = reinterpret_cast<float4*>(common + 32 * k3CommonF2);  // [6][32]
     const WorkItem wi = items[blockIdx.x];
     int o[3];
     unpack_k0(wi.origin, o);
     for (int i = threadIdx.x; i < tg.tile_cells / 2; i += blockDim.x)
         reinterpret_cast<float4*>(tile)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    __syncthreads();
     const float2* __restrict__ yb = y + (int64_t)b * g.M;
+    const int r = lane >> 2, q = lane & 3;
     for (int s0 = wi.s_begin; s0 < wi.s_end; s0 += 32) {
         const int si = s0 + lane;
         const int cnt = min(32, wi.s_end - s0);
+        __syncthreads();              // tile zeroed (first round) / previous round's records consumed
         if (si < wi.s_end) {
             int k0[3];
             unpack_k0(__ldg(&s.kpack[si]), k0);
-            const float d0 = __ldg(&s.delta[si]), d1 = __ldg(&s.delta[g.M + si]), d2 = __ldg(&s.delta[2 * g.M + si]);
             const float2 yv = __ldg(&yb[__ldg(&s.perm[si])]);
-            const int c0 = (k0[0] - o[0]) & (g.K[0] - 1), c1 = (k0[1] - o[1]) & (g.K[1] - 1);
-            const int c2 = (k0[2] - o[2]) & (g.K[2] - 1);
+            const int c0 = (k0[0] - o[0]) & (g.K[0] - 1);
             // this warp's plane of the sample: tile-local plane c0 + j0 = warp (mod 6)
             const int j0 = (warp - c0 % 6 + 6) % 6;
             float wz[kJ];
-            kb_weights(P, d0, wz);
+            kb_weights(P, __ldg(&s.delta[si]), wz);
             float wsel = wz[0];
 #pragma unroll
             for (int j = 1; j < kJ; ++j) wsel = (j0 == j) ? wz[j] : wsel;
-            stage_sample_2d(P, rowrec, colrec, lane, c1, c2, d1, d2, cscale(yv, wsel), tg.pitch, (c0 + j0) * tg.plane);
+            perwarp[warp * 32 + lane] = make_float4(yv.x * wsel, yv.y * wsel, __int_as_float((c0 + j0) * tg.plane), 0.f);
+            if (warp == 0) {
+                const int c1 = (k0[1] - o[1]) & (g.K[1] - 1), c2 = (k0[2] - o[2]) & (g.K[2] - 1);
+                float w1[kJ], w2[kJ];
+                kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
+                kb_weights(P, __ldg(&s.delta[2 * g.M + si]), w2);
+                const int par = c2 & 1, base = c1 * tg.pitch + (c2 - par);
+                float2* rec = common + lane * k3CommonF2;
+#pragma unroll
+                for (int rr = 0; rr < kJ; ++rr) rec[rr] = make_float2(w1[rr], __int_as_float(base + rr * tg.pitch));
+                rec[6] = par ? make_float2(0.f, w2[0]) : make_float2(w2[0], w2[1]);
+                rec[7] = par ? make_float2(w2[1], w2[2]) : make_float2(w2[2], w2[3]);
+                rec[8] = par ? make_float2(w2[3], w2[4]) : make_float2(w2[4], w2[5]);
+                rec[9] = par ? make_float2(w2[5], 0.f) : make_float2(0.f, 0.f);
+            }
         }
-        __syncwarp();
-        apply_staged(tile, rowrec, colrec, cnt, lane);
-        __syncwarp();
+        __syncthreads();
+        if (lane < 24) {
+            const float4* pw = perwarp + warp * 32;
+            for (int sidx = 0; sidx < cnt; ++sidx) {
+                const float4 ps = pw[sidx];
+                const float2 wr = common[sidx * k3CommonF2 + r];
+                const float2 cc = common[sidx * k3CommonF2 + 6 + q];
+                const float rx = ps.x * wr.x, ry = ps.y * wr.x;
+                float4* cell = reinterpret_cast<float4*>(tile + __float_as_int(ps.z) + __float_as_int(wr.y) + 2 * q);
+                float4 a = *cell;
+                a.x = fmaf(rx, cc.x, a.x);
+                a.y = fmaf(ry, cc.x, a.y);
+                a.z = fmaf(rx, cc.y, a.z);
+                a.w = fmaf(ry, cc.y, a.w);
+                *cell = a;
+            }
+        }
     }
     __syncthreads();
     flush_tile<3, DET>(tile, tg, g, wi.origin, grid + (int64_t)b * g.cells,
