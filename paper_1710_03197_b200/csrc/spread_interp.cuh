@@ -327,18 +327,37 @@ gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
         }
         __syncthreads();
         if (lane < 24) {
+            // Run-length merge: consecutive samples of the sorted order that share all three stencil base indices (a
+            // radial readout oversampled 2x advances half a cell per sample) hit the same cells; their contributions
+            // are summed in registers and written with ONE read-modify-write.  The test is warp-uniform.
             const float4* pw = perwarp + warp * 32;
+            int prevkey = -1;
+            float4 pend = make_float4(0.f, 0.f, 0.f, 0.f);
             for (int sidx = 0; sidx < cnt; ++sidx) {
                 const float4 ps = pw[sidx];
                 const float2 wr = common[sidx * k3CommonF2 + r];
                 const float2 cc = common[sidx * k3CommonF2 + 6 + q];
                 const float rx = ps.x * wr.x, ry = ps.y * wr.x;
-                float4* cell = reinterpret_cast<float4*>(tile + __float_as_int(ps.z) + __float_as_int(wr.y) + 2 * q);
+                const int key = __float_as_int(ps.z) + __float_as_int(wr.y);
+                if (key != prevkey) {
+                    if (prevkey >= 0) {
+                        float4* cell = reinterpret_cast<float4*>(tile + prevkey + 2 * q);
+                        float4 a = *cell;
+                        a.x += pend.x; a.y += pend.y; a.z += pend.z; a.w += pend.w;
+                        *cell = a;
+                    }
+                    pend = make_float4(0.f, 0.f, 0.f, 0.f);
+                    prevkey = key;
+                }
+                pend.x = fmaf(rx, cc.x, pend.x);
+                pend.y = fmaf(ry, cc.x, pend.y);
+                pend.z = fmaf(rx, cc.y, pend.z);
+                pend.w = fmaf(ry, cc.y, pend.w);
+            }
+            if (prevkey >= 0) {
+                float4* cell = reinterpret_cast<float4*>(tile + prevkey + 2 * q);
                 float4 a = *cell;
-                a.x = fmaf(rx, cc.x, a.x);
-                a.y = fmaf(ry, cc.x, a.y);
-                a.z = fmaf(rx, cc.y, a.z);
-                a.w = fmaf(ry, cc.y, a.w);
+                a.x += pend.x; a.y += pend.y; a.z += pend.z; a.w += pend.w;
                 *cell = a;
             }
         }
