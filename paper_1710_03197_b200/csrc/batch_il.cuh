@@ -296,15 +296,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     } while (!ok);
 }
 
-constexpr int kStageCap = 48;      // samples per list per staging round
-constexpr int kGridSmemBytes = 3 * kStageCap * (kTabW * 4 + kIL * 8) + 16;
+constexpr int kStageCap = 48;      // samples per list per staging round (one group per CTA)
+constexpr int kStageCap2 = 32;     // ... when a CTA handles two groups (64 images)
+template <int NG> struct GridStage {
+    static constexpr int CAP = (NG == 1) ? kStageCap : kStageCap2;
+    static constexpr int BYTES = 3 * CAP * (kTabW * 4 + NG * kIL * 8) + 16;
+};
 
-// Adds staged samples [i0, i1) (indices into one staged list) to the accumulators of output row `row`.
+// Adds staged samples [i0, i1) (indices into one staged list) to the accumulators of output row `row`, for NG groups of
+// 32 images that share the staged table records (weights, row lookup): only the y row and the FMAs are per group.
 // Accumulators are kept as packed pairs for Blackwell's two-wide FP32 FMA (fma.rn.f32x2, SASS FFMA2):
 // ax[k] = (re of cell 2k, re of cell 2k+1), ay[k] = the imaginary parts; the weight pair of two adjacent cells is one
 // aligned register pair straight out of the 128-bit table load, so one FFMA2 updates two cells.
-template <int OFF>
-__device__ __forceinline__ void il_accumulate_smem(float2 (&ax)[kBandW / 2], float2 (&ay)[kBandW / 2],
+template <int OFF, int NG, int CAP>
+__device__ __forceinline__ void il_accumulate_smem(float2 (&ax)[NG][kBandW / 2], float2 (&ay)[NG][kBandW / 2],
                                                    const float* __restrict__ rec_s, const float2* __restrict__ y_s,
                                                    int row, int kmask, int i0, int i1) {
 #pragma unroll 4
@@ -314,31 +319,36 @@ __device__ __forceinline__ void il_accumulate_smem(float2 (&ax)[kBandW / 2], flo
         const float w0 = rec[j0];
         const float4 pa = *reinterpret_cast<const float4*>(rec + OFF);
         const float4 pb = *reinterpret_cast<const float4*>(rec + OFF + 4);
-        const float2 yv = y_s[i * kIL];
-        const float tx = w0 * yv.x, ty = w0 * yv.y;
-        const float2 txx = make_float2(tx, tx), tyy = make_float2(ty, ty);
-        ax[0] = __ffma2_rn(make_float2(pa.x, pa.y), txx, ax[0]); ay[0] = __ffma2_rn(make_float2(pa.x, pa.y), tyy, ay[0]);
-        ax[1] = __ffma2_rn(make_float2(pa.z, pa.w), txx, ax[1]); ay[1] = __ffma2_rn(make_float2(pa.z, pa.w), tyy, ay[1]);
-        ax[2] = __ffma2_rn(make_float2(pb.x, pb.y), txx, ax[2]); ay[2] = __ffma2_rn(make_float2(pb.x, pb.y), tyy, ay[2]);
-        ax[3] = __ffma2_rn(make_float2(pb.z, pb.w), txx, ax[3]); ay[3] = __ffma2_rn(make_float2(pb.z, pb.w), tyy, ay[3]);
+#pragma unroll
+        for (int gq = 0; gq < NG; ++gq) {
+            const float2 yv = y_s[(gq * 3 * CAP + i) * kIL];
+            const float tx = w0 * yv.x, ty = w0 * yv.y;
+            const float2 txx = make_float2(tx, tx), tyy = make_float2(ty, ty);
+            ax[gq][0] = __ffma2_rn(make_float2(pa.x, pa.y), txx, ax[gq][0]); ay[gq][0] = __ffma2_rn(make_float2(pa.x, pa.y), tyy, ay[gq][0]);
+            ax[gq][1] = __ffma2_rn(make_float2(pa.z, pa.w), txx, ax[gq][1]); ay[gq][1] = __ffma2_rn(make_float2(pa.z, pa.w), tyy, ay[gq][1]);
+            ax[gq][2] = __ffma2_rn(make_float2(pb.x, pb.y), txx, ax[gq][2]); ay[gq][2] = __ffma2_rn(make_float2(pb.x, pb.y), tyy, ay[gq][2]);
+            ax[gq][3] = __ffma2_rn(make_float2(pb.z, pb.w), txx, ax[gq][3]); ay[gq][3] = __ffma2_rn(make_float2(pb.z, pb.w), tyy, ay[gq][3]);
+        }
     }
 }
 
-// CTA = one work item (band, nrows rows).  The samples that touch the item's rows are, per list (this band class 0,
-// this band class 1, previous band class 0), ONE contiguous range of the V^H order (two at the periodic row seam), so
-// their table records (96 B each) and their y_il rows (256 B each) are contiguous in global memory: one elected
-// thread issues bulk copies of up to kStageCap samples per list into shared memory, all warps wait on the mbarrier,
-// and every warp then accumulates its own row from shared memory.  Global-memory latency is paid once per round per
-// CTA instead of once per warp per four samples.
+// CTA = one work item (band, nrows rows) x NG groups of 32 images (blockIdx.y = first group / NG, plus group0).  The
+// samples that touch the item's rows are, per list (this band class 0, this band class 1, previous band class 0), ONE
+// contiguous range of the V^H order (two at the periodic row seam), so their table records (96 B each) and their y_il
+// rows (256 B each per group) are contiguous in global memory: one elected thread issues bulk copies of up to CAP samples
+// per list into shared memory, all warps wait on the mbarrier, and every warp then accumulates its own row from shared
+// memory.  Global-memory latency is paid once per round per CTA instead of once per warp per four samples.
+template <int NG>
 __global__ void __launch_bounds__(256)
 gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const float2* __restrict__ y_il,
-                   float2* __restrict__ grid_il) {
+                   float2* __restrict__ grid_il, int group0) {
+    constexpr int CAP = GridStage<NG>::CAP;
     extern __shared__ __align__(128) unsigned char gsm[];
-    float2* y_s = reinterpret_cast<float2*>(gsm);                                           // [3][cap][32]
-    float* rec_s = reinterpret_cast<float*>(gsm + 3 * kStageCap * kIL * 8);                 // [3][cap][24]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(gsm + 3 * kStageCap * (kIL * 8 + kTabW * 4));
+    float2* y_s = reinterpret_cast<float2*>(gsm);                                           // [NG][3][CAP][32]
+    float* rec_s = reinterpret_cast<float*>(gsm + NG * 3 * CAP * kIL * 8);                  // [3][CAP][24]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(gsm + 3 * CAP * (NG * kIL * 8 + kTabW * 4));
     const IlItem it = items[blockIdx.x];
-    const int grp = blockIdx.y;
+    const int grp = group0 + blockIdx.y * NG;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nsplit = 8 / it.nrows, lsplit = 31 - __clz(nsplit);       // nsplit is a power of two
     const int row = it.r0 + (warp >> lsplit), part = warp & (nsplit - 1);
@@ -348,9 +358,11 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
     if (threadIdx.x == 0) mbar_init(bar, 1);
     __syncthreads();
     uint32_t phase = 0;
-    float2 ax[kBandW / 2], ay[kBandW / 2];
+    float2 ax[NG][kBandW / 2], ay[NG][kBandW / 2];
 #pragma unroll
-    for (int c = 0; c < kBandW / 2; ++c) { ax[c] = make_float2(0.f, 0.f); ay[c] = make_float2(0.f, 0.f); }
+    for (int gq = 0; gq < NG; ++gq)
+#pragma unroll
+        for (int c = 0; c < kBandW / 2; ++c) { ax[gq][c] = make_float2(0.f, 0.f); ay[gq][c] = make_float2(0.f, 0.f); }
     // stencil base rows that touch the item: r0-5 .. r0+nrows-1 (mod K0): one row segment, or two at the seam
     const int nseg = (it.r0 >= kJ - 1) ? 1 : 2;
 #pragma unroll 1
@@ -358,7 +370,6 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
         const int slo = (sg == 0) ? max(it.r0 - (kJ - 1), 0) : K0 - (kJ - 1) + it.r0;
         const int shi = (sg == 0) ? it.r0 + it.nrows - 1 : K0 - 1;
         const int shift = (sg == 0) ? 0 : K0;
-        // CTA ranges (cb_, ce_) and this warp's ranges (wb_, we_) per list
         int cbeg[3], cend[3], wbeg[3], wend[3];
         const int wlo = max(slo, row + shift - (kJ - 1)), whi = min(shi, row + shift);
         int rounds = 0;
@@ -369,7 +380,7 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
             cend[q] = __ldg(&s.rowptr[base + shi + 1]);
             if (wlo <= whi) { wbeg[q] = __ldg(&s.rowptr[base + wlo]); wend[q] = __ldg(&s.rowptr[base + whi + 1]); }
             else { wbeg[q] = 0; wend[q] = 0; }
-            rounds = max(rounds, (cend[q] - cbeg[q] + kStageCap - 1) / kStageCap);
+            rounds = max(rounds, (cend[q] - cbeg[q] + CAP - 1) / CAP);
         }
 #pragma unroll 1
         for (int k = 0; k < rounds; ++k) {
@@ -377,16 +388,19 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
                 uint32_t bytes = 0;
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
-                    const int c0 = cbeg[q] + k * kStageCap, n = min(kStageCap, cend[q] - c0);
-                    if (n > 0) bytes += (uint32_t)n * (kTabW * 4 + kIL * 8);
+                    const int c0 = cbeg[q] + k * CAP, n = min(CAP, cend[q] - c0);
+                    if (n > 0) bytes += (uint32_t)n * (kTabW * 4 + NG * kIL * 8);
                 }
                 mbar_expect_tx(bar, bytes);
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
-                    const int c0 = cbeg[q] + k * kStageCap, n = min(kStageCap, cend[q] - c0);
+                    const int c0 = cbeg[q] + k * CAP, n = min(CAP, cend[q] - c0);
                     if (n > 0) {
-                        bulk_g2s(rec_s + q * kStageCap * kTabW, s.wtab + (int64_t)c0 * kTabW, (uint32_t)n * kTabW * 4, bar);
-                        bulk_g2s(y_s + q * kStageCap * kIL, Y + (int64_t)c0 * kIL, (uint32_t)n * kIL * 8, bar);
+                        bulk_g2s(rec_s + q * CAP * kTabW, s.wtab + (int64_t)c0 * kTabW, (uint32_t)n * kTabW * 4, bar);
+#pragma unroll
+                        for (int gq = 0; gq < NG; ++gq)
+                            bulk_g2s(y_s + (gq * 3 + q) * CAP * kIL, Y + ((int64_t)gq * g.M + c0) * kIL,
+                                     (uint32_t)n * kIL * 8, bar);
                     }
                 }
             }
@@ -394,37 +408,43 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
             phase ^= 1;
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
-                const int c0 = cbeg[q] + k * kStageCap, c1 = min(c0 + kStageCap, cend[q]);
+                const int c0 = cbeg[q] + k * CAP, c1 = min(c0 + CAP, cend[q]);
                 const int x0 = max(wbeg[q], c0), x1 = min(wend[q], c1);       // my row's samples within the staged chunk
                 if (x1 > x0) {
                     const int n = x1 - x0;
                     const int i0 = x0 - c0 + ((n * part) >> lsplit), i1 = x0 - c0 + ((n * (part + 1)) >> lsplit);
-                    if (q == 2) il_accumulate_smem<16>(ax, ay, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
-                    else        il_accumulate_smem<8>(ax, ay, rec_s + q * kStageCap * kTabW, y_s + q * kStageCap * kIL + lane, row, K0 - 1, i0, i1);
+                    if (q == 2) il_accumulate_smem<16, NG, CAP>(ax, ay, rec_s + q * CAP * kTabW, y_s + q * CAP * kIL + lane, row, K0 - 1, i0, i1);
+                    else        il_accumulate_smem<8, NG, CAP>(ax, ay, rec_s + q * CAP * kTabW, y_s + q * CAP * kIL + lane, row, K0 - 1, i0, i1);
                 }
             }
             __syncthreads();      // every warp is done with the staged chunk before the next round overwrites it
         }
     }
-    float2 acc[kBandW];
 #pragma unroll
-    for (int c = 0; c < kBandW / 2; ++c) {
-        acc[2 * c] = make_float2(ax[c].x, ay[c].x);
-        acc[2 * c + 1] = make_float2(ax[c].y, ay[c].y);
+    for (int gq = 0; gq < NG; ++gq) {
+        float2 acc[kBandW];
+#pragma unroll
+        for (int c = 0; c < kBandW / 2; ++c) {
+            acc[2 * c] = make_float2(ax[gq][c].x, ay[gq][c].x);
+            acc[2 * c + 1] = make_float2(ax[gq][c].y, ay[gq][c].y);
+        }
+        if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row (staging area reused)
+            float2* red = y_s;  // [8][kBandW][32]
+            if (gq > 0) __syncthreads();
+#pragma unroll
+            for (int c = 0; c < kBandW; ++c) red[(warp * kBandW + c) * kIL + lane] = acc[c];
+            __syncthreads();
+            if (part == 0)
+                for (int q = 1; q < nsplit; ++q)
+#pragma unroll
+                    for (int c = 0; c < kBandW; ++c) acc[c] = cadd(acc[c], red[((warp + q) * kBandW + c) * kIL + lane]);
+        }
+        if (part == 0) {
+            float2* __restrict__ dst = grid_il + (((int64_t)(grp + gq) * K0 + row) * K1 + it.cb * kBandW) * kIL + lane;
+#pragma unroll
+            for (int c = 0; c < kBandW; ++c) dst[c * kIL] = acc[c];
+        }
     }
-    if (nsplit > 1) {       // fixed-order sum of the partial accumulators of one row (staging area reused)
-        float2* red = y_s;  // [8][kBandW][32]
-#pragma unroll
-        for (int c = 0; c < kBandW; ++c) red[(warp * kBandW + c) * kIL + lane] = acc[c];
-        __syncthreads();
-        if (part != 0) return;
-        for (int q = 1; q < nsplit; ++q)
-#pragma unroll
-            for (int c = 0; c < kBandW; ++c) acc[c] = cadd(acc[c], red[((warp + q) * kBandW + c) * kIL + lane]);
-    }
-    float2* __restrict__ dst = grid_il + (((int64_t)grp * K0 + row) * K1 + it.cb * kBandW) * kIL + lane;
-#pragma unroll
-    for (int c = 0; c < kBandW; ++c) dst[c * kIL] = acc[c];
 }
 
 // x[n] = sum_b img[b][n]  is done by coil_sum_kernel (solver.cuh).

@@ -187,7 +187,8 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(interp_tiled_3d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kInterp3dSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(gridding_il_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGridSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(gridding_il_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<1>::BYTES)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(gridding_il_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<2>::BYTES)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     return cudaSuccess;
 }
@@ -512,11 +513,20 @@ static int run_gridding_il(nufft_plan_t p, int batch, const float2* y_il, float2
         CU_TRY(cudaMemsetAsync(grid, 0, (size_t)il_groups(batch) * kIL * p->cells * sizeof(float2), st));
         return NUFFT_OK;
     }
-    const dim3 blocks((unsigned)p->n_il_items, (unsigned)il_groups(batch));
+    const int ng = il_groups(batch);
     ProfScope ps(p, "gridding", st);
-    gridding_il_kernel<<<blocks, 256, kGridSmemBytes, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid);
+    // CTAs handle two groups (64 images) at a time: the staged weight records and row lookups are shared
+    if (ng >= 2) {
+        const dim3 blocks((unsigned)p->n_il_items, (unsigned)(ng / 2));
+        gridding_il_kernel<2><<<blocks, 256, GridStage<2>::BYTES, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid, 0);
+        p->launches++;
+    }
+    if (ng & 1) {
+        const dim3 blocks((unsigned)p->n_il_items, 1u);
+        gridding_il_kernel<1><<<blocks, 256, GridStage<1>::BYTES, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid, ng - 1);
+        p->launches++;
+    }
     CU_TRY(cudaGetLastError());
-    p->launches++;
     return NUFFT_OK;
 }
 
