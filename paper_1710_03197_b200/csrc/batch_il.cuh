@@ -297,7 +297,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 }
 
 constexpr int kStageCap = 48;      // samples per list per staging round (one group per CTA)
-constexpr int kStageCap2 = 32;     // ... when a CTA handles two groups (64 images)
+constexpr int kStageCap2 = 40;     // ... when a CTA handles two groups (64 images)
 template <int NG> struct GridStage {
     static constexpr int CAP = (NG == 1) ? kStageCap : kStageCap2;
     static constexpr int BYTES = 3 * CAP * (kTabW * 4 + NG * kIL * 8) + 16;
