@@ -13,7 +13,7 @@
  *   L1TV-OLS     split Bregman, eqs.(13)-(22)                       PAPER.md:158-198 (R13-R18)
  *
  * Conventions (all binding):
- *   - d in {2,3}.  Image x is C-order [batch][N0][N1]([N2]) complex64; image index n_a sits at position
+ *   - d in {1,2,3}.  Image x is C-order [batch][N0]([N1]([N2])) complex64; image index n_a sits at position
  *     n_a - N_a/2 (R4).  Samples y are [batch][M] complex64 in the caller's sample order.  om is [M][d] float64,
  *     radians per image sample, axis a of om pairs with image axis a; values outside [-pi,pi) are wrapped.
  *   - forward sign e^{-i om.(n - N/2)}; adjoint is the exact conjugate transpose (no 1/prod(K) factor, R5).
@@ -28,7 +28,8 @@
  *   - transform calls are asynchronous: they enqueue kernels on `stream` and return.  A plan owns one workspace:
  *     use one stream at a time per plan.  Distinct plans are independent.
  *   - outputs are overwritten, never accumulated into.  In-place (x_in == x_out) is allowed for selfadjoint.
- *   - supported: d in {2,3}; Jd[a] == 6; Kd[a] == 2*Nd[a]; Kd[a] in {32,64,128,256,512,1024};
+ *   - supported: d in {1,2,3} (1-D: "1D signals"; planar path, atomic V^H only -- adjoint_mode = 1 is
+ *     refused); Jd[a] == 6; Kd[a] == 2*Nd[a]; Kd[a] in {32,64,128,256,512,1024};
  *     1 <= batch <= max_batch.  Anything else -> NUFFT_EINVAL (there is no slow path and no CPU fallback).
  */
 #ifndef NUFFT_B200_H

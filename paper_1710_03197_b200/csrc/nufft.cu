@@ -250,7 +250,10 @@ static RowPassParams row_params(nufft_plan_t p, int batch, const float2* img_in,
     auto sc = [&](int a) -> const float* { return p->unit_scale ? p->d_ones : (p->inv_scale ? p->d_sinv[a] : p->d_scale[a]); };
     r.s_line = sc(d - 1);
     r.tw = p->d_tw[d - 1];
-    if (d == 2) {
+    if (d == 1) {          // one line per image: no outer axes
+        r.s_outer0 = p->d_ones; r.s_outer1 = nullptr;
+        r.n_outer0 = 1; r.n_outer1 = 1; r.k_outer0 = 1; r.k_outer1 = 1;
+    } else if (d == 2) {
         r.s_outer0 = sc(0); r.s_outer1 = nullptr;
         r.n_outer0 = p->N[0]; r.n_outer1 = 1; r.k_outer0 = p->K[0]; r.k_outer1 = 1;
     } else {
@@ -269,6 +272,7 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
     RowPassParams r = row_params(p, batch, x, nullptr, grid, coil, same_image);
     { ProfScope ps(p, "fft_rows_fwd", st); NU_TRY(dispatch_rows(p->K[d - 1], false, r, st)); }
     p->launches++;
+    if (d == 1) return NUFFT_OK;
     if (d == 2) {
         ColPassParams c{};
         c.grid = grid; c.tw = p->d_tw[0];
@@ -298,7 +302,14 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
 // a5 + a6: x = S^H F^H grid  (grid destroyed; coil != nullptr: x_b = conj(c_b) . S^H F^H grid_b)
 static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
     const int d = p->d;
-    if (d == 2) {
+    if (d == 1) {
+        // the Toeplitz spectrum multiply normally rides on the first adjoint column pass; 1-D has none
+        if (p->cur_mult) {
+            spectrum_mul_kernel<<<(int)std::max<int64_t>(1, std::min<int64_t>((p->cells * batch + 255) / 256, 148 * 8)), 256, 0, st>>>(grid, p->cur_mult, p->cells, batch);
+            CU_TRY(cudaGetLastError());
+            p->launches++;
+        }
+    } else if (d == 2) {
         ColPassParams c{};
         c.grid = grid; c.tw = p->d_tw[0];
         c.batch_stride = p->cells; c.outer_stride = 0; c.line_stride = p->K[1];
@@ -354,7 +365,8 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
         return NUFFT_OK;
     }
     const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
-    if (p->d == 2) interp_direct_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
+    if (p->d == 1) interp_direct_kernel<1><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
+    else if (p->d == 2) interp_direct_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     else           interp_direct_kernel<3><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     CU_TRY(cudaGetLastError());
     p->launches++;
@@ -377,7 +389,10 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
         NU_TRY(dev_alloc((void**)&p->d_slabs, (size_t)p->max_batch * slab_stride * sizeof(float2), &p->bytes_work));
     if (!det) { ProfScope ps(p, "grid_zero", st); CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st)); }
     ProfScope ps(p, "gridding", st);
-    if (p->d == 2) {
+    if (p->d == 1) {       // 1-D: one thread per sample, one vector atomic per stencil point (the grid was zeroed above)
+        const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
+        gridding_atomic_kernel<1><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), y, grid, p->poly);
+    } else if (p->d == 2) {
         const dim3 blocks((unsigned)((p->n_items + kGrid2dWarps - 1) / kGrid2dWarps), (unsigned)batch);
         const size_t sm = smem_grid2d(p);
         if (det) gridding_tiled_2d_kernel<true><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly);
@@ -683,10 +698,10 @@ static int plan_build(nufft_plan_t p, const double* om) {
         NU_TRY(dev_upload(&p->d_ones, std::vector<float>((size_t)nmax, 1.0f), &p->bytes_plan));
     }
     // tiles
-    const int def2[3] = {16, 32, 1}, def3[3] = {8, 8, 16};
+    const int def1[3] = {32, 1, 1}, def2[3] = {16, 32, 1}, def3[3] = {8, 8, 16};
     for (int a = 0; a < 3; ++a) {
         int t = (a < d) ? p->opts.tile[a] : 1;
-        if (a < d && t <= 0) t = std::min((d == 2) ? def2[a] : def3[a], p->K[a]);
+        if (a < d && t <= 0) t = std::min((d == 1) ? def1[a] : ((d == 2) ? def2[a] : def3[a]), p->K[a]);
         if (a < d && (t < 8 || t > p->K[a] || (p->K[a] % t) != 0 || (t & 1))) return NUFFT_EINVAL;
         p->tile[a] = t;
         p->ntile[a] = (a < d) ? p->K[a] / t : 1;
@@ -801,11 +816,12 @@ static int plan_build(nufft_plan_t p, const double* om) {
 extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int* Jd, int64_t M, const double* om,
                           int max_batch, const nufft_opts* opts, nufft_plan_t* out) {
     if (out) *out = nullptr;
-    if (!out || !Nd || !Kd || !Jd || (d != 2 && d != 3) || M < 0 || (M > 0 && !om) || max_batch < 1) return NUFFT_EINVAL;
+    if (!out || !Nd || !Kd || !Jd || (d < 1 || d > 3) || M < 0 || (M > 0 && !om) || max_batch < 1) return NUFFT_EINVAL;
     if (M > (int64_t)0x7fffffff) return NUFFT_EINVAL;
     for (int a = 0; a < d; ++a) {
         if (Jd[a] != kJ || !supported_K(Kd[a]) || Kd[a] != 2 * Nd[a]) return NUFFT_EINVAL;
     }
+    if (d == 1 && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;      // 1-D V^H is the atomic kernel only
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
                  opts->interp_mode > 1 || opts->batch_layout < 0 || opts->batch_layout > 1))
         return NUFFT_EINVAL;

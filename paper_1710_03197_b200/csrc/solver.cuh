@@ -254,6 +254,14 @@ weight_mul_kernel(float2* __restrict__ out, const float2* __restrict__ y, const 
         out[i] = cscale(y[i], __ldg(&w[i % M].x));
 }
 
+// grid[b][i] *= spec[i]   (1-D Toeplitz: there is no adjoint column pass to carry the spectrum multiply)
+__global__ void __launch_bounds__(256)
+spectrum_mul_kernel(float2* __restrict__ grid, const float2* __restrict__ spec, int64_t cells, int batch) {
+    const int64_t n = cells * batch;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        grid[i] = cmul(grid[i], __ldg(&spec[i % cells]));
+}
+
 // ---- Toeplitz point-spread function (reading R22) ----
 // T2 is the adjoint NUFFT of the weights onto the 2N image (pixel n <-> displacement d = n - N).  Zero the d = -N
 // hyperplanes (pixel 0 of every axis), which a linear convolution of two length-N supports never uses.
@@ -261,7 +269,7 @@ __global__ void __launch_bounds__(256) psf_zero_planes_kernel(float2* __restrict
     const int64_t n = (int64_t)K0 * K1 * K2;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const int c2 = (int)(i % K2), c1 = (int)((i / K2) % K1), c0 = (int)(i / ((int64_t)K1 * K2));
-        if (c0 == 0 || c1 == 0 || (K2 > 1 && c2 == 0)) T[i] = make_float2(0.f, 0.f);
+        if (c0 == 0 || (K1 > 1 && c1 == 0) || (K2 > 1 && c2 == 0)) T[i] = make_float2(0.f, 0.f);
     }
 }
 // T^[k] = sum_d T[d] e^{-2 pi i k d / K} = (-1)^{sum k_a} FFT(T2)[k]   (d = n - K/2 per axis), times `scale` = 1/prod(K):

@@ -42,7 +42,15 @@ interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, 
     for (int a = 0; a < D; ++a) kb_weights(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
     const float2* __restrict__ G = grid + (int64_t)b * g.cells;
     float2 acc = make_float2(0.f, 0.f);
-    if (D == 2) {
+    if (D == 1) {
+        const int K0 = g.K[0];
+#pragma unroll
+        for (int j0 = 0; j0 < kJ; ++j0) {
+            const float2 v = __ldg(&G[(k0[0] + j0) & (K0 - 1)]);
+            acc.x = fmaf(w[0][j0], v.x, acc.x);
+            acc.y = fmaf(w[0][j0], v.y, acc.y);
+        }
+    } else if (D == 2) {
         const int K0 = g.K[0], K1 = g.K[1];
 #pragma unroll
         for (int j0 = 0; j0 < kJ; ++j0) {
@@ -101,7 +109,11 @@ gridding_atomic_kernel(SampleData s, GridGeom g, const float2* __restrict__ y, f
     for (int a = 0; a < D; ++a) kb_weights(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
     const float2 yv = __ldg(&y[(int64_t)b * g.M + __ldg(&s.perm[i])]);
     float2* __restrict__ G = grid + (int64_t)b * g.cells;
-    if (D == 2) {
+    if (D == 1) {
+        const int K0 = g.K[0];
+#pragma unroll
+        for (int j0 = 0; j0 < kJ; ++j0) atomicAdd(&G[(k0[0] + j0) & (K0 - 1)], cscale(yv, w[0][j0]));
+    } else if (D == 2) {
         const int K0 = g.K[0], K1 = g.K[1];
 #pragma unroll
         for (int j0 = 0; j0 < kJ; ++j0) {

@@ -178,3 +178,35 @@ def test_cg_kspace(ci, scale):
         else:
             assert rel(xg, xo) < 1e-4, (niter, rel(xg, xo))
     p.destroy()
+
+
+def test_one_dimensional_transforms_and_solvers():
+    """d = 1 ("1D signals in the time-domain"): forward / adjoint / A^H A, batch, density weights, Toeplitz,
+    image-space and k-space CG against the oracle."""
+    rng = np.random.default_rng(31)
+    for N, M, B in ((64, 500, 1), (512, 4001, 5), (16, 77, 3)):
+        Nd, Kd, Jd = (N,), (2 * N,), (6,)
+        om = rng.uniform(-np.pi, np.pi, (M, 1))
+        om[:5, 0] = [-np.pi, 0.0, 2 * np.pi * 3 / (2 * N), np.pi - 1e-9, 7.0]      # seam, grid points, wrapped
+        cfg = dict(Nd=Nd, Kd=Kd, Jd=Jd, om=om)
+        p = make_plan(cfg, max_batch=B)
+        x = wl.image_gaussian(Nd, batch=B)
+        y = wl.data_gaussian(M, batch=B)
+        yg, xg, sg = host(p.forward(dev(x))), host(p.adjoint(dev(y))), host(p.selfadjoint(dev(x)))
+        for b in range(B):
+            yo = orc.forward(x[b].astype(np.complex128), om, Nd, Kd, Jd)
+            assert rel(yg[b], yo) < TOL
+            assert rel(xg[b], orc.adjoint(y[b].astype(np.complex128), om, Nd, Kd, Jd)) < TOL
+            assert rel(sg[b], orc.adjoint(yo, om, Nd, Kd, Jd)) < TOL
+        assert rel(host(p.density_weights(1)).real, nxt.density_weights(om, Nd, Kd, Jd, 1)) < TOL
+        if 4 * N <= 1024:
+            p.toeplitz_build()
+            That, _ = nxt.toeplitz_kernel(om, Nd, Kd, Jd)
+            got = host(p.selfadjoint_toeplitz(dev(x)))
+            assert rel(got[0], nxt.selfadjoint_toeplitz(x[0].astype(np.complex128), That, Nd)) < TOL
+        AHy = orc.adjoint(y[0].astype(np.complex128), om, Nd, Kd, Jd)
+        xo, _ = sol.cg(lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd), AHy, 3)
+        assert rel(host(p.solve_cg(dev(y[0]), 3)), xo) < 1e-4
+        xk, _ = nxt.cg_kspace(y[0].astype(np.complex128), om, Nd, Kd, Jd, 2)
+        assert rel(host(p.solve_cg_kspace(dev(y[0]), 2)), xk) < 1e-4
+        p.destroy()
