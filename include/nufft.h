@@ -55,13 +55,15 @@ typedef enum {
 
 /* Options.  Zero-initialise or call nufft_default_opts first. */
 typedef struct {
-    int coef_mode;      /* 0 = interpolation weights recomputed on the fly from a piecewise polynomial fit of the
-                               Kaiser-Bessel kernel (12 + 4 B per sample of plan data in 2-D);
-                           1 = weights read from a per-sample separable table (4 + 4 d J bytes per sample)       */
-    int adjoint_mode;   /* 0 = V^H by tile-sorted shared-memory accumulation, one vector-atomic flush per tile
-                               (summation order across tiles free: reproducible to rounding only);
+    int coef_mode;      /* must be 0: the library chooses per kernel from measured cost: planar V / V^H
+                               and interleaved V recompute the weights on the fly from a piecewise polynomial fit of
+                               the Kaiser-Bessel kernel (4 + 4 d bytes of plan data per sample); interleaved V^H reads a
+                               float64-built separable table (96 B per sample).  Any other value -> NUFFT_EINVAL      */
+    int adjoint_mode;   /* planar path: 0 = V^H by tile-sorted shared-memory accumulation, one vector-atomic flush per
+                               tile (summation order across tiles free: reproducible to rounding only);
                            1 = deterministic: tiles flushed to private slabs and summed in fixed order
-                               (bit-reproducible run to run)                                                      */
+                               (bit-reproducible run to run).  The interleaved path (batch >= 16) is always
+                               deterministic (gather form, fixed order)                                             */
     int interp_mode;    /* 0 = library default: 3-D planar V stages the padded tile of a work item in shared memory
                                (half-warp per sample), 2-D planar V gathers through L1/L2; 1 = always direct gather */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
