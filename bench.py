@@ -492,6 +492,27 @@ def extra_legs(nb, torch, peak, args):
         "toeplitz_selfadjoint_coils_ms": toep_ms, "l1tv_ols_20it_toeplitz_ms": tv_toep_ms,
         "density_weights_4it_ms": dcf_ms,
         "note": "cfg5 problem; Toeplitz: crop(F^H(T^ . F(pad c_i x))) summed over 32 coils, T^ built once per plan"}
+    # the same 20 iterations with the inner CG steps replayed as CUDA graphs (opts.use_graphs; non-default stream)
+    pg = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=nc, use_graphs=1)
+    pg.set_coils(c)
+    pg.toeplitz_build()
+    pg.toeplitz_enable(True)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        xs2 = pg.solve_l1tv_ols(y5, 1.0, 0.02, 1, 1, 3, use_coils=True)
+        evs = []
+        for _ in range(3):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(side)
+            pg.solve_l1tv_ols(y5, 1.0, 0.02, 4, 5, 3, use_coils=True, x=xs2)
+            b.record(side)
+            evs.append((a, b))
+    side.synchronize()
+    torch.cuda.current_stream().wait_stream(side)
+    out["next_rows"]["l1tv_ols_20it_toeplitz_graph_ms"] = float(np.median([a.elapsed_time(b) for a, b in evs]))
+    pg.destroy()
     out["cfg5_2d_multicoil_l1tv"] = {
         "workload": "Nd=256^2 Kd=512^2 M=65536 radial 128x512, 32 coils", "forward_coils_ms": fwc_ms,
         "adjoint_coils_ms": adc_ms, "selfadjoint_coils_ms": sac_ms, "l1tv_ols_20it_ms": tv_ms,
