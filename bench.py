@@ -354,7 +354,7 @@ def run_ours(args):
             "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
             "config": {"workload": WORKLOAD, "batch": B, "pairs_per_step": B, "l2": "flushed between steps (256 MiB memset)",
                        "parallelism": "replicas x%d" % world, "adjoint_mode": 0,
-                       "batch_layout": "interleaved [group][K0][K1][32] (batch >= 16)" if B >= 16 else "planar"},
+                       "batch_layout": "interleaved [group][K0][K1][32] (batch >= 12)" if B >= 12 else "planar"},
             "clocks": clocks,
             "e2e": {"value": world * B / (e2e_ms / K_steps * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": int(x_host.numel() * 8), "d2h_bytes_per_step": int(xo_host.numel() * 8),

@@ -62,7 +62,7 @@ typedef struct {
     int adjoint_mode;   /* planar path: 0 = V^H by tile-sorted shared-memory accumulation, one vector-atomic flush per
                                tile (summation order across tiles free: reproducible to rounding only);
                            1 = deterministic: tiles flushed to private slabs and summed in fixed order
-                               (bit-reproducible run to run).  The interleaved path (batch >= 16) is always
+                               (bit-reproducible run to run).  The interleaved path (batch >= 12) is always
                                deterministic (gather form, fixed order)                                             */
     int interp_mode;    /* 0 = library default: 3-D planar V stages the padded tile of a work item in shared memory
                                (half-warp per sample), 2-D planar V gathers through L1/L2; 1 = always direct gather */
@@ -73,10 +73,10 @@ typedef struct {
                                first iteration of a call runs eagerly, the graph is cached in the plan.  Needs a
                                non-default stream (the legacy stream cannot capture: eager launches are used).  Default 0 */
     int batch_layout;   /* workspace layout of batched 2-D transforms (PAPER.md:52 batch mode, :251-258 coils):
-                           0 = auto: calls with batch >= 16 use the batch-interleaved grid [group][K0][K1][32]
+                           0 = auto: calls with batch >= 12 (the measured crossover) use the batch-interleaved grid [group][K0][K1][32]
                                (lanes = images; V^H in gather form with register accumulators, deterministic),
                                smaller batches and 3-D use the planar grid [batch][K0][K1]([K2]);
-                           1 = always planar                                                                      */
+                           1 = always planar;  2 = interleaved for every batch >= 2 (for measuring the crossover)  */
 } nufft_opts;
 
 int nufft_default_opts(nufft_opts *o);

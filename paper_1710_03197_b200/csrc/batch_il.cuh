@@ -1,4 +1,4 @@
-// batch_il.cuh -- the batch-interleaved 2-D path (steps a1..a6 and a8 of SURVEY.md 8(a) for batches >= 16 images that
+// batch_il.cuh -- the batch-interleaved 2-D path (steps a1..a6 and a8 of SURVEY.md 8(a) for batches >= 12 images that
 // share one trajectory: the paper's batch mode PAPER.md:52 and the multi-coil operator PAPER.md:251-258).
 //
 // Why a second layout.  At J = 6 every sample touches 36 complex64 grid cells; with a planar grid and one thread per

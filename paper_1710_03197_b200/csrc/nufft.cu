@@ -81,6 +81,7 @@ struct nufft_plan_s {
     int64_t launches = 0;
     // batch-interleaved 2-D path (batch_il.cuh): cell-sorted plan data, V^H weight table, row pointers, work items
     bool il_ok = false;
+    int il_min_batch = 12;
     int batch_pad = 1;              // max_batch rounded up to whole groups of 32 when il_ok
     uint32_t* d_il_kpack = nullptr;
     float* d_il_delta = nullptr;
@@ -420,7 +421,8 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
 // ------------------------------------------------------------------------------------------------------------
 // batch-interleaved 2-D path (batch_il.cuh)
 // ------------------------------------------------------------------------------------------------------------
-static bool use_il(nufft_plan_t p, int batch) { return p->il_ok && batch >= 16; }
+static constexpr int kIlMinBatch = 12;    // measured crossover of the planar and interleaved paths
+static bool use_il(nufft_plan_t p, int batch) { return p->il_ok && batch >= p->il_min_batch; }
 static int il_groups(int batch) { return (batch + kIL - 1) / kIL; }
 
 template <int K> static void launch_il_rows(bool adj, const IlRowParams& p, int blocks, cudaStream_t st) {
@@ -823,7 +825,7 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     }
     if (d == 1 && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;      // 1-D V^H is the atomic kernel only
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
-                 opts->interp_mode > 1 || opts->batch_layout < 0 || opts->batch_layout > 1))
+                 opts->interp_mode > 1 || opts->batch_layout < 0 || opts->batch_layout > 2))
         return NUFFT_EINVAL;
     static cudaError_t cfg = configure_all();
     if (cfg != cudaSuccess) { g_last_cuda_error = (int)cfg; return NUFFT_ECUDA; }
@@ -833,7 +835,8 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     p->M = M;
     p->max_batch = max_batch;
     if (opts) p->opts = *opts;
-    p->il_ok = (d == 2) && max_batch >= 16 && p->opts.batch_layout == 0 && Kd[1] >= 2 * kBandW;
+    p->il_min_batch = (p->opts.batch_layout == 2) ? 2 : kIlMinBatch;
+    p->il_ok = (d == 2) && max_batch >= p->il_min_batch && p->opts.batch_layout != 1 && Kd[1] >= 2 * kBandW;
     p->batch_pad = p->il_ok ? ((max_batch + kIL - 1) / kIL) * kIL : max_batch;
     p->nimg = 1; p->cells = 1;
     for (int a = 0; a < d; ++a) {
