@@ -103,7 +103,11 @@ int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c6
  * pageable memory works but serialises the copies.  The batch is cut into chunks (32 images on the interleaved path);
  * chunk c+1 is copied in on an internal copy stream while the kernels of chunk c run on `stream` and chunk c-1 is
  * copied back on a second copy stream; `stream` is made to wait for the last copy back before the call's work counts
- * as finished.  Device staging buffers (2 x 2 chunks) belong to the plan. */
+ * as finished.  Device staging buffers (2 x 2 chunks) belong to the plan.
+ * nufft_host_input_ready(p, 1): the caller promises that the host INPUT of every later *_host call is final when the call
+ * is made (it is not the target of work still pending on `stream`); the copy in then need not wait for `stream` and may
+ * overlap the copy back of the previous call.  Outputs stay stream-ordered.  Default 0 (strict stream order). */
+int nufft_host_input_ready(nufft_plan_t p, int on);
 int nufft_forward_host(nufft_plan_t p, int batch, const nufft_c64 *x_host, nufft_c64 *y_host, void *stream);
 int nufft_adjoint_host(nufft_plan_t p, int batch, const nufft_c64 *y_host, nufft_c64 *x_host, void *stream);
 int nufft_selfadjoint_host(nufft_plan_t p, int batch, const nufft_c64 *x_in_host, nufft_c64 *x_out_host, void *stream);

@@ -16,7 +16,7 @@ _I64P = _c.POINTER(_c.c_int64)
 
 EXPORTED_SYMBOLS = [
     "nufft_default_opts", "nufft_plan", "nufft_forward", "nufft_adjoint", "nufft_selfadjoint",
-    "nufft_forward_host", "nufft_adjoint_host", "nufft_selfadjoint_host",
+    "nufft_forward_host", "nufft_adjoint_host", "nufft_selfadjoint_host", "nufft_host_input_ready",
     "nufft_density_weights", "nufft_adjoint_dcf", "nufft_toeplitz_build", "nufft_toeplitz_enable",
     "nufft_selfadjoint_toeplitz", "nufft_selfadjoint_toeplitz_coils", "nufft_solve_l1tv_lad", "nufft_solve_cg_kspace",
     "nufft_stage_scale_fft", "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale",
@@ -62,6 +62,7 @@ def lib():
                  "nufft_selfadjoint_host", "nufft_stage_scale_fft",
                  "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale"):
         getattr(L, name).argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR]
+    L.nufft_host_input_ready.argtypes = [_PLAN, _c.c_int]
     L.nufft_density_weights.argtypes = [_PLAN, _c.c_int, _PTR, _PTR]
     L.nufft_adjoint_dcf.argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR, _PTR]
     L.nufft_toeplitz_build.argtypes = [_PLAN, _PTR, _PTR]
@@ -373,6 +374,9 @@ class NufftPlan:
     def _new_host(self, *shape):
         import torch
         return torch.empty(shape, dtype=torch.complex64, pin_memory=True)
+
+    def host_input_ready(self, on=True):
+        _check(lib().nufft_host_input_ready(self._h, int(bool(on))), "nufft_host_input_ready")
 
     def forward_host(self, x_host, y_host=None):
         """x_host: pinned CPU complex64 [b][Nd] -> y_host pinned CPU [b][M].  Asynchronous on the current stream."""

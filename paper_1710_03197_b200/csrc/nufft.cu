@@ -109,6 +109,8 @@ struct nufft_plan_s {
     int cg_iter_launches = 0;
     // host-buffer pipeline (nufft_*_host): copy streams, events, double-buffered device staging, lazy
     bool hp_ready = false;
+    bool hp_input_ready = false;    // nufft_host_input_ready
+    bool hp_used[2] = {false, false};
     int hp_chunk = 1;
     cudaStream_t hp_h2d = nullptr, hp_d2h = nullptr;
     cudaEvent_t hp_in[2] = {nullptr, nullptr}, hp_cmp[2] = {nullptr, nullptr}, hp_out[2] = {nullptr, nullptr}, hp_start = nullptr;
@@ -1025,12 +1027,15 @@ static int host_pipeline(nufft_plan_t p, int kind, int batch, const nufft_c64* i
     const int64_t n_in = (kind == 1) ? p->M : p->nimg, n_out = (kind == 0) ? p->M : p->nimg;
     const int CH = p->hp_chunk;
     CU_TRY(cudaEventRecord(p->hp_start, st));
-    CU_TRY(cudaStreamWaitEvent(p->hp_h2d, p->hp_start, 0));
+    // strict mode: the copies in are ordered after everything already enqueued on the caller's stream.  With
+    // nufft_host_input_ready(p, 1) the caller promises that the host input is final when the call is made, so the
+    // first copy in may overlap the copy back of the previous call (only the staging buffers are waited for).
+    if (!p->hp_input_ready) CU_TRY(cudaStreamWaitEvent(p->hp_h2d, p->hp_start, 0));
     CU_TRY(cudaStreamWaitEvent(p->hp_d2h, p->hp_start, 0));
     int c = 0;
     for (int b0 = 0; b0 < batch; b0 += CH, ++c) {
         const int n = std::min(CH, batch - b0), buf = c & 1;
-        if (c >= 2) CU_TRY(cudaStreamWaitEvent(p->hp_h2d, p->hp_cmp[buf], 0));      // kernels of chunk c-2 have read din[buf]
+        if (c >= 2 || p->hp_used[buf]) CU_TRY(cudaStreamWaitEvent(p->hp_h2d, p->hp_cmp[buf], 0));   // last reader of din[buf]
         if (n_in > 0)
             CU_TRY(cudaMemcpyAsync(p->hp_din[buf], (const float2*)in_host + (int64_t)b0 * n_in,
                                    (size_t)n * n_in * sizeof(float2), cudaMemcpyHostToDevice, p->hp_h2d));
@@ -1043,6 +1048,7 @@ static int host_pipeline(nufft_plan_t p, int kind, int batch, const nufft_c64* i
         else rc = nufft_selfadjoint(p, n, (const nufft_c64*)p->hp_din[buf], (nufft_c64*)p->hp_dout[buf], st);
         NU_TRY(rc);
         CU_TRY(cudaEventRecord(p->hp_cmp[buf], st));
+        p->hp_used[buf] = true;
         CU_TRY(cudaStreamWaitEvent(p->hp_d2h, p->hp_cmp[buf], 0));
         if (n_out > 0)
             CU_TRY(cudaMemcpyAsync((float2*)out_host + (int64_t)b0 * n_out, p->hp_dout[buf],
@@ -1055,6 +1061,11 @@ static int host_pipeline(nufft_plan_t p, int kind, int batch, const nufft_c64* i
     return NUFFT_OK;
 }
 
+extern "C" int nufft_host_input_ready(nufft_plan_t p, int on) {
+    if (!p) return NUFFT_EINVAL;
+    p->hp_input_ready = on != 0;
+    return NUFFT_OK;
+}
 extern "C" int nufft_forward_host(nufft_plan_t p, int batch, const nufft_c64* x_host, nufft_c64* y_host, void* stream) {
     if (bad_batch(p, batch) || !x_host || (!y_host && p->M > 0)) return NUFFT_EINVAL;
     return host_pipeline(p, 0, batch, x_host, y_host, (cudaStream_t)stream);

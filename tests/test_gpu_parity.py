@@ -437,6 +437,13 @@ def test_host_buffer_pipeline_matches_device_calls():
         assert rel(sx.numpy(), host(p.selfadjoint(dev(x)))) < 2e-6
     yo = orc.forward(x[37].astype(np.complex128), cfg["om"], cfg["Nd"], cfg["Kd"], cfg["Jd"])
     assert rel(fy.numpy()[37], yo) < TOL
+    # relaxed input ordering (nufft_host_input_ready): back-to-back calls whose copies in overlap the previous copies back
+    p.host_input_ready(True)
+    ref = host(p.selfadjoint(dev(x)))
+    outs = [p.selfadjoint_host(xh) for _ in range(4)]
+    torch.cuda.synchronize()
+    for o in outs:
+        assert rel(o.numpy(), ref) < 2e-6
     p.destroy()
 
 
