@@ -571,3 +571,27 @@ def test_cg_iterations_replayed_as_cuda_graph_match_eager():
     assert rel(host(x3), xo) < 1e-4
     pe.destroy()
     pg.destroy()
+
+
+@pytest.mark.parametrize("Nd,B", [((32, 64), 1), ((64, 32), 13), ((16, 16, 32), 2), ((128,), 3)])
+def test_linearity_and_adjointness_properties(Nd, B):
+    """Properties that hold at any size (no oracle involved): A(a x1 + b x2) = a A x1 + b A x2, the same for A^H, and
+    <A x, y> = <x, A^H y> per batch element, on planar (B < 12), interleaved (B >= 12), 3-D and 1-D plans."""
+    rng = np.random.default_rng(41)
+    d = len(Nd)
+    M = 3000
+    cfg = dict(Nd=tuple(Nd), Kd=tuple(2 * n for n in Nd), Jd=(6,) * d, om=rng.uniform(-np.pi, np.pi, (M, d)))
+    p = make_plan(cfg, max_batch=B)
+    x1, x2 = wl.image_gaussian(Nd, seed=1, batch=B), wl.image_gaussian(Nd, seed=2, batch=B)
+    y1, y2 = wl.data_gaussian(M, seed=3, batch=B), wl.data_gaussian(M, seed=4, batch=B)
+    a, b = 0.7 - 0.2j, -1.3 + 0.5j
+    A = lambda v: host(p.forward(dev(v))).astype(np.complex128)
+    AH = lambda v: host(p.adjoint(dev(v))).astype(np.complex128)
+    assert rel(A((a * x1 + b * x2).astype(np.complex64)), a * A(x1) + b * A(x2)) < 2e-6
+    assert rel(AH((a * y1 + b * y2).astype(np.complex64)), a * AH(y1) + b * AH(y2)) < 2e-6
+    Ax, AHy = A(x1), AH(y1)
+    for i in range(B):
+        lhs = np.vdot(Ax[i], y1[i].astype(np.complex128))
+        rhs = np.vdot(x1[i].astype(np.complex128).ravel(), AHy[i].ravel())
+        assert abs(lhs - rhs) / abs(lhs) < 2e-5
+    p.destroy()
