@@ -412,6 +412,31 @@ def extra_legs(nb, torch, peak, args):
                           "adjoint_ms": time_calls(lambda: p.adjoint(y, xo), 20, flush),
                           "selfadjoint_ms": time_calls(lambda: p.selfadjoint(x, xo), 20, flush)}
     p.destroy()
+    # the same with opts.use_graphs (repeated calls with fixed pointers replayed as CUDA graphs; non-default stream)
+    pg = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1, use_graphs=1)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+
+    def time_side(fn, n):
+        evs = []
+        with torch.cuda.stream(side):
+            for _ in range(3):
+                fn()
+            for _ in range(n):
+                flush.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(side)
+                fn()
+                b.record(side)
+                evs.append((a, b))
+        side.synchronize()
+        return float(np.median([a.elapsed_time(b) for a, b in evs]))
+
+    out["cfg2_batch1"].update({"forward_graph_ms": time_side(lambda: pg.forward(x, y), 20),
+                               "adjoint_graph_ms": time_side(lambda: pg.adjoint(y, xo), 20),
+                               "selfadjoint_graph_ms": time_side(lambda: pg.selfadjoint(x, xo), 20)})
+    torch.cuda.current_stream().wait_stream(side)
+    pg.destroy()
     # config 4, 3-D
     cfg = wl.config(3)
     N, K, M = cfg["Nd"][0], cfg["Kd"][0], cfg["om"].shape[0]

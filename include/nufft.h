@@ -68,10 +68,13 @@ typedef struct {
                                (half-warp per sample), 2-D planar V gathers through L1/L2; 1 = always direct gather */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
-    int use_graphs;     /* 1 = the CG iterations of nufft_solve_cg and of the L1TV solvers' inner solves are replayed as one
-                               CUDA graph per iteration (pointers are fixed and every scalar lives on the device); the
-                               first iteration of a call runs eagerly, the graph is cached in the plan.  Needs a
-                               non-default stream (the legacy stream cannot capture: eager launches are used).  Default 0 */
+    int use_graphs;     /* 1 = CUDA-graph replay of launch-bound work on a non-default stream (the legacy stream cannot
+                               capture: eager launches are used there):
+                               - nufft_forward / nufft_adjoint / nufft_selfadjoint: a call whose (batch, pointers, stream)
+                                 was seen before is replayed as one graph (small FIFO cache in the plan; the first call of
+                                 each kind runs eagerly);
+                               - the CG iterations of nufft_solve_cg and of the L1TV solvers' inner solves: one graph per
+                                 iteration (pointers are fixed, every scalar lives on the device).  Default 0           */
     int batch_layout;   /* workspace layout of batched 2-D transforms (PAPER.md:52 batch mode, :251-258 coils):
                            0 = auto: calls with batch >= 12 (the measured crossover) use the batch-interleaved grid [group][K0][K1][32]
                                (lanes = images; V^H in gather form with register accumulators, deterministic),

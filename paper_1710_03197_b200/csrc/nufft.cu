@@ -104,6 +104,9 @@ struct nufft_plan_s {
     const float2* cur_mult = nullptr;   // transient: the first adjoint column pass multiplies by this spectrum
     float2* d_dcf_img = nullptr;
     float2* d_dcf_t = nullptr;
+    struct OpGraph { int kind, batch; const void* in; void* out; void* stream; cudaGraphExec_t exec; int launches; };
+    std::vector<OpGraph> op_graphs;         // replayable transform calls (opts.use_graphs)
+    bool op_warm[3][2] = {{false, false}, {false, false}, {false, false}};
     cudaGraphExec_t cg_graph = nullptr;     // one CG iteration (opts.use_graphs)
     CgGraphKey cg_key{};
     int cg_iter_launches = 0;
@@ -872,6 +875,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     if (p->cg_graph) cudaGraphExecDestroy(p->cg_graph);
+    for (auto& og : p->op_graphs) cudaGraphExecDestroy(og.exec);
     if (p->hp_h2d) cudaStreamDestroy(p->hp_h2d);
     if (p->hp_d2h) cudaStreamDestroy(p->hp_d2h);
     for (int i = 0; i < 2; ++i) {
@@ -958,9 +962,7 @@ extern "C" int nufft_stage_fft_scale(nufft_plan_t p, int batch, nufft_c64* grid,
     return run_fft_scale(p, batch, (float2*)grid, (float2*)x, nullptr, (cudaStream_t)stream);
 }
 
-extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* y, void* stream) {
-    if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
+static int forward_impl(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* y, cudaStream_t st) {
     if (use_il(p, batch)) {
         NU_TRY(run_scale_fft_il(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
         NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, st));
@@ -970,9 +972,7 @@ extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nuff
     return run_interp(p, batch, p->d_grid, (float2*)y, st);
 }
 
-extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nufft_c64* x, void* stream) {
-    if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
+static int adjoint_impl(nufft_plan_t p, int batch, const nufft_c64* y, nufft_c64* x, cudaStream_t st) {
     if (use_il(p, batch)) {
         NU_TRY(run_y_to_il(p, batch, (const float2*)y, st));
         NU_TRY(run_gridding_il(p, batch, p->d_yil, p->d_grid, st));
@@ -982,9 +982,7 @@ extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nuff
     return run_fft_scale(p, batch, p->d_grid, (float2*)x, nullptr, st);
 }
 
-extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
-    if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
+static int selfadjoint_impl(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, cudaStream_t st) {
     if (use_il(p, batch)) {     // the intermediate samples stay sorted and interleaved: no scatter, no gather
         NU_TRY(run_scale_fft_il(p, batch, (const float2*)x_in, p->d_grid, nullptr, false, st));
         NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, st));
@@ -995,6 +993,73 @@ extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_i
     NU_TRY(run_interp(p, batch, p->d_grid, p->d_ywork, st));
     NU_TRY(run_gridding(p, batch, p->d_ywork, p->d_grid, st));
     return run_fft_scale(p, batch, p->d_grid, (float2*)x_out, nullptr, st);
+}
+
+// opts.use_graphs: a transform call whose (kind, batch, pointers, stream) was seen before is replayed as one CUDA graph
+// (solver loops and the host pipeline call with fixed pointers; single small transforms are launch-latency bound).  The
+// first call of each kind and layout runs eagerly so that lazy allocations happen outside a capture; calls made while the
+// stream is already capturing (the CG iteration graph) and calls on the legacy stream run eagerly.
+template <class F>
+static int run_graphed(nufft_plan_t p, int kind, int batch, const void* in, void* out, cudaStream_t st, F impl) {
+    const int il = use_il(p, batch) ? 1 : 0;
+    bool eager = !p->opts.use_graphs || p->prof_on || st == nullptr || !p->op_warm[kind][il];
+    if (!eager) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) eager = true;
+    }
+    if (eager) {
+        const int rc = impl();
+        if (rc == NUFFT_OK) p->op_warm[kind][il] = true;
+        return rc;
+    }
+    for (auto& g : p->op_graphs)
+        if (g.kind == kind && g.batch == batch && g.in == in && g.out == out && g.stream == (void*)st) {
+            CU_TRY(cudaGraphLaunch(g.exec, st));
+            p->launches += g.launches;
+            return NUFFT_OK;
+        }
+    const int64_t l0 = p->launches;
+    CU_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    const int rc = impl();
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(st, &g);
+    const int nl = (int)(p->launches - l0);
+    p->launches = l0;
+    if (rc != NUFFT_OK || e != cudaSuccess || !g) {
+        if (g) cudaGraphDestroy(g);
+        (void)cudaGetLastError();
+        if (rc != NUFFT_OK) return rc;
+        g_last_cuda_error = (int)e;
+        return NUFFT_ECUDA;
+    }
+    nufft_plan_s::OpGraph og{kind, batch, in, out, (void*)st, nullptr, nl};
+    const cudaError_t ei = cudaGraphInstantiate(&og.exec, g, 0);
+    cudaGraphDestroy(g);
+    if (ei != cudaSuccess) { g_last_cuda_error = (int)ei; (void)cudaGetLastError(); return NUFFT_ECUDA; }
+    if (p->op_graphs.size() >= 16) {            // small FIFO cache
+        cudaGraphExecDestroy(p->op_graphs.front().exec);
+        p->op_graphs.erase(p->op_graphs.begin());
+    }
+    p->op_graphs.push_back(og);
+    CU_TRY(cudaGraphLaunch(og.exec, st));
+    p->launches += nl;
+    return NUFFT_OK;
+}
+
+extern "C" int nufft_forward(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* y, void* stream) {
+    if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    return run_graphed(p, 0, batch, x, y, st, [&]() { return forward_impl(p, batch, x, y, st); });
+}
+extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nufft_c64* x, void* stream) {
+    if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    return run_graphed(p, 1, batch, y, x, st, [&]() { return adjoint_impl(p, batch, y, x, st); });
+}
+extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
+    if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    return run_graphed(p, 2, batch, x_in, x_out, st, [&]() { return selfadjoint_impl(p, batch, x_in, x_out, st); });
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -595,3 +595,32 @@ def test_linearity_and_adjointness_properties(Nd, B):
         rhs = np.vdot(x1[i].astype(np.complex128).ravel(), AHy[i].ravel())
         assert abs(lhs - rhs) / abs(lhs) < 2e-5
     p.destroy()
+
+
+def test_transform_calls_replayed_as_cuda_graphs_match_eager():
+    """opts.use_graphs: repeated forward / adjoint / selfadjoint calls with the same pointers on a non-default stream are
+    graph replays; results are the bits of the eager plan (deterministic V^H), also after the inputs change in place."""
+    for cfg, B in ((wl.config(0), 1), (wl.config(0), 20), (wl.config(3, scale=8), 1)):
+        M = cfg["om"].shape[0]
+        pe = make_plan(cfg, max_batch=B, adjoint_mode=1)
+        pg = make_plan(cfg, max_batch=B, adjoint_mode=1, use_graphs=1)
+        x = dev(wl.image_gaussian(cfg["Nd"], batch=B))
+        y = dev(wl.data_gaussian(M, batch=B))
+        yo, xo, so = pe._new(B, M), pe._new(B, *cfg["Nd"]), pe._new(B, *cfg["Nd"])
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        for rep in range(4):                       # eager, capture, replay, replay (inputs changed in place)
+            if rep == 3:
+                x.mul_(0.5)
+                y.add_(1.0)
+                torch.cuda.synchronize()
+            with torch.cuda.stream(side):
+                pg.forward(x, yo)
+                pg.adjoint(y, xo)
+                pg.selfadjoint(x, so)
+            side.synchronize()
+            assert np.array_equal(host(yo).view(np.uint32), host(pe.forward(x)).view(np.uint32))
+            assert np.array_equal(host(xo).view(np.uint32), host(pe.adjoint(y)).view(np.uint32))
+            assert np.array_equal(host(so).view(np.uint32), host(pe.selfadjoint(x)).view(np.uint32))
+        pe.destroy()
+        pg.destroy()
