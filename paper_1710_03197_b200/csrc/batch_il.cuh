@@ -109,6 +109,8 @@ fft_il_rows_adj_kernel(IlRowParams p) {
 struct IlPlan {
     const uint32_t* kpack;    // V order: stencil base index per axis (10 bits each)
     const float* delta;       // V order: [2][M]
+    const uint32_t* kpack_c;  // caller order (trajectory-coherent plans only, else null)
+    const float* delta_c;     // caller order [2][M]
     const int32_t* v2h;       // V-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
     const float* wtab;        // V^H order: [M][kTabW] = w0[6], k0_0 (int bits), pad, w1 part A[8], w1 part B[8] (float64-built)
@@ -120,26 +122,37 @@ struct IlPlan {
 // the samples one by one with warp-uniform weights: 36 loads of 256 contiguous bytes and 72 + 12 FMAs per lane.
 constexpr int kInterpWarps = 8;
 constexpr int kInterpChunk = 64;     // consecutive sorted samples per CTA
-// Output: y_il[group][sorted sample][32] (coalesced); y_from_il_kernel restores the caller's order when needed.
+constexpr int kInterpChunkCaller = 64;   // ... in the caller-order variant (its output tile lives in shared memory)
+// CALLER = false: samples are walked in V order and the output is y_il[group][V^H position][32] (coalesced rows);
+//                 y_from_il_kernel restores the caller's order when needed.
+// CALLER = true:  trajectory-coherent plans (consecutive caller samples are neighbours in k-space: radial spokes, spiral
+//                 arms): samples are walked in the CALLER's order (kpack_c / delta_c), which has the same L1 locality
+//                 along the readout, and the 64 x 32 result tile is written through shared memory straight into
+//                 y[batch][M] (512 contiguous bytes per image): no layout pass at all.
+template <bool CALLER, int CHUNK>
 __global__ void __launch_bounds__(256)
-interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y_il, KernelPoly P) {
-    __shared__ float4 wrec[kInterpChunk * 4];
+interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y_il, int batch,
+                 KernelPoly P) {
+    __shared__ float4 wrec[CHUNK * 4];
+    __shared__ float2 otile[CALLER ? CHUNK : 1][33];
+    const uint32_t* __restrict__ kpk = CALLER ? s.kpack_c : s.kpack;
+    const float* __restrict__ dlt = CALLER ? s.delta_c : s.delta;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = blockIdx.y;
-    const int64_t s0 = (int64_t)blockIdx.x * kInterpChunk;
-    const int cnt = (int)min((int64_t)kInterpChunk, g.M - s0);
+    const int64_t s0 = (int64_t)blockIdx.x * CHUNK;
+    const int cnt = (int)min((int64_t)CHUNK, g.M - s0);
     for (int t = threadIdx.x; t < cnt; t += blockDim.x) {
         const int64_t si = s0 + t;
-        const uint32_t kp = __ldg(&s.kpack[si]);
+        const uint32_t kp = __ldg(&kpk[si]);
         float w0[kJ], w1[kJ];
-        kb_weights(P, __ldg(&s.delta[si]), w0);
-        kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
+        kb_weights(P, __ldg(&dlt[si]), w0);
+        kb_weights(P, __ldg(&dlt[g.M + si]), w1);
         float4* r = &wrec[t * 4];
         r[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
         r[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
         r[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
         r[3] = make_float4(__int_as_float((int)(kp & 1023u)), __int_as_float((int)((kp >> 10) & 1023u)),
-                           __int_as_float(__ldg(&s.v2h[si])), 0.f);
+                           __int_as_float(CALLER ? 0 : __ldg(&s.v2h[si])), 0.f);
     }
     __syncthreads();
     const int K0 = g.K[0], K1 = g.K[1];
@@ -182,7 +195,17 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
                 acc.y = fmaf(w0[j0], r.y, acc.y);
             }
         }
-        y_il[((int64_t)grp * g.M + __float_as_int(rd.z)) * kIL + lane] = acc;
+        if (CALLER) otile[sidx][lane] = acc;
+        else y_il[((int64_t)grp * g.M + __float_as_int(rd.z)) * kIL + lane] = acc;
+    }
+    if (CALLER) {     // y_il is the caller's y[batch][M] here: warp w writes images 4w .. 4w+3, 64 consecutive samples each
+        __syncthreads();
+#pragma unroll
+        for (int li = 0; li < kIL / kInterpWarps; ++li) {
+            const int l = warp * (kIL / kInterpWarps) + li, b = grp * kIL + l;
+            if (b >= batch) continue;
+            for (int t = lane; t < cnt; t += 32) y_il[(int64_t)b * g.M + s0 + t] = otile[t][l];
+        }
     }
 }
 

@@ -89,6 +89,9 @@ struct nufft_plan_s {
     float* d_il_wtab = nullptr;
     int32_t* d_il_rowptr = nullptr;
     int32_t* d_il_v2h = nullptr;     // V-order position -> V^H-order position
+    uint32_t* d_il_kpack_c = nullptr;    // caller-order copies for trajectory-coherent plans (il_coherent)
+    float* d_il_delta_c = nullptr;
+    bool il_coherent = false;
     IlItem* d_il_items = nullptr;
     int n_il_items = 0;
     float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
@@ -472,6 +475,7 @@ static IlPlan il_plan(nufft_plan_t p) {
     IlPlan s{};
     s.kpack = p->d_il_kpack; s.delta = p->d_il_delta; s.pos = p->d_il_pos; s.wtab = p->d_il_wtab;
     s.rowptr = p->d_il_rowptr; s.v2h = p->d_il_v2h;
+    s.kpack_c = p->d_il_kpack_c; s.delta_c = p->d_il_delta_c;
     return s;
 }
 
@@ -502,7 +506,17 @@ static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* 
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + kInterpChunk - 1) / kInterpChunk), (unsigned)il_groups(batch));
     ProfScope ps(p, "interp", st);
-    interp_il_kernel<<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, p->poly);
+    interp_il_kernel<false, kInterpChunk><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+// a3 for trajectory-coherent plans: y[batch][M] in the caller's order straight from the kernel (no layout pass)
+static int run_interp_il_caller(nufft_plan_t p, int batch, const float2* grid, float2* y, cudaStream_t st) {
+    if (p->M == 0) return NUFFT_OK;
+    const dim3 blocks((unsigned)((p->M + kInterpChunkCaller - 1) / kInterpChunkCaller), (unsigned)il_groups(batch));
+    ProfScope ps(p, "interp", st);
+    interp_il_kernel<true, kInterpChunkCaller><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
     CU_TRY(cudaGetLastError());
     p->launches++;
     return NUFFT_OK;
@@ -680,6 +694,21 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
         }
     std::stable_sort(items.begin(), items.end(), [](const IlItem& a, const IlItem& b) { return a.load > b.load; });
     p->n_il_items = (int)items.size();
+    // trajectory coherence of the caller's order: consecutive samples within two cells of each other on both axes
+    // (modulo the grid) in at least 90 % of the cases -> V can walk the caller's order and write y directly
+    {
+        int64_t near = 0;
+        for (int64_t m = 1; m < M; ++m) {
+            int d0 = std::abs(row_of(kpack[m]) - row_of(kpack[m - 1])), d1 = std::abs(col_of(kpack[m]) - col_of(kpack[m - 1]));
+            d0 = std::min(d0, K0 - d0); d1 = std::min(d1, K1 - d1);
+            near += (d0 <= 2 && d1 <= 2) ? 1 : 0;
+        }
+        p->il_coherent = (M > 1) && (near * 10 >= (M - 1) * 9) && p->opts.interp_mode == 0;
+        if (p->il_coherent) {
+            NU_TRY(dev_upload(&p->d_il_kpack_c, kpack, &p->bytes_plan));
+            NU_TRY(dev_upload(&p->d_il_delta_c, delta, &p->bytes_plan));
+        }
+    }
     NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_delta, dl_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_v2h, v2h, &p->bytes_plan));
@@ -873,6 +902,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_kspace);
     cudaFree(p->d_ones); cudaFree(p->d_that); cudaFree(p->d_dcf_img); cudaFree(p->d_dcf_t);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
+    cudaFree(p->d_il_kpack_c); cudaFree(p->d_il_delta_c);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     if (p->cg_graph) cudaGraphExecDestroy(p->cg_graph);
     for (auto& og : p->op_graphs) cudaGraphExecDestroy(og.exec);
@@ -965,6 +995,7 @@ extern "C" int nufft_stage_fft_scale(nufft_plan_t p, int batch, nufft_c64* grid,
 static int forward_impl(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* y, cudaStream_t st) {
     if (use_il(p, batch)) {
         NU_TRY(run_scale_fft_il(p, batch, (const float2*)x, p->d_grid, nullptr, false, st));
+        if (p->il_coherent) return run_interp_il_caller(p, batch, p->d_grid, (float2*)y, st);
         NU_TRY(run_interp_il(p, batch, p->d_grid, p->d_ywork, st));
         return run_y_from_il(p, batch, p->d_ywork, (float2*)y, st);
     }
@@ -1171,6 +1202,7 @@ extern "C" int nufft_forward_coils(nufft_plan_t p, const nufft_c64* x, nufft_c64
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
         NU_TRY(run_scale_fft_il(p, p->ncoil, (const float2*)x, p->d_grid, p->d_coils, true, st));
+        if (p->il_coherent) return run_interp_il_caller(p, p->ncoil, p->d_grid, (float2*)y, st);
         NU_TRY(run_interp_il(p, p->ncoil, p->d_grid, p->d_ywork, st));
         return run_y_from_il(p, p->ncoil, p->d_ywork, (float2*)y, st);
     }

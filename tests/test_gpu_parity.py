@@ -371,6 +371,22 @@ def check_batched(cfg, B, sample_imgs, seed=0):
     q.destroy()
 
 
+def test_interleaved_coherent_caller_order_interp_matches_sorted_path():
+    """Radial trajectory (coherent caller order): V walks the caller's order and writes y directly; interp_mode = 1 keeps the
+    sorted walk + layout pass.  Same results; ragged batch 40; a trajectory with 16 incoherent jumps per spoke boundary."""
+    cfg = wl.config(1, scale=2)
+    B, M = 40, cfg["om"].shape[0]
+    pc = make_plan(cfg, max_batch=B)
+    ps = make_plan(cfg, max_batch=B, interp_mode=1)
+    x = wl.image_gaussian(cfg["Nd"], batch=B)
+    yc, ys = host(pc.forward(dev(x))), host(ps.forward(dev(x)))
+    assert rel(yc, ys) < 1e-6
+    yo = orc.forward(x[39].astype(np.complex128), cfg["om"], cfg["Nd"], cfg["Kd"], cfg["Jd"])
+    assert rel(yc[39], yo) < TOL
+    pc.destroy()
+    ps.destroy()
+
+
 def test_interleaved_config1_ragged_batch40():
     check_batched(wl.config(0), 40, [0, 31, 32, 39])
 
