@@ -100,6 +100,57 @@ fft_il_rows_adj_kernel(IlRowParams p) {
     fft_line<K, false, true>(q0, active, lay, p.tw, ld, st);
 }
 
+// Multi-coil variant of the pass above with the coil sum of eq. (35) fused: x[n] = sum_i conj(c_i[n]) (S^H F^H grid_i)[n].
+// CTA = one image row; it walks the coils T at a time (thread (t, q0) works on coil o T + t), multiplies by conj(c_i),
+// sums the T coils of an octet with lane shuffles (the T lanes of a q0 are adjacent) and keeps the running sum over the
+// octets in registers: the per-coil images are never written, coil_sum_kernel is not needed, the order is fixed.
+template <int K>
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
+fft_il_rows_adj_coilsum_kernel(IlRowParams p) {
+    constexpr int N = K / 2, T = Rad<K>::TS, E = Rad<K>::E;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, q0 = threadIdx.x / T;
+    const int n0 = blockIdx.x;
+    const int g0 = (n0 - p.n_outer / 2) & (p.k_outer - 1);
+    const float so = __ldg(&p.s_outer[n0]);
+    const float* __restrict__ sl = p.s_line;
+    LayStrided<K, T> lay{smem + t};
+    float2 acc[E];
+    int nidx[E];
+#pragma unroll
+    for (int c = 0; c < E; ++c) { acc[c] = make_float2(0.f, 0.f); nidx[c] = 0; }
+    const int noct = (p.batch + T - 1) / T;
+    for (int o = 0; o < noct; ++o) {
+        const int b = o * T + t;
+        const bool active = b < p.batch;
+        const int bb = active ? b : 0;
+        const float2* __restrict__ src = p.grid + (((int64_t)(bb / kIL) * p.k_outer + g0) * K) * kIL + (bb % kIL);
+        const float2* __restrict__ csrc = p.coil + ((int64_t)bb * p.n_outer + n0) * N;
+        int cnt = 0;
+        auto ld = [&](int i) -> float2 { return active ? cconj(src[(int64_t)i * kIL]) : make_float2(0.f, 0.f); };
+        auto st = [&](int i, float2 v) {
+            const int n = (i + N / 2) & (K - 1);
+            float2 r = cscale(cconj(v), so * __ldg(&sl[n]));
+            r = active ? cmul(r, cconj(__ldg(&csrc[n]))) : make_float2(0.f, 0.f);
+#pragma unroll
+            for (int off = T / 2; off > 0; off >>= 1) {
+                r.x += __shfl_xor_sync(0xffffffffu, r.x, off);
+                r.y += __shfl_xor_sync(0xffffffffu, r.y, off);
+            }
+            acc[cnt] = cadd(acc[cnt], r);
+            nidx[cnt] = n;
+            ++cnt;
+        };
+        fft_line<K, false, true>(q0, true, lay, p.tw, ld, st);
+        __syncthreads();          // the exchange buffers are reused by the next octet
+    }
+    if (t == 0) {
+        float2* __restrict__ dst = p.img_out + (int64_t)n0 * N;
+#pragma unroll
+        for (int c = 0; c < E / 2; ++c) dst[nidx[c]] = acc[c];
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // plan data of the interleaved path (built by plan_build_il in nufft.cu).  Two sample orders:
 //   V order    key (column band, row k0_0, column):  kpack, delta, v2h

@@ -175,6 +175,8 @@ template <int K> static cudaError_t configure_fft() {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_il_rows_adj_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_il_rows_adj_coilsum_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_cols_kernel<K, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_cols_kernel<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
@@ -454,6 +456,23 @@ static int dispatch_il_rows(int K, bool adj, const IlRowParams& p, cudaStream_t 
     CU_TRY(cudaGetLastError());
     return NUFFT_OK;
 }
+template <int K> static void launch_il_rows_coilsum(const IlRowParams& p, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
+    fft_il_rows_adj_coilsum_kernel<K><<<p.n_outer, threads, smem_cols<K>(), st>>>(p);
+}
+static int dispatch_il_rows_coilsum(int K, const IlRowParams& p, cudaStream_t st) {
+    switch (K) {
+        case 32: launch_il_rows_coilsum<32>(p, st); break;
+        case 64: launch_il_rows_coilsum<64>(p, st); break;
+        case 128: launch_il_rows_coilsum<128>(p, st); break;
+        case 256: launch_il_rows_coilsum<256>(p, st); break;
+        case 512: launch_il_rows_coilsum<512>(p, st); break;
+        case 1024: launch_il_rows_coilsum<1024>(p, st); break;
+        default: return NUFFT_EINVAL;
+    }
+    CU_TRY(cudaGetLastError());
+    return NUFFT_OK;
+}
 static IlRowParams il_row_params(nufft_plan_t p, int batch, const float2* img_in, float2* img_out, float2* grid,
                                  const float2* coil, bool same_image) {
     IlRowParams r{};
@@ -489,7 +508,8 @@ static int run_scale_fft_il(nufft_plan_t p, int batch, const float2* x, float2* 
     return NUFFT_OK;
 }
 // a5 + a6 on the interleaved grid
-static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
+static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st,
+                            bool coil_sum = false) {
     {
         ColPassParams c = il_col_params(p, batch, grid);
         c.mult = p->cur_mult; c.mult_shift = 5;
@@ -497,7 +517,13 @@ static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, 
         NU_TRY(dispatch_cols(p->K[0], true, c, st));
     }
     IlRowParams r = il_row_params(p, batch, nullptr, x, grid, coil, false);
-    { ProfScope ps(p, "fft_rows_adj", st); NU_TRY(dispatch_il_rows(p->K[1], true, r, st)); }
+    if (coil_sum) {      // x is the coil-summed image [N0][N1] (eq. 35): the sum is fused into the last pass
+        ProfScope ps(p, "fft_rows_adj", st);
+        NU_TRY(dispatch_il_rows_coilsum(p->K[1], r, st));
+    } else {
+        ProfScope ps(p, "fft_rows_adj", st);
+        NU_TRY(dispatch_il_rows(p->K[1], true, r, st));
+    }
     p->launches += 2;
     return NUFFT_OK;
 }
@@ -1217,8 +1243,7 @@ extern "C" int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64* y, nufft_c64
     if (use_il(p, p->ncoil)) {
         NU_TRY(run_y_to_il(p, p->ncoil, (const float2*)y, st));
         NU_TRY(run_gridding_il(p, p->ncoil, p->d_yil, p->d_grid, st));
-        NU_TRY(run_fft_scale_il(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
-        return coil_reduce(p, (float2*)x, st);
+        return run_fft_scale_il(p, p->ncoil, p->d_grid, (float2*)x, p->d_coils, st, true);
     }
     NU_TRY(run_gridding(p, p->ncoil, (const float2*)y, p->d_grid, st));
     NU_TRY(run_fft_scale(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
@@ -1233,8 +1258,7 @@ extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nu
         NU_TRY(run_scale_fft_il(p, p->ncoil, (const float2*)x_in, p->d_grid, p->d_coils, true, st));
         NU_TRY(run_interp_il(p, p->ncoil, p->d_grid, p->d_ywork, st));
         NU_TRY(run_gridding_il(p, p->ncoil, p->d_ywork, p->d_grid, st));
-        NU_TRY(run_fft_scale_il(p, p->ncoil, p->d_grid, p->d_imgwork, p->d_coils, st));
-        return coil_reduce(p, (float2*)x_out, st);
+        return run_fft_scale_il(p, p->ncoil, p->d_grid, (float2*)x_out, p->d_coils, st, true);
     }
     NU_TRY(run_scale_fft(p, p->ncoil, (const float2*)x_in, p->d_grid, p->d_coils, true, st));
     NU_TRY(run_interp(p, p->ncoil, p->d_grid, p->d_ywork, st));
@@ -1369,14 +1393,18 @@ extern "C" int nufft_toeplitz_enable(nufft_plan_t p, int on) {
 }
 
 // x_out = crop(F^H(T^ . F(pad x_in))); coils: sum_i conj(c_i) crop(F^H(T^ . F(pad c_i x_in)))
-static int run_toeplitz(nufft_plan_t p, int batch, const float2* x_in, float2* x_out, const float2* coil, bool same_image,
-                        cudaStream_t st) {
+// coil != nullptr on the interleaved path: x_out is the coil-SUMMED image (sum fused into the last pass); on the planar path
+// x_out receives the per-coil images and the caller reduces them.  *summed tells which.
+static int run_toeplitz(nufft_plan_t p, int batch, const float2* x_in, float2* x_out, float2* x_sum, const float2* coil,
+                        bool same_image, cudaStream_t st, bool* summed = nullptr) {
     p->unit_scale = true;
     p->cur_mult = p->d_that;
     int rc;
     if (use_il(p, batch)) {
         rc = run_scale_fft_il(p, batch, x_in, p->d_grid, coil, same_image, st);
-        if (rc == NUFFT_OK) rc = run_fft_scale_il(p, batch, p->d_grid, x_out, coil, st);
+        const bool fuse = coil != nullptr && x_sum != nullptr;
+        if (rc == NUFFT_OK) rc = run_fft_scale_il(p, batch, p->d_grid, fuse ? x_sum : x_out, coil, st, fuse);
+        if (summed) *summed = fuse;
     } else {
         rc = run_scale_fft(p, batch, x_in, p->d_grid, coil, same_image, st);
         if (rc == NUFFT_OK) rc = run_fft_scale(p, batch, p->d_grid, x_out, coil, st);
@@ -1389,7 +1417,7 @@ static int run_toeplitz(nufft_plan_t p, int batch, const float2* x_in, float2* x
 extern "C" int nufft_selfadjoint_toeplitz(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
     if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
     if (!p->d_that) return NUFFT_ESTATE;
-    return run_toeplitz(p, batch, (const float2*)x_in, (float2*)x_out, nullptr, false, (cudaStream_t)stream);
+    return run_toeplitz(p, batch, (const float2*)x_in, (float2*)x_out, nullptr, nullptr, false, (cudaStream_t)stream);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -1420,8 +1448,9 @@ extern "C" int nufft_selfadjoint_toeplitz_coils(nufft_plan_t p, const nufft_c64*
     if (!p || !x_in || !x_out) return NUFFT_EINVAL;
     if (p->ncoil < 1 || !p->d_that) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    NU_TRY(run_toeplitz(p, p->ncoil, (const float2*)x_in, p->d_imgwork, p->d_coils, true, st));
-    return coil_reduce(p, (float2*)x_out, st);
+    bool summed = false;
+    NU_TRY(run_toeplitz(p, p->ncoil, (const float2*)x_in, p->d_imgwork, (float2*)x_out, p->d_coils, true, st, &summed));
+    return summed ? NUFFT_OK : coil_reduce(p, (float2*)x_out, st);
 }
 
 static int apply_aha(nufft_plan_t p, bool coils, const float2* in, float2* out, cudaStream_t st) {
