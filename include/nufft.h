@@ -65,7 +65,11 @@ typedef struct {
                                (bit-reproducible run to run).  The interleaved path (batch >= 12) is always
                                deterministic (gather form, fixed order)                                             */
     int interp_mode;    /* 0 = library default: 3-D planar V stages the padded tile of a work item in shared memory
-                               (half-warp per sample), 2-D planar V gathers through L1/L2; 1 = always direct gather */
+                               (half-warp per sample), 2-D planar V gathers through L1/L2, interleaved V walks the
+                               CALLER's sample order and writes y directly when the trajectory is coherent (>= 90 % of
+                               consecutive samples within two grid cells: radial spokes, spiral arms);
+                           1 = the plain variants: direct gather in 3-D, sorted walk + layout pass on the interleaved
+                               path (kept for cross-checks)                                                        */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
     int use_graphs;     /* 1 = CUDA-graph replay of launch-bound work on a non-default stream (the legacy stream cannot
