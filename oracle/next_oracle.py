@@ -13,8 +13,10 @@ Readings of the paper taken here (R21-R24; R23 and R24 are stated in t
          (elementwise magnitude, as in ref. [7]'s iteration), a fixed iteration count given by the caller.
     R22  the paper's own "Toeplitz" precomputes the sparse V^H V; SURVEY 8(f)-1 asks for the true
          Toeplitz embedding of ref. [6]: A^H A x = crop(F^H(T^ . F(pad x))) on the 2N grid, T^ = F(T),
-         T[d] = sum_m w_m e^{i om_m . d}, d in [-N, N)^dim, obtained by ONE adjoint NUFFT of the weights onto a 2N image
-         (4N grid).  It equals the back-to-back operator up to the interpolation-kernel error (~1e-5), not to rounding.
+         T[d] = sum_m w_m e^{i om_m . d}, d in [-N, N)^dim, obtained from 2^dim adjoint NUFFTs of phase-modulated weights
+         on the plan's own geometry (one per half-shift s in {-N/2, +N/2}^dim; no larger grid is needed, so every
+         supported size works).  It equals the back-to-back operator up to the interpolation-kernel error (~1e-5), not
+         to rounding.
 
 Parity pins (tests/test_oracle_next.py):
     density_weights        Cartesian full sampling: fixed point w = 1 / prod(N) (closed form, A A^H = prod(N) I);
@@ -56,14 +58,20 @@ def adjoint_dcf(y, w, om, Nd, Kd, Jd):
 
 def toeplitz_kernel(om, Nd, Kd, Jd, w=None):
     """T^ = FFT over the 2N grid of the point-spread function T[d] = sum_m w_m e^{i om_m . d}, d in [-N, N)^dim (R22).
-    T comes from one adjoint NUFFT of the weights onto an image of size 2N (grid 4N): its pixel n sits at position
-    n - N = d.  Returns (T^ complex128 of shape 2N, T of shape 2N with d = n - N)."""
+    T is assembled from 2^dim adjoint NUFFTs on the SAME Nd / Kd geometry: with d = d' + s, d' in [-N/2, N/2)^dim and
+    s in {-N/2, +N/2}^dim,  T[d' + s] = sum_m (w_m e^{i om_m . s}) e^{i om_m . d'}  is the adjoint NUFFT of the modulated
+    weights, whose pixel n sits at position n - N/2 = d'.  Block h in {0,1}^dim (s_a = (h_a - 1/2) N_a) fills
+    T[h_a N_a : (h_a + 1) N_a] of the array indexed by n2 = d + N.  Returns (T^ complex128 of shape 2N, T)."""
+    import itertools
     Nd = tuple(int(n) for n in Nd)
-    N2 = tuple(2 * n for n in Nd)
-    K2 = tuple(4 * n for n in Nd)
-    M = np.asarray(om).shape[0]
+    om = np.asarray(om, dtype=np.float64)
+    M = om.shape[0]
     wv = np.ones(M, dtype=np.complex128) if w is None else np.asarray(w, dtype=np.complex128)
-    T = orc.adjoint(wv, om, N2, K2, Jd)
+    T = np.zeros(tuple(2 * n for n in Nd), dtype=np.complex128)
+    for h in itertools.product((0, 1), repeat=len(Nd)):
+        shift = np.array([(ha - 0.5) * n for ha, n in zip(h, Nd)])
+        blk = orc.adjoint(wv * np.exp(1j * (om @ shift)), om, Nd, Kd, Jd)
+        T[tuple(slice(ha * n, (ha + 1) * n) for ha, n in zip(h, Nd))] = blk
     # d = -N (pixel 0 on every axis) is never used by a linear convolution of two length-N supports; drop it
     for a in range(len(Nd)):
         sl = [slice(None)] * len(Nd)
