@@ -487,6 +487,21 @@ def extra_legs(nb, torch, peak, args):
             evs.append((a, b))
     side.synchronize()
     out["cfg3_2d_spiral_cg50"]["cg50_graph_ms"] = float(np.median([a.elapsed_time(b) for a, b in evs]))
+    # next row 8(f)-1 on config 3: the same 50 iterations with A^H A in Toeplitz form (no V / V^H per iteration)
+    pg.toeplitz_build()
+    pg.toeplitz_enable(True)
+    with torch.cuda.stream(side):
+        pg.solve_cg(y3, 5, x=xs)
+        evs = []
+        for _ in range(3):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(side)
+            pg.solve_cg(y3, 50, x=xs)
+            b.record(side)
+            evs.append((a, b))
+    side.synchronize()
+    out["cfg3_2d_spiral_cg50"]["cg50_toeplitz_graph_ms"] = float(np.median([a.elapsed_time(b) for a, b in evs]))
     torch.cuda.current_stream().wait_stream(side)
     pg.destroy()
     # config 5: 32-coil 2-D radial, multi-coil A^H A and 20 split-Bregman L1TV-OLS iterations (interleaved path)

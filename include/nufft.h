@@ -165,11 +165,12 @@ int nufft_adjoint_dcf(nufft_plan_t p, int batch, const nufft_c64 *y, const nufft
 
 /* Toeplitz form of A^H A ("precomputing A^H A", ref.[6]; reading R22):
  *   A^H A x = crop(F^H(T^ . F(pad x))) on the same K = 2N grid, T^ = F(T), T[d] = sum_m w_m e^{i om_m . d}.
- * nufft_toeplitz_build computes T^ once per plan with ONE adjoint NUFFT of the weights w (device complex64 [M], or NULL
- * = all ones) onto a 2N image through a temporary second plan (4N grid: needs 2*Kd[a] <= 1024, else NUFFT_EINVAL);
- * synchronises the stream.  The result differs from the back-to-back nufft_selfadjoint by the interpolation-kernel
- * error (~1e-5 relative), not by rounding; V and V^H no longer run.  nufft_toeplitz_enable(p, 1) makes nufft_solve_cg
- * and nufft_solve_l1tv_ols apply A^H A this way (NUFFT_ESTATE before a build). */
+ * nufft_toeplitz_build computes T^ once per plan from 2^d adjoint NUFFTs of the weights w (device complex64 [M], or NULL =
+ * all ones), phase-modulated on the host in float64, on the plan's OWN geometry: with d = d' + s, d' in [-N/2, N/2)^d and
+ * s in {-N/2, +N/2}^d, T[d' + s] = sum_m (w_m e^{i om_m . s}) e^{i om_m . d'} is the adjoint NUFFT of the modulated weights;
+ * every supported size works (no larger grid).  Synchronises the stream.  The result differs from the back-to-back
+ * nufft_selfadjoint by the interpolation-kernel error (~1e-5 relative), not by rounding; V and V^H no longer run.
+ * nufft_toeplitz_enable(p, 1) makes nufft_solve_cg and the L1TV solvers apply A^H A this way (NUFFT_ESTATE before a build). */
 int nufft_toeplitz_build(nufft_plan_t p, const nufft_c64 *w, void *stream);
 int nufft_toeplitz_enable(nufft_plan_t p, int on);
 int nufft_selfadjoint_toeplitz(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);

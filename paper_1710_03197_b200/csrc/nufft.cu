@@ -1350,38 +1350,52 @@ static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st) {
 
 extern "C" int nufft_toeplitz_build(nufft_plan_t p, const nufft_c64* w, void* stream) {
     if (!p) return NUFFT_EINVAL;
-    for (int a = 0; a < p->d; ++a)
-        if (2 * p->K[a] > 1024) return NUFFT_EINVAL;         // the point-spread function needs a 4N grid
     cudaStream_t st = (cudaStream_t)stream;
+    const int d = p->d;
+    const int64_t M = p->M;
     if (!p->d_that) NU_TRY(dev_alloc((void**)&p->d_that, (size_t)p->cells * sizeof(float2), &p->bytes_plan));
-    // T[d] = sum_m w_m e^{i om_m . d}: one adjoint NUFFT of the weights onto the 2N image (R22)
-    int64_t N2[3], K2[3];
-    int J[3] = {kJ, kJ, kJ};
-    for (int a = 0; a < p->d; ++a) { N2[a] = p->K[a]; K2[a] = 2 * p->K[a]; }
-    nufft_opts o2;
-    nufft_default_opts(&o2);
-    o2.batch_layout = 1;
-    nufft_plan_t p2 = nullptr;
-    NU_TRY(nufft_plan(p->d, N2, K2, J, p->M, p->om_host.data(), 1, &o2, &p2));
-    int rc = NUFFT_OK;
-    float2* ones = nullptr;
-    if (!w && p->M > 0) {
-        rc = dev_alloc((void**)&ones, (size_t)p->M * sizeof(float2), nullptr);
-        if (rc == NUFFT_OK) dcf_init_kernel<<<ew_blocks(p->M), 256, 0, st>>>(ones, p->M);
+    if (!p->d_dcf_img) NU_TRY(dev_alloc((void**)&p->d_dcf_img, (size_t)p->nimg * sizeof(float2), &p->bytes_work));
+    // T[d' + s] = sum_m (w_m e^{i om_m . s}) e^{i om_m . d'}: 2^d adjoint NUFFTs of phase-modulated weights on this plan's own
+    // geometry, one per half-shift s in {-N/2, +N/2}^d (R22); the modulation is computed on the host in float64.
+    std::vector<float2> wh((size_t)std::max<int64_t>(M, 1), make_float2(1.f, 0.f)), wmod((size_t)std::max<int64_t>(M, 1));
+    if (w && M > 0) {
+        CU_TRY(cudaMemcpyAsync(wh.data(), w, (size_t)M * sizeof(float2), cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
     }
-    if (rc == NUFFT_OK) rc = nufft_adjoint(p2, 1, w ? w : (const nufft_c64*)ones, (nufft_c64*)p->d_that, st);
+    float2* d_wmod = nullptr;
+    NU_TRY(dev_alloc((void**)&d_wmod, (size_t)std::max<int64_t>(M, 1) * sizeof(float2), nullptr));
+    int rc = NUFFT_OK;
+    const int nb_img = ew_blocks(p->nimg);
+    for (int blk = 0; blk < (1 << d) && rc == NUFFT_OK; ++blk) {
+        int h[3] = {0, 0, 0};
+        double shift[3] = {0.0, 0.0, 0.0};
+        for (int a = 0; a < d; ++a) { h[a] = (blk >> a) & 1; shift[a] = (h[a] - 0.5) * (double)p->N[a]; }
+        for (int64_t m = 0; m < M; ++m) {
+            double ph = 0.0;
+            for (int a = 0; a < d; ++a) ph += p->om_host[(size_t)m * d + a] * shift[a];
+            const double c = std::cos(ph), sn = std::sin(ph);
+            wmod[m] = make_float2((float)(wh[m].x * c - wh[m].y * sn), (float)(wh[m].x * sn + wh[m].y * c));
+        }
+        cudaError_t e = cudaMemcpyAsync(d_wmod, wmod.data(), (size_t)std::max<int64_t>(M, 1) * sizeof(float2), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);          // wmod is reused by the next block
+        if (e != cudaSuccess) { g_last_cuda_error = (int)e; rc = NUFFT_ECUDA; break; }
+        rc = adjoint_impl(p, 1, (const nufft_c64*)d_wmod, (nufft_c64*)p->d_dcf_img, st);
+        if (rc != NUFFT_OK) break;
+        psf_place_block_kernel<<<nb_img, 256, 0, st>>>(p->d_that, p->d_dcf_img, p->N[0], p->N[1], p->N[2], h[0], h[1], h[2]);
+        p->launches++;
+    }
     if (rc == NUFFT_OK) {
         const int nb = ew_blocks(p->cells);
-        psf_zero_planes_kernel<<<nb, 256, 0, st>>>(p->d_that, p->K[0], p->K[1], p->d == 3 ? p->K[2] : 1);
+        psf_zero_planes_kernel<<<nb, 256, 0, st>>>(p->d_that, p->K[0], p->K[1], d == 3 ? p->K[2] : 1);
         rc = fft_full_inplace(p, p->d_that, st);
-        if (rc == NUFFT_OK) psf_sign_kernel<<<nb, 256, 0, st>>>(p->d_that, p->K[0], p->K[1], p->d == 3 ? p->K[2] : 1,
+        if (rc == NUFFT_OK) psf_sign_kernel<<<nb, 256, 0, st>>>(p->d_that, p->K[0], p->K[1], d == 3 ? p->K[2] : 1,
                                                                    (float)(1.0 / (double)p->cells));
         p->launches += 2;
     }
-    cudaError_t e = cudaStreamSynchronize(st);      // the temporary plan and `ones` are released below
-    nufft_destroy(p2);
-    cudaFree(ones);
+    const cudaError_t e = cudaStreamSynchronize(st);
+    cudaFree(d_wmod);
     if (rc == NUFFT_OK && e != cudaSuccess) { g_last_cuda_error = (int)e; rc = NUFFT_ECUDA; }
+    if (rc == NUFFT_OK && cudaGetLastError() != cudaSuccess) rc = NUFFT_ECUDA;
     return rc;
 }
 

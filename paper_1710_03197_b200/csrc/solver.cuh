@@ -272,6 +272,19 @@ __global__ void __launch_bounds__(256) psf_zero_planes_kernel(float2* __restrict
         if (c0 == 0 || (K1 > 1 && c1 == 0) || (K2 > 1 && c2 == 0)) T[i] = make_float2(0.f, 0.f);
     }
 }
+// T[h N + n] = blk[n] per axis: one N^d block of the point-spread function into the (2N)^d array (R22)
+__global__ void __launch_bounds__(256)
+psf_place_block_kernel(float2* __restrict__ T, const float2* __restrict__ blk, int N0, int N1, int N2, int h0, int h1, int h2) {
+    const int64_t n = (int64_t)N0 * N1 * N2;
+    const int64_t K1 = 2 * (int64_t)N1, K2 = (N2 > 1) ? 2 * (int64_t)N2 : 1;
+    const int64_t K1e = (N1 > 1) ? K1 : 1;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int n2 = (int)(i % N2), n1 = (int)((i / N2) % N1), n0 = (int)(i / ((int64_t)N1 * N2));
+        const int64_t o = ((int64_t)(h0 * N0 + n0) * K1e + (h1 * N1 + n1)) * K2 + (h2 * N2 + n2);
+        T[o] = blk[i];
+    }
+}
+
 // T^[k] = sum_d T[d] e^{-2 pi i k d / K} = (-1)^{sum k_a} FFT(T2)[k]   (d = n - K/2 per axis), times `scale` = 1/prod(K):
 // the path's F^H is the unnormalised conjugate transpose (R5), so F^H(T^ . F z) carries a factor prod(K).
 __global__ void __launch_bounds__(256) psf_sign_kernel(float2* __restrict__ T, int K0, int K1, int K2, float scale) {

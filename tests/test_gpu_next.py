@@ -89,7 +89,7 @@ def test_toeplitz_selfadjoint(ci, scale, batch):
     p.destroy()
 
 
-def test_toeplitz_with_density_weights_and_unsupported_size():
+def test_toeplitz_with_density_weights_and_state_errors():
     import paper_1710_03197_b200 as nb
     cfg = wl.config(1, scale=4)
     Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
@@ -101,13 +101,25 @@ def test_toeplitz_with_density_weights_and_unsupported_size():
     That, _ = nxt.toeplitz_kernel(om, Nd, Kd, Jd, wo)
     assert rel(host(p.selfadjoint_toeplitz(dev(x)))[0], nxt.selfadjoint_toeplitz(x.astype(np.complex128), That, Nd)) < TOL
     p.destroy()
-    big = wl.config(2)                      # 512^2 image: the PSF would need a 2048 grid
-    q = make_plan(big)
+    q = make_plan(cfg)
     with pytest.raises(nb.NufftError):
-        q.toeplitz_build()
-    with pytest.raises(nb.NufftError):
-        q.toeplitz_enable(True)
+        q.toeplitz_enable(True)             # no spectrum built yet
     q.destroy()
+
+
+def test_toeplitz_config3_full_size():
+    """512^2 image / 1024^2 grid (BASELINE config 3): the PSF comes from four adjoint NUFFTs on the plan's own grid, so the
+    largest supported size works; A^H A in Toeplitz form against the oracle of the same embedding and the back-to-back one."""
+    cfg = wl.config(2)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    p = make_plan(cfg)
+    p.toeplitz_build()
+    x = wl.image_gaussian(Nd)
+    got = host(p.selfadjoint_toeplitz(dev(x)))[0]
+    That, _ = nxt.toeplitz_kernel(om, Nd, Kd, Jd)
+    assert rel(got, nxt.selfadjoint_toeplitz(x.astype(np.complex128), That, Nd)) < TOL
+    assert rel(got, orc.selfadjoint(x.astype(np.complex128), om, Nd, Kd, Jd)) < 1e-4
+    p.destroy()
 
 
 def test_cg_and_multicoil_with_toeplitz_operator():
