@@ -1209,6 +1209,7 @@ extern "C" int nufft_set_coils(nufft_plan_t p, int ncoil, const nufft_c64* c) {
     if (!p || ncoil < 0 || ncoil > p->max_batch || (ncoil > 0 && !c)) return NUFFT_EINVAL;
     p->ncoil = ncoil;
     p->d_coils = (ncoil > 0) ? (const float2*)c : nullptr;
+    if (p->cg_graph) { cudaGraphExecDestroy(p->cg_graph); p->cg_graph = nullptr; }   // the coil pointer is baked into it
     if (ncoil > 0 && !p->d_imgwork)
         NU_TRY(dev_alloc((void**)&p->d_imgwork, (size_t)p->max_batch * p->nimg * sizeof(float2), &p->bytes_work));
     return NUFFT_OK;
