@@ -208,6 +208,8 @@ int nufft_profile_reset(nufft_plan_t p);
 int nufft_profile_count(nufft_plan_t p);
 int nufft_profile_get(nufft_plan_t p, int i, const char **name, double *total_ms, int64_t *launches);
 
+/* Frees the plan, its device buffers, streams, events and cached graphs.  The caller must first synchronise every stream
+ * that still has work of this plan enqueued (the library does not wait).  Borrowed coil maps are not freed. */
 int nufft_destroy(nufft_plan_t p);
 
 const char *nufft_strerror(int code);
