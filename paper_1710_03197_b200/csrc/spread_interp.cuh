@@ -438,7 +438,7 @@ constexpr int k3Plane = k3P1 * k3Pitch;
 constexpr int k3Cells = k3P0 * k3Plane;                        // 4056 cells = 32448 B
 constexpr int k3Chunk = 128;                                   // samples whose weights are staged at a time
 constexpr int k3RecW = 28;                                     // floats per staged sample record
-constexpr int kInterp3dSmem = k3Cells * 8 + k3Chunk * k3RecW * 4;
+constexpr int kInterp3dSmem = k3Cells * 8 + k3Chunk * k3RecW * 4 + 16;
 
 __global__ void __launch_bounds__(256)
 interp_tiled_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ items, const float2* __restrict__ grid,
@@ -452,14 +452,24 @@ interp_tiled_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ it
     unpack_k0(wi.origin, o);
     const int K0 = g.K[0], K1 = g.K[1], K2 = g.K[2];
     const float2* __restrict__ G = grid + (int64_t)b * g.cells;
-    // stage the padded tile: 169 rows x 12 float4 (24 cells); rows and the 16-byte pairs wrap periodically
-    for (int idx = threadIdx.x; idx < k3P0 * k3P1 * (k3Pitch / 2); idx += blockDim.x) {
-        const int row = idx / (k3Pitch / 2), c4 = idx - row * (k3Pitch / 2);
-        const int lx = row / k3P1, ly = row - lx * k3P1;
-        const int gx = (o[0] + lx) & (K0 - 1), gy = (o[1] + ly) & (K1 - 1), gz = (o[2] + 2 * c4) & (K2 - 1);
-        reinterpret_cast<float4*>(tile)[idx] =
-            __ldg(reinterpret_cast<const float4*>(G + ((int64_t)gx * K1 + gy) * K2 + gz));
+    // stage the padded tile with bulk copies (cp.async.bulk + mbarrier, SASS UBLKCP): one 192-byte row (24 cells) per
+    // thread, rows wrap periodically, a row that crosses the seam of the last axis is split in two copies
+    uint64_t* bar = reinterpret_cast<uint64_t*>(recs + k3Chunk * k3RecW);
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_expect_tx(bar, (uint32_t)(k3P0 * k3P1 * k3Pitch * 8));
     }
+    __syncthreads();
+    for (int row = threadIdx.x; row < k3P0 * k3P1; row += blockDim.x) {
+        const int lx = row / k3P1, ly = row - lx * k3P1;
+        const int gx = (o[0] + lx) & (K0 - 1), gy = (o[1] + ly) & (K1 - 1), gz = o[2] & (K2 - 1);
+        const float2* src = G + ((int64_t)gx * K1 + gy) * K2;
+        float2* dst = tile + row * k3Pitch;
+        const int first = min(k3Pitch, K2 - gz);
+        bulk_g2s(dst, src + gz, (uint32_t)first * 8, bar);
+        if (first < k3Pitch) bulk_g2s(dst + first, src, (uint32_t)(k3Pitch - first) * 8, bar);
+    }
+    mbar_wait(bar, 0);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int half = lane >> 4, rr = (lane >> 3) & 1, cc = lane & 7;
     const int lane_off = rr * k3Pitch + cc;
