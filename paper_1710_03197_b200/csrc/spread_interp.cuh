@@ -375,6 +375,24 @@ gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
         }
     }
     __syncthreads();
+    if (!DET && tg.pitch * 8 % 16 == 0) {
+        // flush by the TMA engine: one bulk f32 reduce-add per padded row (rows wrap periodically; a row that crosses the
+        // seam of the last axis is split); the tile's untouched cells are zeros and add nothing
+        fence_proxy_async_smem();
+        float2* __restrict__ Gb = grid + (int64_t)b * g.cells;
+        const int rows = tg.P[0] * tg.P[1];
+        for (int row = threadIdx.x; row < rows; row += blockDim.x) {
+            const int lx = row / tg.P[1], ly = row - lx * tg.P[1];
+            const int gx = (o[0] + lx) & (g.K[0] - 1), gy = (o[1] + ly) & (g.K[1] - 1), gz = o[2] & (g.K[2] - 1);
+            float2* dst = Gb + ((int64_t)gx * g.K[1] + gy) * g.K[2];
+            const float2* src = tile + row * tg.pitch;
+            const int first = min(tg.pitch, g.K[2] - gz);
+            bulk_s2g_add_f32(dst + gz, src, (uint32_t)first * 8);
+            if (first < tg.pitch) bulk_s2g_add_f32(dst, src + first, (uint32_t)(tg.pitch - first) * 8);
+        }
+        bulk_commit_and_wait_read();      // shared memory must stay valid until the engine has read it
+        return;
+    }
     flush_tile<3, DET>(tile, tg, g, wi.origin, grid + (int64_t)b * g.cells,
                        DET ? slabs + (int64_t)b * slab_batch_stride + (int64_t)wi.slab * tg.tile_cells : nullptr,
                        threadIdx.x, blockDim.x);
