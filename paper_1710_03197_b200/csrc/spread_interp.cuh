@@ -275,6 +275,20 @@ gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
         apply_staged(tile, rowrec, colrec, cnt, lane);
         __syncwarp();
     }
+    if (!DET) {       // flush by the TMA engine: one bulk f32 reduce-add per padded row (split at the seam of axis 1)
+        fence_proxy_async_smem();
+        float2* __restrict__ Gb = grid + (int64_t)b * g.cells;
+        for (int row = lane; row < tg.P[0]; row += 32) {
+            const int gx = (o[0] + row) & (g.K[0] - 1), gz = o[1] & (g.K[1] - 1);
+            float2* dst = Gb + (int64_t)gx * g.K[1];
+            const float2* src = tile + row * tg.pitch;
+            const int first = min(tg.pitch, g.K[1] - gz);
+            bulk_s2g_add_f32(dst + gz, src, (uint32_t)first * 8);
+            if (first < tg.pitch) bulk_s2g_add_f32(dst, src + first, (uint32_t)(tg.pitch - first) * 8);
+        }
+        bulk_commit_and_wait_read();
+        return;
+    }
     flush_tile<2, DET>(tile, tg, g, wi.origin, grid + (int64_t)b * g.cells,
                        DET ? slabs + (int64_t)b * slab_batch_stride + (int64_t)wi.slab * tg.tile_cells : nullptr, lane, 32);
 }
