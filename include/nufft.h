@@ -17,8 +17,9 @@
  *     n_a - N_a/2 (R4).  Samples y are [batch][M] complex64 in the caller's sample order.  om is [M][d] float64,
  *     radians per image sample, axis a of om pairs with image axis a; values outside [-pi,pi) are wrapped.
  *   - forward sign e^{-i om.(n - N/2)}; adjoint is the exact conjugate transpose (no 1/prod(K) factor, R5).
- *   - interpolator: Kaiser-Bessel, width J = 6 grid cells, beta = pi sqrt((J/sigma)^2 (sigma-1/2)^2 - 0.8),
- *     sigma = K/N = 2, scaling factors 1/Phi (R1-R3); periodic grid (R7).
+ *   - interpolator: Kaiser-Bessel of width J grid cells ("interpolator size"; J = 6 is the paper's
+ *     workload and the tuned path), beta = pi sqrt((J/sigma)^2 (sigma-1/2)^2 - 0.8), sigma = K/N = 2, scaling factors
+ *     1/Phi (R1-R3); periodic grid (R7).
  *   - complex64 = two IEEE float32 (re, im), i.e. CUDA float2; declared here as nufft_c64 so that this header
  *     needs no CUDA include.  `stream` arguments are a cudaStream_t passed as void* (NULL = default stream).
  *   - POINTER KINDS.  "host" = ordinary host memory read during the call.  "device" = CUDA device memory,
@@ -29,8 +30,12 @@
  *     use one stream at a time per plan.  Distinct plans are independent.
  *   - outputs are overwritten, never accumulated into.  In-place (x_in == x_out) is allowed for selfadjoint.
  *   - supported: d in {1,2,3} (1-D: "1D signals"; planar path, atomic V^H only -- adjoint_mode = 1 is
- *     refused); Jd[a] == 6; Kd[a] == 2*Nd[a]; Kd[a] in {32,64,128,256,512,1024};
- *     1 <= batch <= max_batch.  Anything else -> NUFFT_EINVAL (there is no slow path and no CPU fallback).
+ *     refused); Jd[a] the same on every axis, 2 <= Jd <= 8 (odd widths included); Kd[a] == 2*Nd[a];
+ *     Kd[a] in {32,64,128,256,512,1024}; 1 <= batch <= max_batch.  Jd == 6 runs the tiled / batch-interleaved kernels;
+ *     every other width runs the direct V (one thread per sample, prod(J) gathered loads) and the atomic V^H (one
+ *     vector atomic per stencil point into a zeroed grid), planar layout at every batch size, adjoint_mode = 1
+ *     refused; all transforms, solvers, density weights and the Toeplitz form work on such plans.
+ *     Anything else -> NUFFT_EINVAL (there is no CPU fallback).
  */
 #ifndef NUFFT_B200_H
 #define NUFFT_B200_H
@@ -69,7 +74,9 @@ typedef struct {
                                CALLER's sample order and writes y directly when the trajectory is coherent (>= 90 % of
                                consecutive samples within two grid cells: radial spokes, spiral arms);
                            1 = the plain variants: direct gather in 3-D, sorted walk + layout pass on the interleaved
-                               path (kept for cross-checks)                                                        */
+                               path (kept for cross-checks);
+                           2 = the generic-width kernels (direct V, atomic V^H, planar) even at Jd = 6: what a plan
+                               with Jd != 6 runs, selectable at Jd = 6 for cross-checks against the tuned kernels   */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
     int use_graphs;     /* 1 = CUDA-graph replay of launch-bound work on a non-default stream (the legacy stream cannot

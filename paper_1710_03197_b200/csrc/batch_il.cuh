@@ -273,11 +273,15 @@ y_to_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y, fl
     if (m0 >= M) return;
     const int cnt = (int)min((int64_t)32, M - m0);
     const int my = (lane < cnt) ? __ldg(&pos[m0 + lane]) : 0;
-#pragma unroll 8
+    // all 32 row loads of the warp are issued before the first one is consumed (the pass is latency-bound otherwise)
+    float2 v[kIL];
+#pragma unroll
     for (int l = 0; l < kIL; ++l) {
         const int b = grp * kIL + l;
-        tile[warp][lane][l] = (lane < cnt && b < batch) ? __ldg(&y[(int64_t)b * M + m0 + lane]) : make_float2(0.f, 0.f);
+        v[l] = (lane < cnt && b < batch) ? __ldg(&y[(int64_t)b * M + m0 + lane]) : make_float2(0.f, 0.f);
     }
+#pragma unroll
+    for (int l = 0; l < kIL; ++l) tile[warp][lane][l] = v[l];
     __syncwarp();
     float2* __restrict__ dst = y_il + (int64_t)grp * M * kIL + lane;
     for (int k = 0; k < cnt; ++k) {

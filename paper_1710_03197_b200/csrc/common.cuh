@@ -16,7 +16,9 @@ __host__ __device__ __forceinline__ float2 cscale(float2 a, float s) { return ma
 // a * (-i)
 __host__ __device__ __forceinline__ float2 cmul_mi(float2 a) { return make_float2(a.y, -a.x); }
 
-constexpr int kJ = 6;          // interpolation kernel width in grid cells (Jd), the one supported value
+constexpr int kJ = 6;          // interpolation kernel width in grid cells (Jd) of the tuned (tiled / interleaved) kernels
+constexpr int kJmin = 2;       // other widths kJmin..kJmax run on the direct V / atomic V^H kernels
+constexpr int kJmax = 8;
 constexpr int kPolyDeg = 9;    // degree of the piecewise polynomial fit of the Kaiser-Bessel kernel
 constexpr int kPolyHalf = 5;   // even / odd coefficient count ((kPolyDeg + 1) / 2)
 
@@ -44,6 +46,32 @@ __device__ __forceinline__ void kb_weights(const KernelPoly& P, float delta, flo
         o *= z;
         w[j] = e + o;
         w[kJ - 1 - j] = e - o;
+    }
+    if (delta == 0.0f) w[0] = 0.0f;
+}
+
+// Any width J in [kJmin, kJmax]: ceil(J/2) even/odd pairs, phi_{J-1-j}(z) = phi_j(-z) (for odd J the middle piece is its
+// own mirror image).  With J = 6 and KernelPoly this is kb_weights above.
+struct KernelPolyG {
+    float ev[(kJmax + 1) / 2][kPolyHalf];
+    float od[(kJmax + 1) / 2][kPolyHalf];
+};
+
+template <int J, class Poly>
+__device__ __forceinline__ void kb_weights_j(const Poly& P, float delta, float (&w)[J]) {
+    const float z = fmaf(2.0f, delta, -1.0f);
+    const float z2 = z * z;
+#pragma unroll
+    for (int j = 0; j < (J + 1) / 2; ++j) {
+        float e = P.ev[j][kPolyHalf - 1], o = P.od[j][kPolyHalf - 1];
+#pragma unroll
+        for (int c = kPolyHalf - 2; c >= 0; --c) {
+            e = fmaf(e, z2, P.ev[j][c]);
+            o = fmaf(o, z2, P.od[j][c]);
+        }
+        o *= z;
+        w[j] = e + o;
+        if (J - 1 - j != j) w[J - 1 - j] = e - o;
     }
     if (delta == 0.0f) w[0] = 0.0f;
 }

@@ -49,7 +49,10 @@ struct nufft_plan_s {
     int64_t M = 0, nimg = 0, cells = 0;
     int max_batch = 1;
     nufft_opts opts{};
+    int J = kJ;                     // kernel width (uniform over the axes); J != kJ runs the direct V / atomic V^H kernels
     KernelPoly poly{};
+    KernelPolyG polyg{};            // J != kJ
+    bool generic_j = false;         // J != kJ, or opts.interp_mode == 2 (the same kernels at J = kJ, for cross-checks)
     double poly_err = 0.0;
     // device plan data
     float* d_scale[3] = {nullptr, nullptr, nullptr};
@@ -363,10 +366,34 @@ static SampleData sample_data(nufft_plan_t p) {
     return s;
 }
 
+// Widths other than kJ: direct V and atomic V^H, one instantiation per (d, J)
+#define NU_J_CASES(KERNEL, D, ...)                                                             \
+    switch (p->J) {                                                                            \
+    case 2: KERNEL<D, 2, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    case 3: KERNEL<D, 3, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    case 4: KERNEL<D, 4, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    case 5: KERNEL<D, 5, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    case 6: KERNEL<D, 6, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    case 7: KERNEL<D, 7, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    case 8: KERNEL<D, 8, KernelPolyG><<<blocks, 128, 0, st>>>(__VA_ARGS__); break;             \
+    default: return NUFFT_EINVAL;                                                              \
+    }
+#define NU_DJ_CASES(KERNEL, ...)                                                               \
+    if (p->d == 1) { NU_J_CASES(KERNEL, 1, __VA_ARGS__) }                                      \
+    else if (p->d == 2) { NU_J_CASES(KERNEL, 2, __VA_ARGS__) }                                 \
+    else { NU_J_CASES(KERNEL, 3, __VA_ARGS__) }
+
 // a3: y = V grid
 static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, cudaStream_t st) {
     if (p->M == 0) return NUFFT_OK;
     ProfScope ps(p, "interp", st);
+    if (p->generic_j) {
+        const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
+        NU_DJ_CASES(interp_direct_kernel, sample_data(p), grid_geom(p), grid, y, p->polyg)
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+        return NUFFT_OK;
+    }
     if (p->d == 3 && p->opts.interp_mode == 0 && p->tile[0] == k3T0 && p->tile[1] == k3T1 && p->tile[2] == k3T2 && p->n_items > 0) {
         // tile-staged V (default tile only); interp_mode = 1 keeps the direct gather
         const dim3 tb((unsigned)p->n_items, (unsigned)batch);
@@ -393,6 +420,15 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
     const bool det = p->opts.adjoint_mode == 1;
     if (p->M == 0 || p->n_items == 0) {
         CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st));
+        return NUFFT_OK;
+    }
+    if (p->generic_j) {
+        { ProfScope pz(p, "grid_zero", st); CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st)); }
+        ProfScope ps(p, "gridding", st);
+        const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
+        NU_DJ_CASES(gridding_atomic_kernel, sample_data(p), grid_geom(p), y, grid, p->polyg)
+        CU_TRY(cudaGetLastError());
+        p->launches++;
         return NUFFT_OK;
     }
     const int64_t slab_stride = (int64_t)p->n_items * p->tg.tile_cells;
@@ -747,9 +783,10 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
 
 static int plan_build(nufft_plan_t p, const double* om) {
     const int d = p->d;
-    const double J = (double)kJ;
+    const double J = (double)p->J;
     // kernel polynomial, scaling vectors, twiddles (float64 on the host, rounded once)
-    p->poly = host::fit_kernel_poly(J, 2.0, &p->poly_err);
+    if (p->generic_j) p->polyg = host::fit_kernel_poly_g(p->J, 2.0, &p->poly_err);
+    else p->poly = host::fit_kernel_poly(J, 2.0, &p->poly_err);
     for (int a = 0; a < d; ++a) {
         NU_TRY(dev_upload(&p->d_scale[a], host::scaling_vector(p->N[a], p->K[a], J), &p->bytes_plan));
         NU_TRY(dev_upload(&p->d_tw[a], host::twiddle_table(p->K[a]), &p->bytes_plan));
@@ -881,12 +918,15 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     if (!out || !Nd || !Kd || !Jd || (d < 1 || d > 3) || M < 0 || (M > 0 && !om) || max_batch < 1) return NUFFT_EINVAL;
     if (M > (int64_t)0x7fffffff) return NUFFT_EINVAL;
     for (int a = 0; a < d; ++a) {
-        if (Jd[a] != kJ || !supported_K(Kd[a]) || Kd[a] != 2 * Nd[a]) return NUFFT_EINVAL;
+        if (Jd[a] != Jd[0] || Jd[a] < kJmin || Jd[a] > kJmax || Jd[a] > Kd[a] || !supported_K(Kd[a]) || Kd[a] != 2 * Nd[a])
+            return NUFFT_EINVAL;
     }
-    if (d == 1 && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;      // 1-D V^H is the atomic kernel only
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
-                 opts->interp_mode > 1 || opts->batch_layout < 0 || opts->batch_layout > 2))
+                 opts->interp_mode > 2 || opts->batch_layout < 0 || opts->batch_layout > 2))
         return NUFFT_EINVAL;
+    const bool generic_j = Jd[0] != kJ || (opts && opts->interp_mode == 2);
+    // 1-D and the generic-width path have the atomic V^H only
+    if ((d == 1 || generic_j) && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;
     static cudaError_t cfg = configure_all();
     if (cfg != cudaSuccess) { g_last_cuda_error = (int)cfg; return NUFFT_ECUDA; }
     nufft_plan_t p = new (std::nothrow) nufft_plan_s();
@@ -896,7 +936,9 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     p->max_batch = max_batch;
     if (opts) p->opts = *opts;
     p->il_min_batch = (p->opts.batch_layout == 2) ? 2 : kIlMinBatch;
-    p->il_ok = (d == 2) && max_batch >= p->il_min_batch && p->opts.batch_layout != 1 && Kd[1] >= 2 * kBandW;
+    p->J = Jd[0];
+    p->generic_j = generic_j;
+    p->il_ok = (d == 2) && !generic_j && max_batch >= p->il_min_batch && p->opts.batch_layout != 1 && Kd[1] >= 2 * kBandW;
     p->batch_pad = p->il_ok ? ((max_batch + kIL - 1) / kIL) * kIL : max_batch;
     p->nimg = 1; p->cells = 1;
     for (int a = 0; a < d; ++a) {
@@ -1607,11 +1649,11 @@ extern "C" int nufft_solve_cg_kspace(nufft_plan_t p, const nufft_c64* y, nufft_c
     if (!p->d_kspace) NU_TRY(dev_alloc((void**)&p->d_kspace, (size_t)5 * n * sizeof(float2), &p->bytes_work));
     if (!p->d_sinv[0]) {
         for (int a = 0; a < p->d; ++a) {
-            std::vector<float> s = host::scaling_vector(p->N[a], p->K[a], (double)kJ);
+            std::vector<float> s = host::scaling_vector(p->N[a], p->K[a], (double)p->J);
             // 1 / (s K): computed in float64 from the float64 scaling factor, rounded once
-            const double beta = host::kb_beta((double)kJ, (double)p->K[a] / (double)p->N[a]);
+            const double beta = host::kb_beta((double)p->J, (double)p->K[a] / (double)p->N[a]);
             for (int i = 0; i < p->N[a]; ++i)
-                s[i] = (float)(host::kb_Phi(((double)i - 0.5 * p->N[a]) / (double)p->K[a], (double)kJ, beta) / (double)p->K[a]);
+                s[i] = (float)(host::kb_Phi(((double)i - 0.5 * p->N[a]) / (double)p->K[a], (double)p->J, beta) / (double)p->K[a]);
             NU_TRY(dev_upload(&p->d_sinv[a], s, &p->bytes_plan));
         }
     }

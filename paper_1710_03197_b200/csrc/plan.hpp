@@ -68,14 +68,14 @@ inline std::vector<float2> twiddle_table(int K) {
 }
 
 // Degree-kPolyDeg polynomial interpolant (Chebyshev nodes, float64) of phi_j(z) = phi(J/2 - (z+1)/2 - j), z in
-// [-1,1], j = 0,1,2, converted to the monomial basis and split into even / odd parts (see common.cuh KernelPoly).
-// Returns the max abs fit error over a fine mesh (over all six pieces) in *max_err.
-inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {
+// [-1,1], j = 0 .. npieces-1, converted to the monomial basis and split into even / odd parts (see common.cuh
+// KernelPoly / KernelPolyG).  Returns the max abs fit error over a fine mesh (over all pieces) in *max_err.
+inline void fit_kernel_pieces(double J, double sigma, int npieces, float (*ev)[kPolyHalf], float (*od)[kPolyHalf],
+                              double* max_err) {
     const double beta = kb_beta(J, sigma);
     constexpr int n = kPolyDeg + 1;
-    KernelPoly P;
     double worst = 0.0;
-    for (int j = 0; j < 3; ++j) {
+    for (int j = 0; j < npieces; ++j) {
         auto f = [&](double z) { return kb_phi(0.5 * J - 0.5 * (z + 1.0) - (double)j, J, beta); };
         // Chebyshev coefficients from values at the n Chebyshev-Gauss nodes
         double fx[n], c[n];
@@ -95,7 +95,7 @@ inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {
             for (int i = 0; i < n; ++i) Tn[i] = (i > 0 ? 2.0 * Tk[i - 1] : 0.0) - Tkm1[i];
             for (int i = 0; i < n; ++i) { mono[i] += c[k] * Tn[i]; Tkm1[i] = Tk[i]; Tk[i] = Tn[i]; }
         }
-        for (int h = 0; h < kPolyHalf; ++h) { P.ev[j][h] = (float)mono[2 * h]; P.od[j][h] = (float)mono[2 * h + 1]; }
+        for (int h = 0; h < kPolyHalf; ++h) { ev[j][h] = (float)mono[2 * h]; od[j][h] = (float)mono[2 * h + 1]; }
         for (int i = 0; i <= 2000; ++i) {
             const double z = -1.0 + i * 1e-3;
             double v = 0.0;
@@ -105,6 +105,15 @@ inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {
         }
     }
     if (max_err) *max_err = worst;
+}
+inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {      // J = kJ: three pairs
+    KernelPoly P;
+    fit_kernel_pieces(J, sigma, kJ / 2, P.ev, P.od, max_err);
+    return P;
+}
+inline KernelPolyG fit_kernel_poly_g(int J, double sigma, double* max_err) {      // any J in [kJmin, kJmax]
+    KernelPolyG P{};
+    fit_kernel_pieces((double)J, sigma, (J + 1) / 2, P.ev, P.od, max_err);
     return P;
 }
 

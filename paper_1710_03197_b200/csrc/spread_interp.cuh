@@ -28,24 +28,26 @@ __device__ __forceinline__ void unpack_k0(uint32_t kp, int (&k0)[3]) {
 // ------------------------------------------------------------------------------------------------------------
 // V, direct form: one thread per sample (tile-sorted order, so a warp's stencils share cache lines), the prod(J)
 // stencil values gathered straight from the grid through L1/L2.  y is written in the caller's order.
+// J is a template parameter: widths other than kJ (SURVEY 8(f)-4 "other Jd") run on this kernel and on
+// gridding_atomic_kernel below with a KernelPolyG.
 // ------------------------------------------------------------------------------------------------------------
-template <int D>
+template <int D, int J = kJ, class Poly = KernelPoly>
 __global__ void __launch_bounds__(128)
-interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, float2* __restrict__ y, KernelPoly P) {
+interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, float2* __restrict__ y, Poly P) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.M) return;
     const int b = blockIdx.y;
     int k0[3];
     unpack_k0(__ldg(&s.kpack[i]), k0);
-    float w[D][kJ];
+    float w[D][J];
 #pragma unroll
-    for (int a = 0; a < D; ++a) kb_weights(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
+    for (int a = 0; a < D; ++a) kb_weights_j<J>(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
     const float2* __restrict__ G = grid + (int64_t)b * g.cells;
     float2 acc = make_float2(0.f, 0.f);
     if (D == 1) {
         const int K0 = g.K[0];
 #pragma unroll
-        for (int j0 = 0; j0 < kJ; ++j0) {
+        for (int j0 = 0; j0 < J; ++j0) {
             const float2 v = __ldg(&G[(k0[0] + j0) & (K0 - 1)]);
             acc.x = fmaf(w[0][j0], v.x, acc.x);
             acc.y = fmaf(w[0][j0], v.y, acc.y);
@@ -53,11 +55,11 @@ interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, 
     } else if (D == 2) {
         const int K0 = g.K[0], K1 = g.K[1];
 #pragma unroll
-        for (int j0 = 0; j0 < kJ; ++j0) {
+        for (int j0 = 0; j0 < J; ++j0) {
             const float2* __restrict__ row = G + (int64_t)((k0[0] + j0) & (K0 - 1)) * K1;
             float2 r = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int j1 = 0; j1 < kJ; ++j1) {
+            for (int j1 = 0; j1 < J; ++j1) {
                 const float2 v = __ldg(&row[(k0[1] + j1) & (K1 - 1)]);
                 r.x = fmaf(w[1][j1], v.x, r.x);
                 r.y = fmaf(w[1][j1], v.y, r.y);
@@ -68,15 +70,15 @@ interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, 
     } else {
         const int K0 = g.K[0], K1 = g.K[1], K2 = g.K[2];
 #pragma unroll 1
-        for (int j0 = 0; j0 < kJ; ++j0) {
+        for (int j0 = 0; j0 < J; ++j0) {
             const float2* __restrict__ plane = G + (int64_t)((k0[0] + j0) & (K0 - 1)) * K1 * K2;
             float2 rp = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int j1 = 0; j1 < kJ; ++j1) {
+            for (int j1 = 0; j1 < J; ++j1) {
                 const float2* __restrict__ row = plane + (int64_t)((k0[1] + j1) & (K1 - 1)) * K2;
                 float2 r = make_float2(0.f, 0.f);
 #pragma unroll
-                for (int j2 = 0; j2 < kJ; ++j2) {
+                for (int j2 = 0; j2 < J; ++j2) {
                     const float2 v = __ldg(&row[(k0[2] + j2) & (K2 - 1)]);
                     r.x = fmaf(w[D - 1][j2], v.x, r.x);
                     r.y = fmaf(w[D - 1][j2], v.y, r.y);
@@ -96,44 +98,44 @@ interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, 
 // V^H, baseline form: one thread per sample, one vector atomic (red.global.add.v2.f32) per stencil point into a
 // zeroed grid.  Kept as the simple fallback / cross-check of the tiled kernels.
 // ------------------------------------------------------------------------------------------------------------
-template <int D>
+template <int D, int J = kJ, class Poly = KernelPoly>
 __global__ void __launch_bounds__(128)
-gridding_atomic_kernel(SampleData s, GridGeom g, const float2* __restrict__ y, float2* __restrict__ grid, KernelPoly P) {
+gridding_atomic_kernel(SampleData s, GridGeom g, const float2* __restrict__ y, float2* __restrict__ grid, Poly P) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.M) return;
     const int b = blockIdx.y;
     int k0[3];
     unpack_k0(__ldg(&s.kpack[i]), k0);
-    float w[D][kJ];
+    float w[D][J];
 #pragma unroll
-    for (int a = 0; a < D; ++a) kb_weights(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
+    for (int a = 0; a < D; ++a) kb_weights_j<J>(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
     const float2 yv = __ldg(&y[(int64_t)b * g.M + __ldg(&s.perm[i])]);
     float2* __restrict__ G = grid + (int64_t)b * g.cells;
     if (D == 1) {
         const int K0 = g.K[0];
 #pragma unroll
-        for (int j0 = 0; j0 < kJ; ++j0) atomicAdd(&G[(k0[0] + j0) & (K0 - 1)], cscale(yv, w[0][j0]));
+        for (int j0 = 0; j0 < J; ++j0) atomicAdd(&G[(k0[0] + j0) & (K0 - 1)], cscale(yv, w[0][j0]));
     } else if (D == 2) {
         const int K0 = g.K[0], K1 = g.K[1];
 #pragma unroll
-        for (int j0 = 0; j0 < kJ; ++j0) {
+        for (int j0 = 0; j0 < J; ++j0) {
             float2* __restrict__ row = G + (int64_t)((k0[0] + j0) & (K0 - 1)) * K1;
             const float2 yr = cscale(yv, w[0][j0]);
 #pragma unroll
-            for (int j1 = 0; j1 < kJ; ++j1) atomicAdd(&row[(k0[1] + j1) & (K1 - 1)], cscale(yr, w[1][j1]));
+            for (int j1 = 0; j1 < J; ++j1) atomicAdd(&row[(k0[1] + j1) & (K1 - 1)], cscale(yr, w[1][j1]));
         }
     } else {
         const int K0 = g.K[0], K1 = g.K[1], K2 = g.K[2];
 #pragma unroll 1
-        for (int j0 = 0; j0 < kJ; ++j0) {
+        for (int j0 = 0; j0 < J; ++j0) {
             float2* __restrict__ plane = G + (int64_t)((k0[0] + j0) & (K0 - 1)) * K1 * K2;
             const float2 yp = cscale(yv, w[0][j0]);
 #pragma unroll
-            for (int j1 = 0; j1 < kJ; ++j1) {
+            for (int j1 = 0; j1 < J; ++j1) {
                 float2* __restrict__ row = plane + (int64_t)((k0[1] + j1) & (K1 - 1)) * K2;
                 const float2 yr = cscale(yp, w[1][j1]);
 #pragma unroll
-                for (int j2 = 0; j2 < kJ; ++j2) atomicAdd(&row[(k0[2] + j2) & (K2 - 1)], cscale(yr, w[D - 1][j2]));
+                for (int j2 = 0; j2 < J; ++j2) atomicAdd(&row[(k0[2] + j2) & (K2 - 1)], cscale(yr, w[D - 1][j2]));
             }
         }
     }
