@@ -560,6 +560,29 @@ def extra_legs(nb, torch, peak, args):
         "coil_pairs_per_s": 32 * 1e3 / (fwc_ms + adc_ms),
         "note": "n_outer=4, n_inner=5, n_cg=3, mu=1, lam=0.02 (R17); 32-coil batch on the interleaved grid"}
     p.destroy()
+    # the paper's own experiment shape (512^2 image, non-Cartesian k-space of its ref. [15]) on a synthetic
+    # PROPELLER stand-in, batch 1: the operations of Table 1, whose workload the paper does not state
+    cfg = wl.config_propeller()
+    pp = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1)
+    xt = torch.from_numpy(wl.phantom(cfg["Nd"])).cuda().reshape(1, *cfg["Nd"])
+    yp = pp.forward(xt)
+    xop = pp.adjoint(yp)
+    for _ in range(3):
+        pp.forward(xt, yp), pp.adjoint(yp, xop), pp.selfadjoint(xt, xop)
+    xs = pp.solve_cg(yp, 2)
+    xl = pp.solve_l1tv_ols(yp, 1.0, 0.02, 1, 1, 1)
+    xd = pp.solve_l1tv_lad(yp, 1.0, 0.02, 1, 1, 1)
+    out["paper_2_3_propeller_512"] = {
+        "workload": "Nd=512^2 Kd=1024^2 Jd=6^2, PROPELLER 24 blades x 32 lines x 512 (M=393216), batch 1, synthetic",
+        "forward_ms": time_calls(lambda: pp.forward(xt, yp), 10, flush),
+        "adjoint_ms": time_calls(lambda: pp.adjoint(yp, xop), 10, flush),
+        "selfadjoint_ms": time_calls(lambda: pp.selfadjoint(xt, xop), 10, flush),
+        "cg_20it_ms": time_calls(lambda: pp.solve_cg(yp, 20, x=xs), 3, flush),
+        "l1tv_ols_20it_ms": time_calls(lambda: pp.solve_l1tv_ols(yp, 1.0, 0.02, 4, 5, 3, x=xl), 3, flush),
+        "l1tv_lad_20it_ms": time_calls(lambda: pp.solve_l1tv_lad(yp, 1.0, 0.02, 4, 5, 3, x=xd), 3, flush),
+        "paper_table1_k80_pycuda": "A 6 ms, A^H 6 ms, A^H A 8 ms; CG 1.89 s, L1TV-OLS 1.68 s, L1TV-LAD 1.78 s "
+                                   "(PAPER.md:299-305; sizes and iteration counts not stated: context only)"}
+    pp.destroy()
     # cuFFT reference point for F alone (never linked into the product): full 512^2 FFT of 64 grids via torch.fft
     gref = torch.randn(64, 512, 512, dtype=torch.complex64, device="cuda")
     torch.fft.fftn(gref, dim=(1, 2))

@@ -122,6 +122,12 @@ def test_config2_full_radial_256():
     check_transforms(wl.config(1))
 
 
+def test_propeller_paper_experiment_shape():
+    """PROPELLER stand-in for the paper's own 512^2 experiment, at 128^2 for the oracle."""
+    cfg = wl.config_propeller(scale=4)
+    check_transforms(cfg)
+
+
 def test_config2_phantom_variant():
     cfg = wl.config(1)
     p = make_plan(cfg)
@@ -385,6 +391,11 @@ def test_interleaved_coherent_caller_order_interp_matches_sorted_path():
     assert rel(yc[39], yo) < TOL
     pc.destroy()
     ps.destroy()
+
+
+def test_interleaved_propeller_batch20():
+    """The PROPELLER stand-in on the interleaved path (coherent along each readout line, jumps between lines)."""
+    check_batched(wl.config_propeller(scale=4), 20, [0, 19])
 
 
 def test_interleaved_config1_ragged_batch40():

@@ -283,3 +283,14 @@ def test_workload_generators_shapes_and_ranges():
     assert wl.config(0)["om"][0].tolist() == wl.config(0)["om"][0].tolist()      # seeded
     ph = wl.phantom((64, 64))
     assert ph.dtype == np.complex64 and len(np.unique(ph.real)) < 200
+    # PROPELLER stand-in for the paper's own experiment: blades are rotated copies of a Cartesian strip
+    cfg = wl.config_propeller()
+    assert cfg["Nd"] == (512, 512) and cfg["om"].shape == (24 * 32 * 512, 2)
+    om = cfg["om"].reshape(24, 32, 512, 2)
+    dk = 2 * np.pi / 512
+    assert np.allclose(np.diff(om[0, :, :, 0], axis=1), dk) and np.allclose(np.diff(om[0, :, :, 1], axis=0), dk)
+    r0 = np.linalg.norm(om[0], axis=-1)
+    for b in (1, 7, 23):
+        assert np.allclose(np.linalg.norm(om[b], axis=-1), r0)                   # rotation keeps the radius
+        ang = np.arctan2(om[b, 16, 300, 1], om[b, 16, 300, 0]) - np.arctan2(om[0, 16, 300, 1], om[0, 16, 300, 0])
+        assert np.isclose((ang - np.pi * b / 24 + np.pi) % (2 * np.pi) - np.pi, 0.0, atol=1e-9)

@@ -124,6 +124,33 @@ def traj_spiral_vd(nleaves, npts, nturns=8.0):
     return om.reshape(-1, 2)
 
 
+def traj_propeller(nblades, nlines, nread, N):
+    """2-D PROPELLER: nblades rectangular strips through the origin, blade b rotated by pi b / nblades; a blade has
+    nlines parallel readouts of nread points, line spacing and readout spacing 2 pi / N (Nyquist for an N-pixel image).
+    Synthetic stand-in for the non-Cartesian k-space of the paper's brain simulation (its ref. [15]),
+    which is not in this container.  Sample order: blade, line, readout point."""
+    dk = 2.0 * np.pi / float(N)
+    kx = (np.arange(nread, dtype=np.float64) - nread / 2.0) * dk
+    ky = (np.arange(nlines, dtype=np.float64) - (nlines - 1) / 2.0) * dk
+    om = np.empty((nblades, nlines, nread, 2), dtype=np.float64)
+    for b in range(nblades):
+        th = np.pi * b / nblades
+        c, s_ = np.cos(th), np.sin(th)
+        om[b, :, :, 0] = c * kx[None, :] - s_ * ky[:, None]
+        om[b, :, :, 1] = s_ * kx[None, :] + c * ky[:, None]
+    return om.reshape(-1, 2)
+
+
+def config_propeller(scale=1):
+    """The paper's own experiment shape (512 x 512 image, non-Cartesian k-space of ref. [15]): Nd = 512^2,
+    Kd = 1024^2, Jd = 6, PROPELLER with 24 blades x 32 lines x 512 readout points (M = 393216).  Not a BASELINE config:
+    bench context leg and one parity case."""
+    s = int(scale)
+    N = 512 // s
+    return dict(name="paper_2_3_propeller", Nd=(N, N), Kd=(2 * N, 2 * N), Jd=(6, 6),
+                om=traj_propeller(max(24 // s, 3), max(32 // s, 2), N, N), ncoil=0)
+
+
 def traj_kooshball(nspokes, nread, seed=SEED_KOOSH):
     """3-D radial kooshball: spokes through the origin, directions by spiral phyllotaxis on the upper hemisphere."""
     rng = np.random.default_rng(seed)
