@@ -119,13 +119,14 @@ def _offsets(Jd):
     return np.ndindex(*[int(j) for j in Jd])
 
 
-def interp(G, om, Nd, Kd, Jd):
+def interp(G, om, Nd, Kd, Jd, st=None):
     """V:  y[m] = sum_j  prod_a w_a[m, j_a] * G[(k0 + j) mod K].
 
-    G has shape Kd (C order).  Returns y[M] complex128.
+    G has shape Kd (C order).  Returns y[M] complex128.  st: per-axis (idx, w) lists from another real, separable
+    interpolator (oracle/minmax_oracle.py); default = the Kaiser-Bessel stencils of this module.
     """
     G = np.asarray(G, dtype=np.complex128)
-    st = _stencils(om, Nd, Kd, Jd)
+    st = _stencils(om, Nd, Kd, Jd) if st is None else st
     M = st[0][0].shape[0]
     y = np.zeros(M, dtype=np.complex128)
     for j in _offsets(Jd):
@@ -138,13 +139,13 @@ def interp(G, om, Nd, Kd, Jd):
     return y
 
 
-def grid_adjoint(y, om, Nd, Kd, Jd):
+def grid_adjoint(y, om, Nd, Kd, Jd, st=None):
     """V^H:  G[(k0 + j) mod K] += prod_a w_a[m, j_a] * y[m]   over all m, j.
 
-    The weights are real, so the conjugate transpose of V has the same weights.  Returns G of shape Kd.
+    The weights are real, so the conjugate transpose of V has the same weights.  Returns G of shape Kd.  st as in interp.
     """
     y = np.asarray(y, dtype=np.complex128)
-    st = _stencils(om, Nd, Kd, Jd)
+    st = _stencils(om, Nd, Kd, Jd) if st is None else st
     M = y.shape[0]
     size = int(np.prod(Kd))
     Gr = np.zeros(size)
