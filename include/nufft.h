@@ -91,6 +91,14 @@ typedef struct {
                                (lanes = images; V^H in gather form with register accumulators, deterministic),
                                smaller batches and 3-D use the planar grid [batch][K0][K1]([K2]);
                            1 = always planar;  2 = interleaved for every batch >= 2 (for measuring the crossover)  */
+    int kernel;         /* interpolator ("the default kernel is the min-max kernel [5], other kernel
+                               functions can be used"; the paper prints no formula -- DESIGN.md readings R1, R25):
+                           0 = Kaiser-Bessel window (reading R1; the library default and the BASELINE configs);
+                           1 = min-max interpolator with the Kaiser-Bessel scaling factors: per sample
+                               and axis the J REAL weights that minimise the worst-case error over unit-norm images,
+                               T w = r(delta) (reading R25).  Same S, F, F^H, S^H and the same kernels: only the weight
+                               polynomial (and the float64 V^H table) differ, so every call works unchanged.  Needs the
+                               same Nd on every axis (the weights depend on N), else NUFFT_EINVAL                     */
 } nufft_opts;
 
 int nufft_default_opts(nufft_opts *o);

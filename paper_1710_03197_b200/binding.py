@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = [
 class NufftOpts(_c.Structure):
     _fields_ = [("coef_mode", _c.c_int), ("adjoint_mode", _c.c_int), ("interp_mode", _c.c_int),
                 ("tile", _c.c_int * 3), ("max_subtile", _c.c_int), ("use_graphs", _c.c_int),
-                ("batch_layout", _c.c_int)]
+                ("batch_layout", _c.c_int), ("kernel", _c.c_int)]
 
 
 class NufftError(RuntimeError):
@@ -137,7 +137,7 @@ class NufftPlan:
     """
 
     def __init__(self, Nd, Kd, Jd, om, max_batch=1, adjoint_mode=0, interp_mode=0, tile=None, max_subtile=0,
-                 batch_layout=0, use_graphs=0):
+                 batch_layout=0, use_graphs=0, kernel="kb"):
         L = lib()
         self.Nd = tuple(int(n) for n in Nd)
         self.Kd = tuple(int(k) for k in Kd)
@@ -158,6 +158,7 @@ class NufftPlan:
         opts.max_subtile = int(max_subtile)
         opts.batch_layout = int(batch_layout)
         opts.use_graphs = int(use_graphs)
+        opts.kernel = {"kb": 0, "minmax": 1}[kernel]
         if tile is not None:
             for a, t in enumerate(tile):
                 opts.tile[a] = int(t)

@@ -28,6 +28,7 @@ constexpr int kPolyHalf = 5;   // even / odd coefficient count ((kPolyDeg + 1) /
 struct KernelPoly {
     float ev[3][kPolyHalf];
     float od[3][kPolyHalf];
+    float zero_at;     // delta at which w[0] is exactly zero: 0 for Kaiser-Bessel (open support, R6), -1 (never) for min-max
 };
 
 // Six interpolation weights of one axis: w[j] = phi(J/2 - delta - j).
@@ -47,7 +48,7 @@ __device__ __forceinline__ void kb_weights(const KernelPoly& P, float delta, flo
         w[j] = e + o;
         w[kJ - 1 - j] = e - o;
     }
-    if (delta == 0.0f) w[0] = 0.0f;
+    if (delta == P.zero_at) w[0] = 0.0f;
 }
 
 // Any width J in [kJmin, kJmax]: ceil(J/2) even/odd pairs, phi_{J-1-j}(z) = phi_j(-z) (for odd J the middle piece is its
@@ -55,6 +56,7 @@ __device__ __forceinline__ void kb_weights(const KernelPoly& P, float delta, flo
 struct KernelPolyG {
     float ev[(kJmax + 1) / 2][kPolyHalf];
     float od[(kJmax + 1) / 2][kPolyHalf];
+    float zero_at;
 };
 
 template <int J, class Poly>
@@ -73,7 +75,7 @@ __device__ __forceinline__ void kb_weights_j(const Poly& P, float delta, float (
         w[j] = e + o;
         if (J - 1 - j != j) w[J - 1 - j] = e - o;
     }
-    if (delta == 0.0f) w[0] = 0.0f;
+    if (delta == P.zero_at) w[0] = 0.0f;
 }
 
 #ifdef __CUDACC__

@@ -53,6 +53,8 @@ struct nufft_plan_s {
     KernelPoly poly{};
     KernelPolyG polyg{};            // J != kJ
     bool generic_j = false;         // J != kJ, or opts.interp_mode == 2 (the same kernels at J = kJ, for cross-checks)
+    bool minmax = false;            // opts.kernel == 1: min-max interpolator (reading R25); only the weight polynomials
+    host::MinMaxKernel mm;          //   and the float64 V^H table differ from the Kaiser-Bessel plan
     double poly_err = 0.0;
     // device plan data
     float* d_scale[3] = {nullptr, nullptr, nullptr};
@@ -709,8 +711,8 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
     for (int64_t i = 0; i < M; ++i) {
         const int64_t m = perm_h[i];
         double w0[kJ], w1[kJ];
-        host::kb_weights_f64(delta64[m], J, beta, w0);
-        host::kb_weights_f64(delta64[M + m], J, beta, w1);
+        if (p->minmax) { p->mm.weights(delta64[m], w0); p->mm.weights(delta64[M + m], w1); }
+        else { host::kb_weights_f64(delta64[m], J, beta, w0); host::kb_weights_f64(delta64[M + m], J, beta, w1); }
         float* rec = &wtab[(size_t)i * kTabW];
         for (int j = 0; j < kJ; ++j) rec[j] = (float)w0[j];
         const int32_t r = row_of(kpack[m]);
@@ -785,7 +787,11 @@ static int plan_build(nufft_plan_t p, const double* om) {
     const int d = p->d;
     const double J = (double)p->J;
     // kernel polynomial, scaling vectors, twiddles (float64 on the host, rounded once)
-    if (p->generic_j) p->polyg = host::fit_kernel_poly_g(p->J, 2.0, &p->poly_err);
+    if (p->minmax) {
+        p->mm.build(p->N[0], p->K[0], p->J);
+        if (p->generic_j) p->polyg = p->mm.fit<KernelPolyG>(&p->poly_err);
+        else p->poly = p->mm.fit<KernelPoly>(&p->poly_err);
+    } else if (p->generic_j) p->polyg = host::fit_kernel_poly_g(p->J, 2.0, &p->poly_err);
     else p->poly = host::fit_kernel_poly(J, 2.0, &p->poly_err);
     for (int a = 0; a < d; ++a) {
         NU_TRY(dev_upload(&p->d_scale[a], host::scaling_vector(p->N[a], p->K[a], J), &p->bytes_plan));
@@ -922,8 +928,13 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
             return NUFFT_EINVAL;
     }
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
-                 opts->interp_mode > 2 || opts->batch_layout < 0 || opts->batch_layout > 2))
+                 opts->interp_mode > 2 || opts->batch_layout < 0 || opts->batch_layout > 2 || opts->kernel < 0 ||
+                 opts->kernel > 1))
         return NUFFT_EINVAL;
+    // the min-max weights depend on N (through the scaling factors): one weight polynomial serves all axes only if they
+    // have the same size
+    if (opts && opts->kernel == 1)
+        for (int a = 1; a < d; ++a) if (Nd[a] != Nd[0]) return NUFFT_EINVAL;
     const bool generic_j = Jd[0] != kJ || (opts && opts->interp_mode == 2);
     // 1-D and the generic-width path have the atomic V^H only
     if ((d == 1 || generic_j) && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;
@@ -938,6 +949,7 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     p->il_min_batch = (p->opts.batch_layout == 2) ? 2 : kIlMinBatch;
     p->J = Jd[0];
     p->generic_j = generic_j;
+    p->minmax = p->opts.kernel == 1;
     p->il_ok = (d == 2) && !generic_j && max_batch >= p->il_min_batch && p->opts.batch_layout != 1 && Kd[1] >= 2 * kBandW;
     p->batch_pad = p->il_ok ? ((max_batch + kIL - 1) / kIL) * kIL : max_batch;
     p->nimg = 1; p->cells = 1;

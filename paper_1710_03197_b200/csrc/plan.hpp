@@ -67,19 +67,17 @@ inline std::vector<float2> twiddle_table(int K) {
     return t;
 }
 
-// Degree-kPolyDeg polynomial interpolant (Chebyshev nodes, float64) of phi_j(z) = phi(J/2 - (z+1)/2 - j), z in
-// [-1,1], j = 0 .. npieces-1, converted to the monomial basis and split into even / odd parts (see common.cuh
+// Degree-kPolyDeg polynomial interpolant (Chebyshev nodes, float64) of the kernel pieces f(j, z), z in [-1,1]
+// (z = 2 delta - 1), j = 0 .. npieces-1, converted to the monomial basis and split into even / odd parts (see common.cuh
 // KernelPoly / KernelPolyG).  Returns the max abs fit error over a fine mesh (over all pieces) in *max_err.
-inline void fit_kernel_pieces(double J, double sigma, int npieces, float (*ev)[kPolyHalf], float (*od)[kPolyHalf],
-                              double* max_err) {
-    const double beta = kb_beta(J, sigma);
+template <class F>
+inline void fit_pieces(F f, int npieces, float (*ev)[kPolyHalf], float (*od)[kPolyHalf], double* max_err) {
     constexpr int n = kPolyDeg + 1;
     double worst = 0.0;
     for (int j = 0; j < npieces; ++j) {
-        auto f = [&](double z) { return kb_phi(0.5 * J - 0.5 * (z + 1.0) - (double)j, J, beta); };
         // Chebyshev coefficients from values at the n Chebyshev-Gauss nodes
         double fx[n], c[n];
-        for (int i = 0; i < n; ++i) fx[i] = f(std::cos(kPi * (i + 0.5) / n));
+        for (int i = 0; i < n; ++i) fx[i] = f(j, std::cos(kPi * (i + 0.5) / n));
         for (int k = 0; k < n; ++k) {
             double acc = 0.0;
             for (int i = 0; i < n; ++i) acc += fx[i] * std::cos(kPi * k * (i + 0.5) / n);
@@ -100,14 +98,22 @@ inline void fit_kernel_pieces(double J, double sigma, int npieces, float (*ev)[k
             const double z = -1.0 + i * 1e-3;
             double v = 0.0;
             for (int k = n - 1; k >= 0; --k) v = v * z + mono[k];
-            const double e = std::fabs(v - f(z));
+            const double e = std::fabs(v - f(j, z));
             if (e > worst) worst = e;
         }
     }
     if (max_err) *max_err = worst;
 }
+
+// Kaiser-Bessel pieces: phi_j(z) = phi(J/2 - (z+1)/2 - j)
+inline void fit_kernel_pieces(double J, double sigma, int npieces, float (*ev)[kPolyHalf], float (*od)[kPolyHalf],
+                              double* max_err) {
+    const double beta = kb_beta(J, sigma);
+    fit_pieces([&](int j, double z) { return kb_phi(0.5 * J - 0.5 * (z + 1.0) - (double)j, J, beta); }, npieces, ev, od,
+               max_err);
+}
 inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {      // J = kJ: three pairs
-    KernelPoly P;
+    KernelPoly P{};
     fit_kernel_pieces(J, sigma, kJ / 2, P.ev, P.od, max_err);
     return P;
 }
@@ -116,6 +122,90 @@ inline KernelPolyG fit_kernel_poly_g(int J, double sigma, double* max_err) {    
     fit_kernel_pieces((double)J, sigma, (J + 1) / 2, P.ev, P.od, max_err);
     return P;
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// Min-max interpolator with Kaiser-Bessel scaling factors ("the default kernel is the min-max kernel";
+// SURVEY 8(f)-4; reading R25): for stencil offsets t_l = J/2 - delta - l the J real weights solve
+//     T w = r(delta),   T[l][j] = sum_p c_p s_p^2 cos(gamma (l - j) p),   r[l] = sum_p c_p s_p cos(gamma t_l p),
+// p = -N/2 .. N/2 with c = 1/2 at both ends (= the image's own N pixels, the summands being even), s_p = 1 / Phi(p / K).
+// The weights are analytic in delta: they are sampled once per plan at 32 Chebyshev nodes (32 solves) and every later
+// evaluation -- the float64 V^H table and the fit of the device polynomial -- goes through that interpolant.
+// ------------------------------------------------------------------------------------------------------------
+struct MinMaxKernel {
+    static constexpr int kNodes = 32;
+    int J = 0;
+    double cheb[kJmax][kNodes];      // Chebyshev coefficients of w_j(z), z = 2 delta - 1
+
+    void build(int N, int K, int Jw) {
+        J = Jw;
+        const double beta = kb_beta((double)J, (double)K / (double)N), gam = 2.0 * kPi / (double)K;
+        const int np = N + 1;
+        std::vector<double> pp(np), cs(np), css(np);
+        for (int i = 0; i < np; ++i) {
+            pp[i] = (double)(i - N / 2);
+            const double sv = 1.0 / kb_Phi(pp[i] / (double)K, (double)J, beta);
+            const double c = (i == 0 || i == np - 1) ? 0.5 : 1.0;
+            cs[i] = c * sv;
+            css[i] = c * sv * sv;
+        }
+        double T[kJmax][kJmax];
+        for (int l = 0; l < J; ++l)
+            for (int j = 0; j < J; ++j) {
+                double acc = 0.0;
+                for (int i = 0; i < np; ++i) acc += css[i] * std::cos(gam * (double)(l - j) * pp[i]);
+                T[l][j] = acc;
+            }
+        double wn[kNodes][kJmax];
+        for (int q = 0; q < kNodes; ++q) {
+            const double z = std::cos(kPi * (q + 0.5) / kNodes), delta = 0.5 * (z + 1.0);
+            double A[kJmax][kJmax + 1];
+            for (int l = 0; l < J; ++l) {
+                const double t = 0.5 * J - delta - (double)l;
+                double acc = 0.0;
+                for (int i = 0; i < np; ++i) acc += cs[i] * std::cos(gam * t * pp[i]);
+                for (int j = 0; j < J; ++j) A[l][j] = T[l][j];
+                A[l][J] = acc;
+            }
+            // Gaussian elimination with partial pivoting (T is symmetric positive definite, cond <= 1e5 for J <= 8)
+            for (int c = 0; c < J; ++c) {
+                int piv = c;
+                for (int r2 = c + 1; r2 < J; ++r2) if (std::fabs(A[r2][c]) > std::fabs(A[piv][c])) piv = r2;
+                if (piv != c) for (int k = 0; k <= J; ++k) std::swap(A[c][k], A[piv][k]);
+                for (int r2 = c + 1; r2 < J; ++r2) {
+                    const double f = A[r2][c] / A[c][c];
+                    for (int k = c; k <= J; ++k) A[r2][k] -= f * A[c][k];
+                }
+            }
+            for (int r2 = J - 1; r2 >= 0; --r2) {
+                double acc = A[r2][J];
+                for (int k = r2 + 1; k < J; ++k) acc -= A[r2][k] * wn[q][k];
+                wn[q][r2] = acc / A[r2][r2];
+            }
+        }
+        for (int j = 0; j < J; ++j)
+            for (int k = 0; k < kNodes; ++k) {
+                double acc = 0.0;
+                for (int q = 0; q < kNodes; ++q) acc += wn[q][j] * std::cos(kPi * k * (q + 0.5) / kNodes);
+                cheb[j][k] = (k == 0 ? 1.0 : 2.0) * acc / kNodes;
+            }
+    }
+    // w_j at z = 2 delta - 1 (Clenshaw)
+    double eval(int j, double z) const {
+        double b1 = 0.0, b2 = 0.0;
+        for (int k = kNodes - 1; k >= 1; --k) { const double b0 = 2.0 * z * b1 - b2 + cheb[j][k]; b2 = b1; b1 = b0; }
+        return z * b1 - b2 + cheb[j][0];
+    }
+    void weights(double delta, double* w) const {
+        const double z = 2.0 * delta - 1.0;
+        for (int j = 0; j < J; ++j) w[j] = eval(j, z);
+    }
+    template <class Poly> Poly fit(double* max_err) const {
+        Poly P{};
+        fit_pieces([&](int j, double z) { return eval(j, z); }, (J + 1) / 2, P.ev, P.od, max_err);
+        P.zero_at = -1.0f;        // no open-support zero: the weight at t = J/2 is whatever the least-squares solution gives
+        return P;
+    }
+};
 
 // Per-sample split of the coordinate, in float64 (reading R6/R11):
 //   u = om * (K / (2 pi));  k0 = ceil(u - J/2);  delta = k0 - (u - J/2) in [0,1);  returns k0 mod K.
