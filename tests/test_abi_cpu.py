@@ -43,7 +43,19 @@ def test_strerror_and_arg_validation_without_gpu():
     Jd_bad = (ctypes.c_int * 2)(4, 6)
     Kd_bad = (ctypes.c_int64 * 2)(96, 128)
     assert L.nufft_plan(4, Nd, Kd, Jd, 0, None, 1, None, ctypes.byref(h)) == -1          # d
-    assert L.nufft_plan(2, Nd, Kd, Jd_bad, 0, None, 1, None, ctypes.byref(h)) == -1      # Jd
+    assert L.nufft_plan(2, Nd, Kd, Jd_bad, 0, None, 1, None, ctypes.byref(h)) == -1      # Jd not uniform
+    for j in (1, 9):                                                                      # Jd outside 2..8
+        assert L.nufft_plan(2, Nd, Kd, (ctypes.c_int * 2)(j, j), 0, None, 1, None, ctypes.byref(h)) == -1
+    from paper_1710_03197_b200.binding import NufftOpts
+    o = NufftOpts()
+    assert L.nufft_default_opts(ctypes.byref(o)) == 0 and o.kernel == 0 and o.adjoint_mode == 0
+    o.kernel = 2                                                                          # unknown interpolator
+    assert L.nufft_plan(2, Nd, Kd, Jd, 0, None, 1, ctypes.byref(o), ctypes.byref(h)) == -1
+    o.kernel = 1                                                                          # min-max needs equal Nd (R25)
+    Nd_r, Kd_r = (ctypes.c_int64 * 2)(64, 32), (ctypes.c_int64 * 2)(128, 64)
+    assert L.nufft_plan(2, Nd_r, Kd_r, Jd, 0, None, 1, ctypes.byref(o), ctypes.byref(h)) == -1
+    o.kernel, o.adjoint_mode = 0, 1                                                       # deterministic V^H is J = 6 only
+    assert L.nufft_plan(2, Nd, Kd, (ctypes.c_int * 2)(4, 4), 0, None, 1, ctypes.byref(o), ctypes.byref(h)) == -1
     assert L.nufft_plan(2, Nd, Kd_bad, Jd, 0, None, 1, None, ctypes.byref(h)) == -1      # Kd != 2 Nd / not pow2
     assert L.nufft_plan(2, Nd, Kd, Jd, 0, None, 0, None, ctypes.byref(h)) == -1          # max_batch
     assert L.nufft_plan(2, Nd, Kd, Jd, 5, None, 1, None, ctypes.byref(h)) == -1          # om null with M > 0
