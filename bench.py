@@ -315,6 +315,20 @@ def run_ours(args):
     rows = kernel_table(plan.profile(), algorithmic_bytes(2, Nd[0], Kd[0], M, B), peak)
     plan.profile_enable(False)
 
+    # forward, adjoint and A^H A alone (north star: absolute transforms/s and fraction of the HBM roofline), same batch,
+    # L2 flushed between calls; A^H A keeps y on the device in the interleaved layout (no layout pass either way)
+    ab = algorithmic_bytes(2, Nd[0], Kd[0], M, B)
+    fwd_bytes = ab["fft_rows_fwd"] + ab["fft_cols_fwd"] + ab["interp"]
+    adj_bytes = ab["gridding"] + ab["fft_cols_adj"] + ab["fft_rows_adj"]
+    transforms = {}
+    for name, fn, nbytes in (("forward", lambda: plan.forward(x, y), fwd_bytes),
+                             ("adjoint", lambda: plan.adjoint(y, xo), adj_bytes),
+                             ("selfadjoint", lambda: plan.selfadjoint(x, xo), fwd_bytes + adj_bytes)):
+        fn()
+        ms = timed(fn, K_steps) / K_steps
+        transforms[name] = {"transforms_per_s": world * B / (ms * 1e-3), "ms_per_call": ms, "alg_bytes_per_call": int(nbytes),
+                            "frac_of_hbm_roofline": (nbytes / (ms * 1e-3) / 1e9) / peak}
+
     result = None
     if rank == 0:
         ms_per_step = total_ms / K_steps
@@ -364,6 +378,7 @@ def run_ours(args):
                             "H2D / kernels / D2H"},
             "gpu_launches": int(l1 - l0),
             "roofline": roofline,
+            "transforms": transforms,
             "cpu_baseline": {"value": 1.0 / cpu_s, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
                              "sample": "%d forward+adjoint pairs on one image of the workload (batch element 0)" % cpu_n},
             "paper_context": "PAPER.md Table 1 (:299-300): forward 6 ms + adjoint 6 ms on one K80 GK210 (PyCUDA), "
