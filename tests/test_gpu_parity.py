@@ -281,6 +281,32 @@ def test_multicoil_operator():
     assert rel(host(p.selfadjoint_coils(dev(x))), so) < TOL
 
 
+@pytest.mark.parametrize("Nd,M,nc", [((16, 16, 16), 5003, 4), ((64,), 301, 3), ((32, 16, 32), 9001, 5)])
+def test_multicoil_operator_3d_and_1d(Nd, M, nc):
+    """eqs. (34)-(35) on the planar 3-D and 1-D paths (coil multiply fused into S / S^H, coil_sum_kernel), and CG on
+    A_multi^H A_multi x = A_multi^H y."""
+    cfg = custom_cfg(Nd, M, seed=77)
+    Kd, Jd, om = cfg["Kd"], cfg["Jd"], cfg["om"]
+    rng = np.random.default_rng(78)
+    c = rng.standard_normal((nc,) + tuple(Nd)) + 1j * rng.standard_normal((nc,) + tuple(Nd))
+    c = (c / np.sqrt(np.sum(np.abs(c) ** 2, axis=0, keepdims=True))).astype(np.complex64)
+    p = make_plan(cfg, max_batch=nc)
+    p.set_coils(dev(c))
+    x = wl.image_gaussian(Nd)
+    y = wl.data_gaussian(M, batch=nc)
+    c128 = c.astype(np.complex128)
+    yo = orc.forward_coils(x.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    xo = orc.adjoint_coils(y.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    so = orc.adjoint_coils(yo, c128, om, Nd, Kd, Jd)
+    assert rel(host(p.forward_coils(dev(x))), yo) < TOL
+    assert rel(host(p.adjoint_coils(dev(y))), xo) < TOL
+    assert rel(host(p.selfadjoint_coils(dev(x))), so) < TOL
+    AHA = lambda z: orc.selfadjoint_coils(z, c128, om, Nd, Kd, Jd)
+    xc, _ = sol.cg(AHA, xo, 3)
+    assert rel(host(p.solve_cg(dev(y), 3, use_coils=True)), xc) < 1e-4
+    p.destroy()
+
+
 # ---------------------------------------------------------------------------------------------------------
 # solvers
 # ---------------------------------------------------------------------------------------------------------
