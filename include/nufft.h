@@ -211,6 +211,13 @@ int nufft_solve_cg_kspace(nufft_plan_t p, const nufft_c64 *y, nufft_c64 *x, int 
 int nufft_plan_info(nufft_plan_t p, int64_t *bytes_plan, int64_t *bytes_work,
                     int64_t *n_tiles, int64_t *n_work, int64_t *max_tile_samples);
 
+/* Modes the plan chose (SURVEY 8(b) "modes chosen").  Any pointer may be NULL.  J = kernel width; kernel = 0
+ * Kaiser-Bessel / 1 min-max (opts.kernel); paths = bit mask: 1 = the batch-interleaved 2-D path serves calls with batch >=
+ * its threshold, 2 = its V walks the caller's sample order (trajectory-coherent plan), 4 = the generic-width kernels (direct
+ * V, atomic V^H) serve the plan, 8 = the Toeplitz operator is enabled; poly_err = max abs error of the degree-9 float32
+ * weight polynomial the kernels evaluate against the float64 kernel it was fitted to (weights are <= 1). */
+int nufft_plan_modes(nufft_plan_t p, int *J, int *kernel, int *paths, double *poly_err);
+
 /* Number of kernel launches the library has enqueued for this plan since creation (bench.py's gpu_launches). */
 int64_t nufft_launch_count(nufft_plan_t p);
 

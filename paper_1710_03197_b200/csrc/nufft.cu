@@ -1011,6 +1011,15 @@ extern "C" int nufft_plan_info(nufft_plan_t p, int64_t* bytes_plan, int64_t* byt
     return NUFFT_OK;
 }
 
+extern "C" int nufft_plan_modes(nufft_plan_t p, int* J, int* kernel, int* paths, double* poly_err) {
+    if (!p) return NUFFT_EINVAL;
+    if (J) *J = p->J;
+    if (kernel) *kernel = p->minmax ? 1 : 0;
+    if (paths) *paths = (p->il_ok ? 1 : 0) | (p->il_ok && p->il_coherent ? 2 : 0) | (p->generic_j ? 4 : 0) | (p->toep_on ? 8 : 0);
+    if (poly_err) *poly_err = p->poly_err;
+    return NUFFT_OK;
+}
+
 extern "C" int64_t nufft_launch_count(nufft_plan_t p) { return p ? p->launches : -1; }
 
 static void prof_drain(nufft_plan_t p) {

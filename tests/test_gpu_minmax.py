@@ -123,3 +123,22 @@ def test_minmax_cg_and_toeplitz_consistency():
     x = wl.image_gaussian(Nd)[None]
     assert rel(host(p.selfadjoint_toeplitz(dev(x))), host(p.selfadjoint(dev(x)))) < 1e-4
     p.destroy()
+
+
+def test_plan_modes_report_what_the_plan_chose():
+    import paper_1710_03197_b200 as nb
+    cfg = dict(wl.config(1, scale=2))                         # radial: coherent
+    p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=16)
+    i = p.info()
+    assert i["J"] == 6 and i["kernel"] == "kb" and i["interleaved"] and i["caller_order_interp"]
+    assert not i["generic_width_kernels"] and not i["toeplitz"] and 0 < i["poly_err"] < 1e-7
+    p.toeplitz_build()
+    p.toeplitz_enable(True)
+    assert p.info()["toeplitz"]
+    p.destroy()
+    cfg = rand_cfg((32, 32), 500, J=4)
+    p = make_plan(cfg, max_batch=16)
+    i = p.info()
+    assert i["J"] == 4 and i["kernel"] == "minmax" and i["generic_width_kernels"] and not i["interleaved"]
+    assert 0 < i["poly_err"] < 1e-7
+    p.destroy()
