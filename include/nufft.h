@@ -30,8 +30,11 @@
  *     use one stream at a time per plan.  Distinct plans are independent.
  *   - outputs are overwritten, never accumulated into.  In-place (x_in == x_out) is allowed for selfadjoint.
  *   - supported: d in {1,2,3} (1-D: "1D signals"; planar path, atomic V^H only -- adjoint_mode = 1 is
- *     refused); Jd[a] the same on every axis, 2 <= Jd <= 8 (odd widths included); Kd[a] == 2*Nd[a];
- *     Kd[a] in {32,64,128,256,512,1024}; 1 <= batch <= max_batch.  Jd == 6 runs the tiled / batch-interleaved kernels;
+ *     refused); Jd[a] the same on every axis, 2 <= Jd <= 8 (odd widths included);
+ *     Kd[a] in {32,64,128,256,512,1024}; Nd[a] even, 2 <= Nd[a] < Kd[a], the same ratio Kd[a]/Nd[a] on every axis;
+ *     1 <= batch <= max_batch.  Kd == 2 Nd (the paper's and every BASELINE config's ratio) runs the pruned, fused FFT passes;
+ *     any other ratio runs S + zero-pad and crop + S^H as separate kernels around the unpruned FFT, planar layout, and has
+ *     no Toeplitz form (nufft_toeplitz_build -> NUFFT_EINVAL); everything else works unchanged.  Jd == 6 runs the tiled / batch-interleaved kernels;
  *     every other width runs the direct V (one thread per sample, prod(J) gathered loads) and the atomic V^H (one
  *     vector atomic per stencil point into a zeroed grid), planar layout at every batch size, adjoint_mode = 1
  *     refused; all transforms, solvers, density weights and the Toeplitz form work on such plans.

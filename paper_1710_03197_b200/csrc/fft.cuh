@@ -380,4 +380,67 @@ fft_rows_full_kernel(float2* __restrict__ data, const float2* __restrict__ tw, i
     fft_line<K, false, false>(q0, active, lay, tw, ld, st);
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Oversampling ratios other than 2 (SURVEY 8(f)-4 "other sigma"): any even N < K.  The pruned passes above hard-wire
+// K = 2 N (the zero half is a radix digit), so these plans run S + zero-pad and crop + S^H as separate elementwise
+// kernels around the UNPRUNED in-place FFT (fft_rows_full_kernel, fft_cols_kernel<K, false, true>).  Functional, not
+// tuned.  F^H needs no conjugation pass: sum_k g_k e^{+i gamma k p} = FFT(g)[(-p) mod K].
+// ------------------------------------------------------------------------------------------------------------
+struct PadGeom {
+    int d;
+    int N[3], K[3];
+    const float* s[3];       // scaling vectors per axis (length N[a])
+};
+
+// a1: grid[b][k] = prod_a s_a[n_a] (c_b[n]) x[n] at k_a = (n_a - N_a/2) mod K_a, zero elsewhere (every cell is written)
+__global__ void __launch_bounds__(256)
+pad_scale_kernel(PadGeom P, const float2* __restrict__ x, const float2* __restrict__ coil, float2* __restrict__ grid,
+                 int64_t cells, int64_t nimg, int same_image) {
+    const int b = blockIdx.y;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cells; i += (int64_t)gridDim.x * blockDim.x) {
+        int64_t r = i, idx = 0, mul = 1;
+        float sc = 1.0f;
+        bool inside = true;
+        for (int a = P.d - 1; a >= 0; --a) {
+            const int k = (int)(r % P.K[a]);
+            r /= P.K[a];
+            const int h = P.N[a] / 2;
+            const int n = (k < h) ? k + h : ((k >= P.K[a] - h) ? k - P.K[a] + h : -1);
+            if (n < 0) { inside = false; break; }
+            sc *= __ldg(&P.s[a][n]);
+            idx += (int64_t)n * mul;
+            mul *= P.N[a];
+        }
+        float2 v = make_float2(0.f, 0.f);
+        if (inside) {
+            v = __ldg(&x[(same_image ? 0 : (int64_t)b * nimg) + idx]);
+            if (coil) v = cmul(v, __ldg(&coil[(int64_t)b * nimg + idx]));
+            v = cscale(v, sc);
+        }
+        grid[(int64_t)b * cells + i] = v;
+    }
+}
+
+// a6 after the forward FFT of the gridded data: x[b][n] = prod_a s_a[n_a] conj(c_b[n]) G[b][(-(n - N/2)) mod K]
+__global__ void __launch_bounds__(256)
+crop_scale_kernel(PadGeom P, const float2* __restrict__ G, const float2* __restrict__ coil, float2* __restrict__ x,
+                  int64_t cells, int64_t nimg) {
+    const int b = blockIdx.y;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nimg; i += (int64_t)gridDim.x * blockDim.x) {
+        int64_t r = i, cell = 0, mul = 1;
+        float sc = 1.0f;
+        for (int a = P.d - 1; a >= 0; --a) {
+            const int n = (int)(r % P.N[a]);
+            r /= P.N[a];
+            const int k = (P.N[a] / 2 - n) & (P.K[a] - 1);       // (-(n - N/2)) mod K, K a power of two
+            sc *= __ldg(&P.s[a][n]);
+            cell += (int64_t)k * mul;
+            mul *= P.K[a];
+        }
+        float2 v = cscale(G[(int64_t)b * cells + cell], sc);
+        if (coil) v = cmul(v, cconj(__ldg(&coil[(int64_t)b * nimg + i])));
+        x[(int64_t)b * nimg + i] = v;
+    }
+}
+
 }  // namespace nufft

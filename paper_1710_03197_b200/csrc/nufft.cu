@@ -53,6 +53,7 @@ struct nufft_plan_s {
     KernelPoly poly{};
     KernelPolyG polyg{};            // J != kJ
     bool generic_j = false;         // J != kJ, or opts.interp_mode == 2 (the same kernels at J = kJ, for cross-checks)
+    bool generic_sigma = false;     // Kd != 2 Nd: unpruned FFT + separate pad / crop kernels, planar, direct or tiled V / V^H
     bool minmax = false;            // opts.kernel == 1: min-max interpolator (reading R25); only the weight polynomials
     host::MinMaxKernel mm;          //   and the float64 V^H table differ from the Kaiser-Bessel plan
     double poly_err = 0.0;
@@ -281,10 +282,32 @@ static RowPassParams row_params(nufft_plan_t p, int batch, const float2* img_in,
     return r;
 }
 
+static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int batch = 1);
+static PadGeom pad_geom(nufft_plan_t p) {
+    PadGeom g{};
+    g.d = p->d;
+    for (int a = 0; a < 3; ++a) {
+        g.N[a] = p->N[a]; g.K[a] = p->K[a];
+        g.s[a] = p->unit_scale ? p->d_ones : (p->inv_scale ? p->d_sinv[a] : p->d_scale[a]);
+    }
+    return g;
+}
+static int ew_blocks(int64_t n);
+
 // a1 + a2: grid = F S x  (coil != nullptr: grid_b = F S (c_b . x))
 static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* grid, const float2* coil,
                          bool same_image, cudaStream_t st) {
     const int d = p->d;
+    if (p->generic_sigma) {      // sigma != 2: pad kernel + unpruned FFT
+        {
+            ProfScope ps(p, "pad_scale", st);
+            pad_scale_kernel<<<dim3((unsigned)ew_blocks(p->cells), (unsigned)batch), 256, 0, st>>>(pad_geom(p), x, coil, grid, p->cells, p->nimg, same_image ? 1 : 0);
+            CU_TRY(cudaGetLastError());
+            p->launches++;
+        }
+        ProfScope ps(p, "fft_full_fwd", st);
+        return fft_full_inplace(p, grid, st, batch);
+    }
     RowPassParams r = row_params(p, batch, x, nullptr, grid, coil, same_image);
     { ProfScope ps(p, "fft_rows_fwd", st); NU_TRY(dispatch_rows(p->K[d - 1], false, r, st)); }
     p->launches++;
@@ -318,6 +341,14 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
 // a5 + a6: x = S^H F^H grid  (grid destroyed; coil != nullptr: x_b = conj(c_b) . S^H F^H grid_b)
 static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
     const int d = p->d;
+    if (p->generic_sigma) {      // sigma != 2: unpruned FFT, then crop at the reversed index (= F^H) + S^H
+        { ProfScope ps(p, "fft_full_adj", st); NU_TRY(fft_full_inplace(p, grid, st, batch)); }
+        ProfScope ps(p, "crop_scale", st);
+        crop_scale_kernel<<<dim3((unsigned)ew_blocks(p->nimg), (unsigned)batch), 256, 0, st>>>(pad_geom(p), grid, coil, x, p->cells, p->nimg);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+        return NUFFT_OK;
+    }
     if (d == 1) {
         // the Toeplitz spectrum multiply normally rides on the first adjoint column pass; 1-D has none
         if (p->cur_mult) {
@@ -786,13 +817,14 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
 static int plan_build(nufft_plan_t p, const double* om) {
     const int d = p->d;
     const double J = (double)p->J;
+    const double sigma = (double)p->K[0] / (double)p->N[0];      // the same on every axis (checked by nufft_plan)
     // kernel polynomial, scaling vectors, twiddles (float64 on the host, rounded once)
     if (p->minmax) {
         p->mm.build(p->N[0], p->K[0], p->J);
         if (p->generic_j) p->polyg = p->mm.fit<KernelPolyG>(&p->poly_err);
         else p->poly = p->mm.fit<KernelPoly>(&p->poly_err);
-    } else if (p->generic_j) p->polyg = host::fit_kernel_poly_g(p->J, 2.0, &p->poly_err);
-    else p->poly = host::fit_kernel_poly(J, 2.0, &p->poly_err);
+    } else if (p->generic_j) p->polyg = host::fit_kernel_poly_g(p->J, sigma, &p->poly_err);
+    else p->poly = host::fit_kernel_poly(J, sigma, &p->poly_err);
     for (int a = 0; a < d; ++a) {
         NU_TRY(dev_upload(&p->d_scale[a], host::scaling_vector(p->N[a], p->K[a], J), &p->bytes_plan));
         NU_TRY(dev_upload(&p->d_tw[a], host::twiddle_table(p->K[a]), &p->bytes_plan));
@@ -924,9 +956,11 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     if (!out || !Nd || !Kd || !Jd || (d < 1 || d > 3) || M < 0 || (M > 0 && !om) || max_batch < 1) return NUFFT_EINVAL;
     if (M > (int64_t)0x7fffffff) return NUFFT_EINVAL;
     for (int a = 0; a < d; ++a) {
-        if (Jd[a] != Jd[0] || Jd[a] < kJmin || Jd[a] > kJmax || Jd[a] > Kd[a] || !supported_K(Kd[a]) || Kd[a] != 2 * Nd[a])
-            return NUFFT_EINVAL;
+        if (Jd[a] != Jd[0] || Jd[a] < kJmin || Jd[a] > kJmax || Jd[a] > Kd[a] || !supported_K(Kd[a])) return NUFFT_EINVAL;
+        // any even N < K, with the same oversampling ratio on every axis (one kernel shape beta(J, sigma) for all axes)
+        if (Nd[a] < 2 || (Nd[a] & 1) || Nd[a] >= Kd[a] || Kd[a] * Nd[0] != Kd[0] * Nd[a]) return NUFFT_EINVAL;
     }
+    const bool generic_sigma = Kd[0] != 2 * Nd[0];
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
                  opts->interp_mode > 2 || opts->batch_layout < 0 || opts->batch_layout > 2 || opts->kernel < 0 ||
                  opts->kernel > 1))
@@ -950,7 +984,8 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     p->J = Jd[0];
     p->generic_j = generic_j;
     p->minmax = p->opts.kernel == 1;
-    p->il_ok = (d == 2) && !generic_j && max_batch >= p->il_min_batch && p->opts.batch_layout != 1 && Kd[1] >= 2 * kBandW;
+    p->generic_sigma = generic_sigma;
+    p->il_ok = (d == 2) && !generic_j && !generic_sigma && max_batch >= p->il_min_batch && p->opts.batch_layout != 1 && Kd[1] >= 2 * kBandW;
     p->batch_pad = p->il_ok ? ((max_batch + kIL - 1) / kIL) * kIL : max_batch;
     p->nimg = 1; p->cells = 1;
     for (int a = 0; a < d; ++a) {
@@ -1383,12 +1418,12 @@ template <int K> static void launch_cols_full(const ColPassParams& c, cudaStream
     }
 
 // in-place unpruned forward FFT of a planar K^d array (used once per plan for the Toeplitz spectrum)
-static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st) {
+static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int batch) {
     const int d = p->d;
     const int64_t cells = p->cells;
     {
         const int Kl = p->K[d - 1];
-        const int nlines = (int)(cells / Kl);
+        const int nlines = (int)(cells / Kl) * batch;
 #define CALL_ROWS(KK) launch_rows_full<KK>(data, p->d_tw[d - 1], nlines, st)
         NUFFT_K_SWITCH(Kl, CALL_ROWS)
 #undef CALL_ROWS
@@ -1402,7 +1437,7 @@ static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st) {
         c.line_stride = inner; c.inner = (int)inner;
         c.n_outer = (a == 0) ? 1 : p->K[0]; c.k_outer = 0;
         c.outer_stride = (a == 0) ? 0 : (int64_t)p->K[1] * p->K[2];
-        c.ngroups = c.n_outer * (c.inner / tile_T(p->K[a]));
+        c.ngroups = batch * c.n_outer * (c.inner / tile_T(p->K[a]));
 #define CALL_COLS(KK) launch_cols_full<KK>(c, st)
         NUFFT_K_SWITCH(p->K[a], CALL_COLS)
 #undef CALL_COLS
@@ -1414,6 +1449,7 @@ static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st) {
 
 extern "C" int nufft_toeplitz_build(nufft_plan_t p, const nufft_c64* w, void* stream) {
     if (!p) return NUFFT_EINVAL;
+    if (p->generic_sigma) return NUFFT_EINVAL;      // the embedding lives on the K = 2 N grid (reading R22)
     cudaStream_t st = (cudaStream_t)stream;
     const int d = p->d;
     const int64_t M = p->M;

@@ -1,0 +1,135 @@
+"""GPU parity at oversampling ratios other than 2 (SURVEY 8(f)-4 "other sigma"): plans with any even N < K and the same
+K/N on every axis run S + zero-pad and crop + S^H as separate kernels around the unpruned FFT; V and V^H are the regular
+kernels.  Forward, adjoint, A^H A, batches, coils, CG, k-space CG and density weights against the float64 oracle on the same
+seeded inputs (<= 2e-5 transforms, <= 1e-4 solvers); both interpolators and other widths.
+"""
+import numpy as np
+import pytest
+import torch
+
+import workloads as wl
+from oracle import minmax_oracle as mm
+from oracle import next_oracle as nxt
+from oracle import nufft_oracle as orc
+from oracle import solvers_oracle as sol
+
+pytestmark = pytest.mark.gpu
+TOL = 2e-5
+
+
+def rel(a, b):
+    a = np.asarray(a).ravel()
+    b = np.asarray(b).ravel()
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.complex64)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def cfg_of(Nd, Kd, M, J=6, seed=0):
+    rng = np.random.default_rng(seed)
+    d = len(Nd)
+    om = rng.uniform(-np.pi, np.pi, (M, d))
+    om[0] = -np.pi
+    om[1] = 0.0
+    om[2] = [2 * np.pi * 3 / k for k in Kd]
+    om[3] = np.pi - 1e-9
+    om[4] = 7.0
+    return dict(Nd=tuple(Nd), Kd=tuple(Kd), Jd=(J,) * d, om=om)
+
+
+def check(cfg, batch=1, oracle=orc, **kw):
+    import paper_1710_03197_b200 as nb
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    p = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=batch, **kw)
+    x = np.stack([wl.image_gaussian(Nd, seed=wl.SEED_IMAGE + b) for b in range(batch)])
+    y = np.stack([wl.data_gaussian(om.shape[0], seed=wl.SEED_Y + b) for b in range(batch)])
+    yg, xg, sg = host(p.forward(dev(x))), host(p.adjoint(dev(y))), host(p.selfadjoint(dev(x)))
+    for b in (0, batch - 1):
+        yo = oracle.forward(x[b].astype(np.complex128), om, Nd, Kd, Jd)
+        xo = oracle.adjoint(y[b].astype(np.complex128), om, Nd, Kd, Jd)
+        so = oracle.adjoint(yo, om, Nd, Kd, Jd)
+        errs = (rel(yg[b], yo), rel(xg[b], xo), rel(sg[b], so))
+        assert max(errs) < TOL, (Nd, Kd, b, errs)
+    p.destroy()
+
+
+@pytest.mark.parametrize("Nd,Kd", [((48, 48), (64, 64)), ((20, 40), (32, 64)), ((16, 16), (64, 64)), ((100, 100), (128, 128)),
+                                   ((160, 160), (256, 256)), ((28, 28), (32, 32))])
+def test_transforms_2d_at_sigma(Nd, Kd):
+    check(cfg_of(Nd, Kd, 7001, seed=Nd[0]))
+    check(cfg_of(Nd, Kd, 3001, seed=Nd[0] + 1), batch=17)            # above the interleaved threshold: stays planar
+    check(cfg_of(Nd, Kd, 3001, seed=Nd[0] + 2), adjoint_mode=1)
+
+
+def test_transforms_1d_and_3d_at_sigma():
+    check(cfg_of((40,), (64,), 1001, seed=1), batch=3)
+    check(cfg_of((100,), (128,), 2001, seed=2))
+    check(cfg_of((20, 20, 20), (32, 32, 32), 9001, seed=3))          # tiled 3-D V / V^H
+    check(cfg_of((12, 24, 12), (32, 64, 32), 5001, seed=4), batch=2, interp_mode=1, adjoint_mode=1)
+
+
+def test_other_widths_and_minmax_at_sigma():
+    check(cfg_of((40, 40), (64, 64), 4001, J=4, seed=5))
+    check(cfg_of((40, 40), (64, 64), 4001, J=8, seed=6))
+    check(cfg_of((48, 48), (64, 64), 4001, seed=7), oracle=mm, kernel="minmax")
+    check(cfg_of((20, 20, 20), (32, 32, 32), 4001, J=5, seed=8), oracle=mm, kernel="minmax")
+
+
+def test_radial_256_on_a_384_equivalent_grid():
+    """BASELINE config 2's trajectory with sigma = 1.6 (Nd = 160^2 on the 256^2 grid): a realistic non-2 ratio."""
+    cfg = dict(wl.config(1, scale=2))
+    cfg["Nd"], cfg["Kd"] = (160, 160), (256, 256)
+    check(cfg, batch=2)
+
+
+def test_unsupported_ratios_are_refused():
+    import paper_1710_03197_b200 as nb
+    om = np.zeros((10, 2))
+    for Nd, Kd in [((64, 64), (64, 64)), ((33, 33), (64, 64)), ((48, 32), (64, 64)), ((80, 80), (64, 64))]:
+        with pytest.raises(Exception):
+            nb.NufftPlan(Nd, Kd, (6, 6), om)
+
+
+def test_coils_solvers_and_next_rows_at_sigma():
+    import paper_1710_03197_b200 as nb
+    Nd, Kd, Jd = (40, 40), (64, 64), (6, 6)
+    cfg = cfg_of(Nd, Kd, 4 * 40 * 40, seed=9)
+    om = cfg["om"]
+    M = om.shape[0]
+    nc = 5
+    rng = np.random.default_rng(10)
+    c = rng.standard_normal((nc,) + Nd) + 1j * rng.standard_normal((nc,) + Nd)
+    c = (c / np.sqrt(np.sum(np.abs(c) ** 2, axis=0, keepdims=True))).astype(np.complex64)
+    c128 = c.astype(np.complex128)
+    p = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=nc)
+    p.set_coils(dev(c))
+    x = wl.image_gaussian(Nd)
+    yc = wl.data_gaussian(M, batch=nc)
+    yo = orc.forward_coils(x.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    xo = orc.adjoint_coils(yc.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    assert rel(host(p.forward_coils(dev(x))), yo) < TOL
+    assert rel(host(p.adjoint_coils(dev(yc))), xo) < TOL
+    assert rel(host(p.selfadjoint_coils(dev(x))), orc.adjoint_coils(yo, c128, om, Nd, Kd, Jd)) < TOL
+    # CG (image space) and the paper's k-space CG
+    xt = wl.phantom(Nd)
+    y = orc.forward(xt.astype(np.complex128), om, Nd, Kd, Jd)
+    y = (y + wl.noise_like(y)).astype(np.complex64)
+    AHA = lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd)
+    AHy = orc.adjoint(y.astype(np.complex128), om, Nd, Kd, Jd)
+    xc, _ = sol.cg(AHA, AHy, 6)
+    assert rel(host(p.solve_cg(dev(y), 6)), xc) < 1e-4
+    xk, _ = nxt.cg_kspace(y.astype(np.complex128), om, Nd, Kd, Jd, 3)
+    assert rel(host(p.solve_cg_kspace(dev(y), 3)), xk) < 1e-4
+    assert rel(host(p.density_weights(1)), nxt.density_weights(om, Nd, Kd, Jd, 1)) < TOL
+    # L1TV-OLS on the sigma != 2 plan
+    xl = sol.l1tv_ols(AHA, AHy, 1.0, 0.02, 2, 2, 3)
+    assert rel(host(p.solve_l1tv_ols(dev(y), 1.0, 0.02, 2, 2, 3)), xl) < 1e-4
+    with pytest.raises(Exception):
+        p.toeplitz_build()                                    # the Toeplitz embedding needs K = 2 N (R22)
+    p.destroy()
