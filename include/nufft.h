@@ -31,7 +31,7 @@
  *   - outputs are overwritten, never accumulated into.  In-place (x_in == x_out) is allowed for selfadjoint.
  *   - supported: d in {1,2,3} (1-D: "1D signals"; planar path, atomic V^H only -- adjoint_mode = 1 is
  *     refused); Jd[a] the same on every axis, 2 <= Jd <= 8 (odd widths included);
- *     Kd[a] in {32,64,128,256,512,1024}; Nd[a] even, 2 <= Nd[a] < Kd[a], the same ratio Kd[a]/Nd[a] on every axis;
+ *     Kd[a] in {32,64,128,256,512,1024}; Nd[a] even, 2 <= Nd[a] < Kd[a] (the ratio Kd[a]/Nd[a] may differ per axis);
  *     1 <= batch <= max_batch.  Kd == 2 Nd (the paper's and every BASELINE config's ratio) runs the pruned, fused FFT passes;
  *     any other ratio runs S + zero-pad and crop + S^H as separate kernels around the unpruned FFT, planar layout, and has
  *     no Toeplitz form (nufft_toeplitz_build -> NUFFT_EINVAL); everything else works unchanged.  Jd == 6 runs the tiled / batch-interleaved kernels;
@@ -100,8 +100,8 @@ typedef struct {
                            1 = min-max interpolator with the Kaiser-Bessel scaling factors: per sample
                                and axis the J REAL weights that minimise the worst-case error over unit-norm images,
                                T w = r(delta) (reading R25).  Same S, F, F^H, S^H and the same kernels: only the weight
-                               polynomial (and the float64 V^H table) differ, so every call works unchanged.  Needs the
-                               same Nd on every axis (the weights depend on N), else NUFFT_EINVAL                     */
+                               polynomial (and the float64 V^H table) differ, so every call works unchanged.  The
+                               weights depend on N_a: one polynomial per axis                                        */
 } nufft_opts;
 
 int nufft_default_opts(nufft_opts *o);

@@ -196,8 +196,8 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
         const int64_t si = s0 + t;
         const uint32_t kp = __ldg(&kpk[si]);
         float w0[kJ], w1[kJ];
-        kb_weights(P, __ldg(&dlt[si]), w0);
-        kb_weights(P, __ldg(&dlt[g.M + si]), w1);
+        kb_weights(P, 0, __ldg(&dlt[si]), w0);
+        kb_weights(P, 1, __ldg(&dlt[g.M + si]), w1);
         float4* r = &wrec[t * 4];
         r[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
         r[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);

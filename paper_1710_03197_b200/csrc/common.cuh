@@ -25,24 +25,26 @@ constexpr int kPolyHalf = 5;   // even / odd coefficient count ((kPolyDeg + 1) /
 // Piecewise polynomial fit of phi(J/2 - delta - j), j = 0..5, delta in [0,1), in z = 2 delta - 1.
 // By symmetry phi_{5-j}(z) = phi_j(-z), so three even/odd pairs describe all six pieces:
 //   phi_j(z) = ev[j](z^2) + z od[j](z^2),   phi_{5-j}(z) = ev[j](z^2) - z od[j](z^2),   j = 0,1,2.
+// One set per grid axis: the kernel shape depends on the axis through sigma_a = K_a / N_a (beta, reading R2) and, for the
+// min-max interpolator, through N_a itself (reading R25).
 struct KernelPoly {
-    float ev[3][kPolyHalf];
-    float od[3][kPolyHalf];
+    float ev[3][3][kPolyHalf];      // [axis][piece][coefficient]
+    float od[3][3][kPolyHalf];
     float zero_at;     // delta at which w[0] is exactly zero: 0 for Kaiser-Bessel (open support, R6), -1 (never) for min-max
 };
 
 // Six interpolation weights of one axis: w[j] = phi(J/2 - delta - j).
 // delta == 0 means the sample sits on a grid point: phi(+J/2) = 0 exactly (open support, reading R6).
-__device__ __forceinline__ void kb_weights(const KernelPoly& P, float delta, float (&w)[kJ]) {
+__device__ __forceinline__ void kb_weights(const KernelPoly& P, int a, float delta, float (&w)[kJ]) {
     const float z = fmaf(2.0f, delta, -1.0f);
     const float z2 = z * z;
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
-        float e = P.ev[j][kPolyHalf - 1], o = P.od[j][kPolyHalf - 1];
+        float e = P.ev[a][j][kPolyHalf - 1], o = P.od[a][j][kPolyHalf - 1];
 #pragma unroll
         for (int c = kPolyHalf - 2; c >= 0; --c) {
-            e = fmaf(e, z2, P.ev[j][c]);
-            o = fmaf(o, z2, P.od[j][c]);
+            e = fmaf(e, z2, P.ev[a][j][c]);
+            o = fmaf(o, z2, P.od[a][j][c]);
         }
         o *= z;
         w[j] = e + o;
@@ -54,22 +56,22 @@ __device__ __forceinline__ void kb_weights(const KernelPoly& P, float delta, flo
 // Any width J in [kJmin, kJmax]: ceil(J/2) even/odd pairs, phi_{J-1-j}(z) = phi_j(-z) (for odd J the middle piece is its
 // own mirror image).  With J = 6 and KernelPoly this is kb_weights above.
 struct KernelPolyG {
-    float ev[(kJmax + 1) / 2][kPolyHalf];
-    float od[(kJmax + 1) / 2][kPolyHalf];
+    float ev[3][(kJmax + 1) / 2][kPolyHalf];
+    float od[3][(kJmax + 1) / 2][kPolyHalf];
     float zero_at;
 };
 
 template <int J, class Poly>
-__device__ __forceinline__ void kb_weights_j(const Poly& P, float delta, float (&w)[J]) {
+__device__ __forceinline__ void kb_weights_j(const Poly& P, int a, float delta, float (&w)[J]) {
     const float z = fmaf(2.0f, delta, -1.0f);
     const float z2 = z * z;
 #pragma unroll
     for (int j = 0; j < (J + 1) / 2; ++j) {
-        float e = P.ev[j][kPolyHalf - 1], o = P.od[j][kPolyHalf - 1];
+        float e = P.ev[a][j][kPolyHalf - 1], o = P.od[a][j][kPolyHalf - 1];
 #pragma unroll
         for (int c = kPolyHalf - 2; c >= 0; --c) {
-            e = fmaf(e, z2, P.ev[j][c]);
-            o = fmaf(o, z2, P.od[j][c]);
+            e = fmaf(e, z2, P.ev[a][j][c]);
+            o = fmaf(o, z2, P.od[a][j][c]);
         }
         o *= z;
         w[j] = e + o;

@@ -55,7 +55,7 @@ struct nufft_plan_s {
     bool generic_j = false;         // J != kJ, or opts.interp_mode == 2 (the same kernels at J = kJ, for cross-checks)
     bool generic_sigma = false;     // Kd != 2 Nd: unpruned FFT + separate pad / crop kernels, planar, direct or tiled V / V^H
     bool minmax = false;            // opts.kernel == 1: min-max interpolator (reading R25); only the weight polynomials
-    host::MinMaxKernel mm;          //   and the float64 V^H table differ from the Kaiser-Bessel plan
+    host::MinMaxKernel mm[3];       //   and the float64 V^H table differ from the Kaiser-Bessel plan (one per axis: N_a)
     double poly_err = 0.0;
     // device plan data
     float* d_scale[3] = {nullptr, nullptr, nullptr};
@@ -742,7 +742,7 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
     for (int64_t i = 0; i < M; ++i) {
         const int64_t m = perm_h[i];
         double w0[kJ], w1[kJ];
-        if (p->minmax) { p->mm.weights(delta64[m], w0); p->mm.weights(delta64[M + m], w1); }
+        if (p->minmax) { p->mm[0].weights(delta64[m], w0); p->mm[1].weights(delta64[M + m], w1); }
         else { host::kb_weights_f64(delta64[m], J, beta, w0); host::kb_weights_f64(delta64[M + m], J, beta, w1); }
         float* rec = &wtab[(size_t)i * kTabW];
         for (int j = 0; j < kJ; ++j) rec[j] = (float)w0[j];
@@ -817,14 +817,19 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
 static int plan_build(nufft_plan_t p, const double* om) {
     const int d = p->d;
     const double J = (double)p->J;
-    const double sigma = (double)p->K[0] / (double)p->N[0];      // the same on every axis (checked by nufft_plan)
     // kernel polynomial, scaling vectors, twiddles (float64 on the host, rounded once)
-    if (p->minmax) {
-        p->mm.build(p->N[0], p->K[0], p->J);
-        if (p->generic_j) p->polyg = p->mm.fit<KernelPolyG>(&p->poly_err);
-        else p->poly = p->mm.fit<KernelPoly>(&p->poly_err);
-    } else if (p->generic_j) p->polyg = host::fit_kernel_poly_g(p->J, sigma, &p->poly_err);
-    else p->poly = host::fit_kernel_poly(J, sigma, &p->poly_err);
+    p->poly_err = 0.0;
+    for (int a = 0; a < d; ++a) {       // one kernel shape per axis: sigma_a = K_a / N_a (and N_a itself for min-max)
+        double err = 0.0;
+        const double sigma = (double)p->K[a] / (double)p->N[a];
+        if (p->minmax) {
+            p->mm[a].build(p->N[a], p->K[a], p->J);
+            if (p->generic_j) p->mm[a].fit_axis(p->polyg, a, &err);
+            else p->mm[a].fit_axis(p->poly, a, &err);
+        } else if (p->generic_j) host::fit_kernel_axis(p->polyg, a, p->J, sigma, &err);
+        else host::fit_kernel_axis(p->poly, a, p->J, sigma, &err);
+        p->poly_err = std::max(p->poly_err, err);
+    }
     for (int a = 0; a < d; ++a) {
         NU_TRY(dev_upload(&p->d_scale[a], host::scaling_vector(p->N[a], p->K[a], J), &p->bytes_plan));
         NU_TRY(dev_upload(&p->d_tw[a], host::twiddle_table(p->K[a]), &p->bytes_plan));
@@ -957,18 +962,14 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     if (M > (int64_t)0x7fffffff) return NUFFT_EINVAL;
     for (int a = 0; a < d; ++a) {
         if (Jd[a] != Jd[0] || Jd[a] < kJmin || Jd[a] > kJmax || Jd[a] > Kd[a] || !supported_K(Kd[a])) return NUFFT_EINVAL;
-        // any even N < K, with the same oversampling ratio on every axis (one kernel shape beta(J, sigma) for all axes)
-        if (Nd[a] < 2 || (Nd[a] & 1) || Nd[a] >= Kd[a] || Kd[a] * Nd[0] != Kd[0] * Nd[a]) return NUFFT_EINVAL;
+        if (Nd[a] < 2 || (Nd[a] & 1) || Nd[a] >= Kd[a]) return NUFFT_EINVAL;       // any even N < K, per axis
     }
-    const bool generic_sigma = Kd[0] != 2 * Nd[0];
+    bool generic_sigma = false;
+    for (int a = 0; a < d; ++a) generic_sigma = generic_sigma || Kd[a] != 2 * Nd[a];
     if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
                  opts->interp_mode > 2 || opts->batch_layout < 0 || opts->batch_layout > 2 || opts->kernel < 0 ||
                  opts->kernel > 1))
         return NUFFT_EINVAL;
-    // the min-max weights depend on N (through the scaling factors): one weight polynomial serves all axes only if they
-    // have the same size
-    if (opts && opts->kernel == 1)
-        for (int a = 1; a < d; ++a) if (Nd[a] != Nd[0]) return NUFFT_EINVAL;
     const bool generic_j = Jd[0] != kJ || (opts && opts->interp_mode == 2);
     // 1-D and the generic-width path have the atomic V^H only
     if ((d == 1 || generic_j) && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;

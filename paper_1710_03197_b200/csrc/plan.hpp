@@ -112,15 +112,10 @@ inline void fit_kernel_pieces(double J, double sigma, int npieces, float (*ev)[k
     fit_pieces([&](int j, double z) { return kb_phi(0.5 * J - 0.5 * (z + 1.0) - (double)j, J, beta); }, npieces, ev, od,
                max_err);
 }
-inline KernelPoly fit_kernel_poly(double J, double sigma, double* max_err) {      // J = kJ: three pairs
-    KernelPoly P{};
-    fit_kernel_pieces(J, sigma, kJ / 2, P.ev, P.od, max_err);
-    return P;
-}
-inline KernelPolyG fit_kernel_poly_g(int J, double sigma, double* max_err) {      // any J in [kJmin, kJmax]
-    KernelPolyG P{};
-    fit_kernel_pieces((double)J, sigma, (J + 1) / 2, P.ev, P.od, max_err);
-    return P;
+// one axis of a KernelPoly / KernelPolyG: pieces = ceil(J/2)
+template <class Poly>
+inline void fit_kernel_axis(Poly& P, int a, int J, double sigma, double* max_err) {
+    fit_kernel_pieces((double)J, sigma, (J + 1) / 2, P.ev[a], P.od[a], max_err);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -199,11 +194,9 @@ struct MinMaxKernel {
         const double z = 2.0 * delta - 1.0;
         for (int j = 0; j < J; ++j) w[j] = eval(j, z);
     }
-    template <class Poly> Poly fit(double* max_err) const {
-        Poly P{};
-        fit_pieces([&](int j, double z) { return eval(j, z); }, (J + 1) / 2, P.ev, P.od, max_err);
+    template <class Poly> void fit_axis(Poly& P, int a, double* max_err) const {
+        fit_pieces([&](int j, double z) { return eval(j, z); }, (J + 1) / 2, P.ev[a], P.od[a], max_err);
         P.zero_at = -1.0f;        // no open-support zero: the weight at t = J/2 is whatever the least-squares solution gives
-        return P;
     }
 };
 

@@ -41,7 +41,7 @@ interp_direct_kernel(SampleData s, GridGeom g, const float2* __restrict__ grid, 
     unpack_k0(__ldg(&s.kpack[i]), k0);
     float w[D][J];
 #pragma unroll
-    for (int a = 0; a < D; ++a) kb_weights_j<J>(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
+    for (int a = 0; a < D; ++a) kb_weights_j<J>(P, a, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
     const float2* __restrict__ G = grid + (int64_t)b * g.cells;
     float2 acc = make_float2(0.f, 0.f);
     if (D == 1) {
@@ -108,7 +108,7 @@ gridding_atomic_kernel(SampleData s, GridGeom g, const float2* __restrict__ y, f
     unpack_k0(__ldg(&s.kpack[i]), k0);
     float w[D][J];
 #pragma unroll
-    for (int a = 0; a < D; ++a) kb_weights_j<J>(P, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
+    for (int a = 0; a < D; ++a) kb_weights_j<J>(P, a, __ldg(&s.delta[(int64_t)a * g.M + i]), w[a]);
     const float2 yv = __ldg(&y[(int64_t)b * g.M + __ldg(&s.perm[i])]);
     float2* __restrict__ G = grid + (int64_t)b * g.cells;
     if (D == 1) {
@@ -183,8 +183,8 @@ constexpr int kStageBytes = 32 * (kStageRow * 16 + kStageCol * 8);
 __device__ __forceinline__ void stage_sample_2d(const KernelPoly& P, float4* rowrec, float2* colrec, int lane,
                                                 int c0, int c1, float d0, float d1, float2 yv, int pitch, int base_off) {
     float w0[kJ], w1[kJ];
-    kb_weights(P, d0, w0);
-    kb_weights(P, d1, w1);
+    kb_weights(P, 0, d0, w0);
+    kb_weights(P, 1, d1, w1);
     const int par = c1 & 1, base = base_off + c0 * pitch + (c1 - par);
 #pragma unroll
     for (int r = 0; r < kJ; ++r)
@@ -333,7 +333,7 @@ gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
             // this warp's plane of the sample: tile-local plane c0 + j0 = warp (mod 6)
             const int j0 = (warp - c0 % 6 + 6) % 6;
             float wz[kJ];
-            kb_weights(P, __ldg(&s.delta[si]), wz);
+            kb_weights(P, 0, __ldg(&s.delta[si]), wz);
             float wsel = wz[0];
 #pragma unroll
             for (int j = 1; j < kJ; ++j) wsel = (j0 == j) ? wz[j] : wsel;
@@ -341,8 +341,8 @@ gridding_tiled_3d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
             if (warp == 0) {
                 const int c1 = (k0[1] - o[1]) & (g.K[1] - 1), c2 = (k0[2] - o[2]) & (g.K[2] - 1);
                 float w1[kJ], w2[kJ];
-                kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
-                kb_weights(P, __ldg(&s.delta[2 * g.M + si]), w2);
+                kb_weights(P, 1, __ldg(&s.delta[g.M + si]), w1);
+                kb_weights(P, 2, __ldg(&s.delta[2 * g.M + si]), w2);
                 const int par = c2 & 1, base = c1 * tg.pitch + (c2 - par);
                 float2* rec = common + lane * k3CommonF2;
 #pragma unroll
@@ -516,9 +516,9 @@ interp_tiled_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ it
             int k0[3];
             unpack_k0(__ldg(&s.kpack[si]), k0);
             float w0[kJ], w1[kJ], w2[kJ];
-            kb_weights(P, __ldg(&s.delta[si]), w0);
-            kb_weights(P, __ldg(&s.delta[g.M + si]), w1);
-            kb_weights(P, __ldg(&s.delta[2 * g.M + si]), w2);
+            kb_weights(P, 0, __ldg(&s.delta[si]), w0);
+            kb_weights(P, 1, __ldg(&s.delta[g.M + si]), w1);
+            kb_weights(P, 2, __ldg(&s.delta[2 * g.M + si]), w2);
             float4* r = reinterpret_cast<float4*>(recs + t * k3RecW);
             r[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
             r[1] = make_float4(w0[4], w0[5], 0.f, 0.f);

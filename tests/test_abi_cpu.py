@@ -51,9 +51,9 @@ def test_strerror_and_arg_validation_without_gpu():
     assert L.nufft_default_opts(ctypes.byref(o)) == 0 and o.kernel == 0 and o.adjoint_mode == 0
     o.kernel = 2                                                                          # unknown interpolator
     assert L.nufft_plan(2, Nd, Kd, Jd, 0, None, 1, ctypes.byref(o), ctypes.byref(h)) == -1
-    o.kernel = 1                                                                          # min-max needs equal Nd (R25)
-    Nd_r, Kd_r = (ctypes.c_int64 * 2)(64, 32), (ctypes.c_int64 * 2)(128, 64)
-    assert L.nufft_plan(2, Nd_r, Kd_r, Jd, 0, None, 1, ctypes.byref(o), ctypes.byref(h)) == -1
+    for nd in ((64, 63), (128, 64), (0, 64), (130, 64)):                                  # N odd, N >= K, N < 2
+        Nd_r = (ctypes.c_int64 * 2)(*nd)
+        assert L.nufft_plan(2, Nd_r, Kd, Jd, 0, None, 1, None, ctypes.byref(h)) == -1
     o.kernel, o.adjoint_mode = 0, 1                                                       # deterministic V^H is J = 6 only
     assert L.nufft_plan(2, Nd, Kd, (ctypes.c_int * 2)(4, 4), 0, None, 1, ctypes.byref(o), ctypes.byref(h)) == -1
     assert L.nufft_plan(2, Nd, Kd_bad, Jd, 0, None, 1, None, ctypes.byref(h)) == -1      # Kd != 2 Nd / not pow2

@@ -100,9 +100,11 @@ def test_minmax_other_widths(J):
     check(rand_cfg((16, 16, 16), 3001, J=J, seed=20 + J))
 
 
-def test_minmax_needs_equal_axes():
-    with pytest.raises(Exception):
-        make_plan(rand_cfg((32, 64), 100))
+def test_minmax_non_square_images():
+    """The min-max weights depend on N_a: one weight polynomial per axis."""
+    check(rand_cfg((32, 64), 5001, seed=40))
+    check(rand_cfg((32, 64), 5001, seed=41), batch=17, imgs=(0, 16))          # interleaved path: per-axis float64 table
+    check(rand_cfg((16, 32, 64), 9001, seed=42))
 
 
 def test_minmax_cg_and_toeplitz_consistency():

@@ -74,6 +74,16 @@ def test_transforms_1d_and_3d_at_sigma():
     check(cfg_of((12, 24, 12), (32, 64, 32), 5001, seed=4), batch=2, interp_mode=1, adjoint_mode=1)
 
 
+def test_different_ratio_per_axis():
+    """Non-square images on power-of-two grids (e.g. 192 x 256 on 512 x 512): sigma_a = K_a / N_a per axis, so beta, the
+    scaling factors and the weight polynomial are per axis."""
+    check(cfg_of((48, 32), (64, 64), 5001, seed=11))                  # sigma = (1.33, 2)
+    check(cfg_of((192, 256), (512, 512), 20011, seed=12), batch=2)    # sigma = (2.67, 2)
+    check(cfg_of((20, 32, 24), (32, 64, 32), 9001, seed=13))          # sigma = (1.6, 2, 1.33)
+    check(cfg_of((48, 32), (64, 64), 5001, seed=14), oracle=mm, kernel="minmax")
+    check(cfg_of((48, 32), (64, 64), 3001, J=4, seed=15))
+
+
 def test_other_widths_and_minmax_at_sigma():
     check(cfg_of((40, 40), (64, 64), 4001, J=4, seed=5))
     check(cfg_of((40, 40), (64, 64), 4001, J=8, seed=6))
@@ -91,7 +101,7 @@ def test_radial_256_on_a_384_equivalent_grid():
 def test_unsupported_ratios_are_refused():
     import paper_1710_03197_b200 as nb
     om = np.zeros((10, 2))
-    for Nd, Kd in [((64, 64), (64, 64)), ((33, 33), (64, 64)), ((48, 32), (64, 64)), ((80, 80), (64, 64))]:
+    for Nd, Kd in [((64, 64), (64, 64)), ((33, 33), (64, 64)), ((80, 80), (64, 64))]:
         with pytest.raises(Exception):
             nb.NufftPlan(Nd, Kd, (6, 6), om)
 
@@ -126,7 +136,9 @@ def test_coils_solvers_and_next_rows_at_sigma():
     assert rel(host(p.solve_cg(dev(y), 6)), xc) < 1e-4
     xk, _ = nxt.cg_kspace(y.astype(np.complex128), om, Nd, Kd, Jd, 3)
     assert rel(host(p.solve_cg_kspace(dev(y), 3)), xk) < 1e-4
-    assert rel(host(p.density_weights(1)), nxt.density_weights(om, Nd, Kd, Jd, 1)) < TOL
+    # density weights w = 1 / |A A^H 1|: compared through |A A^H 1| = 1 / w (the L2 norm of w itself is dominated by the
+    # few samples where |A A^H 1| is small, which amplifies the 2e-7 operator rounding by rms / min ~ 200 at this sampling)
+    assert rel(1.0 / host(p.density_weights(1)).real, 1.0 / nxt.density_weights(om, Nd, Kd, Jd, 1)) < TOL
     # L1TV-OLS on the sigma != 2 plan
     xl = sol.l1tv_ols(AHA, AHy, 1.0, 0.02, 2, 2, 3)
     assert rel(host(p.solve_l1tv_ols(dev(y), 1.0, 0.02, 2, 2, 3)), xl) < 1e-4
