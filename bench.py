@@ -598,6 +598,24 @@ def extra_legs(nb, torch, peak, args):
         "paper_table1_k80_pycuda": "A 6 ms, A^H 6 ms, A^H A 8 ms; CG 1.89 s, L1TV-OLS 1.68 s, L1TV-LAD 1.78 s "
                                    "(PAPER.md:299-305; sizes and iteration counts not stated: context only)"}
     pp.destroy()
+    # SURVEY 8(f)-4 variants on config 2's trajectory, batch 1 (functional paths next to the tuned one)
+    cfg = wl.config(1)
+    var = {}
+    for name, Nd_v, Jd_v, kern in (("kb_J6", (256, 256), (6, 6), "kb"), ("minmax_J6", (256, 256), (6, 6), "minmax"),
+                                   ("kb_J4", (256, 256), (4, 4), "kb"), ("kb_J8", (256, 256), (8, 8), "kb"),
+                                   ("kb_J6_sigma1.6", (320, 320), (6, 6), "kb")):
+        pv = nb.NufftPlan(Nd_v, cfg["Kd"], Jd_v, cfg["om"], max_batch=1, kernel=kern)
+        xv = torch.from_numpy(wl.image_gaussian(Nd_v)).cuda().reshape(1, *Nd_v)
+        yv = pv.forward(xv)
+        xov = pv.adjoint(yv)
+        for _ in range(3):
+            pv.forward(xv, yv), pv.adjoint(yv, xov)
+        var[name] = {"forward_ms": time_calls(lambda: pv.forward(xv, yv), 10, flush),
+                     "adjoint_ms": time_calls(lambda: pv.adjoint(yv, xov), 10, flush)}
+        pv.destroy()
+    var["note"] = ("Kd=512^2, radial 256x512; min-max runs the same kernels as Kaiser-Bessel; J != 6 runs the direct V / atomic "
+                   "V^H kernels; sigma != 2 (Nd=320^2) runs pad / crop kernels around the unpruned FFT")
+    out["variants_cfg2_batch1"] = var
     # cuFFT reference point for F alone (never linked into the product): full 512^2 FFT of 64 grids via torch.fft
     gref = torch.randn(64, 512, 512, dtype=torch.complex64, device="cuda")
     torch.fft.fftn(gref, dim=(1, 2))
