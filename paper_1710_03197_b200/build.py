@@ -13,7 +13,7 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libnufft_b200.so")
 SOURCES = ["nufft.cu"]
-DEPS = ["nufft.cu", "common.cuh", "fft.cuh", "plan.hpp", "solver.cuh", "spread_interp.cuh", "batch_il.cuh",
+DEPS = ["nufft.cu", "common.cuh", "fft.cuh", "plan.hpp", "solver.cuh", "spread_interp.cuh", "batch_il.cuh", "win3d.cuh",
         os.path.join("..", "..", "include", "nufft.h")]
 
 NVCC_FLAGS = [

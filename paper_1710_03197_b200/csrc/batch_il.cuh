@@ -162,6 +162,8 @@ struct IlPlan {
     const float* delta;       // V order: [2][M]
     const uint32_t* kpack_c;  // caller order (trajectory-coherent plans only, else null)
     const float* delta_c;     // caller order [2][M]
+    const uint32_t* gbase;    // V order: base cell (row | col << 10) of the sample's window group (interp_il_win_kernel)
+    const uint32_t* gbase_c;  // caller order (trajectory-coherent plans only, else null)
     const int32_t* v2h;       // V-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
     const float* wtab;        // V^H order: [M][kTabW] = w0[6], k0_0 (int bits), pad, w1 part A[8], w1 part B[8] (float64-built)
@@ -256,6 +258,126 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
             const int l = warp * (kIL / kInterpWarps) + li, b = grp * kIL + l;
             if (b >= batch) continue;
             for (int t = lane; t < cnt; t += 32) y_il[(int64_t)b * g.M + s0 + t] = otile[t][l];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a3 with register windows (round 2).  profiles/r01n: interp_il_kernel re-reads all 36 stencil cells of every sample
+// (36 warp loads of 256 B = 72 L1 wavefronts per sample and image group) and sits on the L1 data pipe (85 % busy) at 26 %
+// of the HBM roofline.  Neighbouring samples of the walk order (one grid cell apart along a radial readout; many per cell
+// near the k-space centre) share most of their stencils, so the plan cuts the walk order into GROUPS -- maximal runs of
+// consecutive samples whose stencil bases fit a 3 x 3 box -- and a warp keeps the 8 x 8 cells x 32 images WINDOW of the
+// current group in registers (128 registers per lane): 64 loads per group instead of 36 per sample (config 2: 3.2 samples
+// per group in the caller's order, 5.2 in the sorted order).  Per sample the lane then runs 72 packed FMAs (FFMA2 on
+// (re, im), scalar weights) with weights that are zero outside the sample's own 6 x 6 support: the arithmetic is that of
+// the plain stencil sum.  Weights are evaluated once per sample by one lane (kb_weights) and parked zero-padded in shared
+// memory; all per-sample loads are warp-uniform broadcasts.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kIwWarps = 4;          // warps per CTA, 32 consecutive samples of the walk order each
+constexpr int kIwRec = 20;           // floats per staged sample: w0 padded [8], w1 padded [8], base, output index, 2 pad
+                                     // (5 float4: 5 s mod 8 is a permutation -> conflict-free 128-bit stores)
+
+__device__ __forceinline__ void il_pad8(const float (&w)[kJ], int o, float4& a, float4& b) {
+    const bool o0 = o == 0, o1 = o == 1;
+    a.x = o0 ? w[0] : 0.f;
+    a.y = o0 ? w[1] : (o1 ? w[0] : 0.f);
+    a.z = o0 ? w[2] : (o1 ? w[1] : w[0]);
+    a.w = o0 ? w[3] : (o1 ? w[2] : w[1]);
+    b.x = o0 ? w[4] : (o1 ? w[3] : w[2]);
+    b.y = o0 ? w[5] : (o1 ? w[4] : w[3]);
+    b.z = o0 ? 0.f : (o1 ? w[5] : w[4]);
+    b.w = (o0 || o1) ? 0.f : w[5];
+}
+
+template <bool CALLER>
+__global__ void __launch_bounds__(kIwWarps * 32, 3)
+interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y_out, int batch,
+                     KernelPoly P) {
+    __shared__ __align__(16) float recs[kIwWarps][32][kIwRec];
+    __shared__ float2 otile[CALLER ? kIwWarps * 32 : 1][33];
+    const uint32_t* __restrict__ kpk = CALLER ? s.kpack_c : s.kpack;
+    const float* __restrict__ dlt = CALLER ? s.delta_c : s.delta;
+    const uint32_t* __restrict__ gbs = CALLER ? s.gbase_c : s.gbase;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = blockIdx.y;
+    const int64_t s0 = (int64_t)blockIdx.x * (kIwWarps * 32);
+    const int K0 = g.K[0], K1 = g.K[1];
+    const float2* __restrict__ G = grid_il + (int64_t)grp * g.cells * kIL + lane;
+    const int64_t w0s = s0 + warp * 32;
+    const int cnt = (int)max((int64_t)0, min((int64_t)32, g.M - w0s));
+    {   // stage: lane = sample
+        float4 r0, r1, r2, r3, r4;
+        if (lane < cnt) {
+            const int64_t si = w0s + lane;
+            const uint32_t kp = __ldg(&kpk[si]), gb = __ldg(&gbs[si]);
+            float w[kJ];
+            kb_weights(P, 0, __ldg(&dlt[si]), w);
+            il_pad8(w, (int)(kp & 1023u) - (int)(gb & 1023u), r0, r1);
+            kb_weights(P, 1, __ldg(&dlt[g.M + si]), w);
+            il_pad8(w, (int)((kp >> 10) & 1023u) - (int)((gb >> 10) & 1023u), r2, r3);
+            r4 = make_float4(__int_as_float((int)gb), __int_as_float(CALLER ? 0 : __ldg(&s.v2h[si])), 0.f, 0.f);
+        } else {
+            r0 = r1 = r2 = r3 = make_float4(0.f, 0.f, 0.f, 0.f);
+            r4 = make_float4(__int_as_float(-1), __int_as_float(0), 0.f, 0.f);
+        }
+        float4* r = reinterpret_cast<float4*>(&recs[warp][lane][0]);
+        r[0] = r0; r[1] = r1; r[2] = r2; r[3] = r3; r[4] = r4;
+    }
+    __syncwarp();
+    float2 win[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) win[i][j] = make_float2(0.f, 0.f);
+    int cur = -1;
+#pragma unroll 1
+    for (int t = 0; t < cnt; ++t) {
+        const float* r = &recs[warp][t][0];
+        const float4 a0 = *reinterpret_cast<const float4*>(r), a1 = *reinterpret_cast<const float4*>(r + 4);
+        const float4 b0 = *reinterpret_cast<const float4*>(r + 8), b1 = *reinterpret_cast<const float4*>(r + 12);
+        const float2 mm = *reinterpret_cast<const float2*>(r + 16);
+        const int key = __float_as_int(mm.x);
+        if (key != cur) {       // new group: load its 8 x 8 window (rows and columns wrap periodically)
+            cur = key;
+            const int br = key & 1023, bc = (key >> 10) & 1023;
+            if (bc + 8 <= K1) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float2* __restrict__ pr = G + ((int64_t)((br + i) & (K0 - 1)) * K1 + bc) * kIL;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) win[i][j] = __ldg(pr + j * kIL);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float2* __restrict__ pr = G + (int64_t)((br + i) & (K0 - 1)) * K1 * kIL;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) win[i][j] = __ldg(pr + (int64_t)((bc + j) & (K1 - 1)) * kIL);
+                }
+            }
+        }
+        const float w0[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+        const float w1[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+        float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            float2 rs = __fmul2_rn(make_float2(w1[0], w1[0]), win[i][0]);
+#pragma unroll
+            for (int j = 1; j < 8; ++j) rs = __ffma2_rn(make_float2(w1[j], w1[j]), win[i][j], rs);
+            acc = __ffma2_rn(make_float2(w0[i], w0[i]), rs, acc);
+        }
+        if (CALLER) otile[warp * 32 + t][lane] = acc;
+        else y_out[((int64_t)grp * g.M + __float_as_int(mm.y)) * kIL + lane] = acc;
+    }
+    if (CALLER) {     // y_out is the caller's y[batch][M]: warp w writes images 8 w .. 8 w + 7, 128 consecutive samples each
+        __syncthreads();
+        const int tot = (int)min((int64_t)(kIwWarps * 32), g.M - s0);
+#pragma unroll
+        for (int li = 0; li < kIL / kIwWarps; ++li) {
+            const int l = warp * (kIL / kIwWarps) + li, b = grp * kIL + l;
+            if (b >= batch) continue;
+            for (int t = lane; t < tot; t += 32) y_out[(int64_t)b * g.M + s0 + t] = otile[t][l];
         }
     }
 }

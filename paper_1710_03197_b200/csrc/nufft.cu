@@ -15,6 +15,7 @@
 #include "solver.cuh"
 #include "spread_interp.cuh"
 #include "batch_il.cuh"
+#include "win3d.cuh"
 
 using namespace nufft;
 
@@ -83,6 +84,7 @@ struct nufft_plan_s {
     int n_items = 0;
     float2* d_slabs = nullptr;      // deterministic mode: [max_batch][n_items][tile_cells], lazy
     int64_t n_tiles = 0, n_work = 0, max_tile_samples = 0;
+    bool win3d = false;             // 3-D, J = 6, default tile: samples pencil-sorted inside tiles, register-window V / V^H (win3d.cuh)
     int64_t bytes_plan = 0, bytes_work = 0;
     int64_t launches = 0;
     // batch-interleaved 2-D path (batch_il.cuh): cell-sorted plan data, V^H weight table, row pointers, work items
@@ -95,6 +97,8 @@ struct nufft_plan_s {
     float* d_il_wtab = nullptr;
     int32_t* d_il_rowptr = nullptr;
     int32_t* d_il_v2h = nullptr;     // V-order position -> V^H-order position
+    uint32_t* d_il_gbase = nullptr;      // window-group base cell per sample, V order / caller order (interp_il_win_kernel)
+    uint32_t* d_il_gbase_c = nullptr;
     uint32_t* d_il_kpack_c = nullptr;    // caller-order copies for trajectory-coherent plans (il_coherent)
     float* d_il_delta_c = nullptr;
     bool il_coherent = false;
@@ -207,6 +211,11 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_il_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<1>::BYTES)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_il_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<2>::BYTES)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+#define NU_W3_CFG(NW)                                                                                                                   \
+    if ((e = cudaFuncSetAttribute(interp_win_3d_kernel<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;   \
+    if ((e = cudaFuncSetAttribute(gridding_win_3d_kernel<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;
+    NU_W3_CFG(kW3InterpWarps) NU_W3_CFG(kW3GridWarps)
+#undef NU_W3_CFG
     return cudaSuccess;
 }
 
@@ -399,6 +408,35 @@ static SampleData sample_data(nufft_plan_t p) {
     return s;
 }
 
+// Tensor map of a planar 3-D grid [batch][K0][K1][K2] complex64 seen as float32 [batch][K0][K1][2 K2], box = one padded
+// tile (win3d.cuh).  cuTensorMapEncodeTiled is a host-only driver entry point (no context work), fetched through the
+// runtime so that libcuda is not a link dependency.  Returns false when the driver cannot provide it: the kernels then
+// stage and flush tiles row by row.
+typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static tmap_encode_fn tmap_encoder() {
+    static tmap_encode_fn fn = []() -> tmap_encode_fn {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess) { (void)cudaGetLastError(); return nullptr; }
+        return (tmap_encode_fn)f;
+    }();
+    return fn;
+}
+static bool tile_tensor_map(nufft_plan_t p, int batch, const float2* grid, CUtensorMap* tm) {
+    std::memset(tm, 0, sizeof(*tm));
+    tmap_encode_fn enc = tmap_encoder();
+    if (!enc || p->d != 3) return false;
+    const cuuint64_t gdim[4] = {(cuuint64_t)2 * p->K[2], (cuuint64_t)p->K[1], (cuuint64_t)p->K[0], (cuuint64_t)batch};
+    const cuuint64_t gstr[3] = {(cuuint64_t)p->K[2] * 8, (cuuint64_t)p->K[1] * p->K[2] * 8, (cuuint64_t)p->cells * 8};
+    const cuuint32_t box[4] = {2 * k3Pitch, k3P1, k3P0, 1};
+    const cuuint32_t est[4] = {1, 1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)grid, gdim, gstr, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // Widths other than kJ: direct V and atomic V^H, one instantiation per (d, J)
 #define NU_J_CASES(KERNEL, D, ...)                                                             \
     switch (p->J) {                                                                            \
@@ -427,10 +465,18 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
         p->launches++;
         return NUFFT_OK;
     }
-    if (p->d == 3 && p->opts.interp_mode == 0 && p->tile[0] == k3T0 && p->tile[1] == k3T1 && p->tile[2] == k3T2 && p->n_items > 0) {
-        // tile-staged V (default tile only); interp_mode = 1 keeps the direct gather
+    if (p->d == 3 && (p->opts.interp_mode == 0 || p->opts.interp_mode == 3) && p->tile[0] == k3T0 && p->tile[1] == k3T1 && p->tile[2] == k3T2 && p->n_items > 0) {
+        // tile-staged V (default tile only): register windows over pencil-sorted samples (win3d.cuh); interp_mode = 3 keeps
+        // the half-warp-per-sample kernel of round 1, interp_mode = 1 the direct gather
         const dim3 tb((unsigned)p->n_items, (unsigned)batch);
-        interp_tiled_3d_kernel<<<tb, 256, kInterp3dSmem, st>>>(sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly);
+        if (p->win3d && p->opts.interp_mode == 0) {
+            CUtensorMap tm;
+            const int use_tm = tile_tensor_map(p, batch, grid, &tm) ? 1 : 0;
+            interp_win_3d_kernel<kW3InterpWarps><<<tb, kW3InterpWarps * 32, win3d_smem(kW3InterpWarps), st>>>(
+                sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly, tm, use_tm);
+        }
+        else
+            interp_tiled_3d_kernel<<<tb, 256, kInterp3dSmem, st>>>(sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly);
         CU_TRY(cudaGetLastError());
         p->launches++;
         return NUFFT_OK;
@@ -477,6 +523,12 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
         const size_t sm = smem_grid2d(p);
         if (det) gridding_tiled_2d_kernel<true><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly);
         else     gridding_tiled_2d_kernel<false><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, nullptr, 0, p->poly);
+    } else if (!det && p->win3d && p->opts.adjoint_mode == 0) {
+        const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
+        CUtensorMap tm;
+        const int use_tm = tile_tensor_map(p, batch, grid, &tm) ? 1 : 0;
+        gridding_win_3d_kernel<kW3GridWarps><<<blocks, kW3GridWarps * 32, win3d_smem(kW3GridWarps), st>>>(
+            sample_data(p), grid_geom(p), p->d_items, y, grid, p->poly, tm, use_tm);
     } else {
         const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
         const size_t sm = smem_grid3d(p);
@@ -564,6 +616,7 @@ static IlPlan il_plan(nufft_plan_t p) {
     s.kpack = p->d_il_kpack; s.delta = p->d_il_delta; s.pos = p->d_il_pos; s.wtab = p->d_il_wtab;
     s.rowptr = p->d_il_rowptr; s.v2h = p->d_il_v2h;
     s.kpack_c = p->d_il_kpack_c; s.delta_c = p->d_il_delta_c;
+    s.gbase = p->d_il_gbase; s.gbase_c = p->d_il_gbase_c;
     return s;
 }
 
@@ -601,6 +654,10 @@ static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* 
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + kInterpChunk - 1) / kInterpChunk), (unsigned)il_groups(batch));
     ProfScope ps(p, "interp", st);
+    if (p->opts.interp_mode != 3) {     // register windows over the block-sorted walk (interp_mode = 3: round-1 kernel)
+        const dim3 wb((unsigned)((p->M + kIwWarps * 32 - 1) / (kIwWarps * 32)), (unsigned)il_groups(batch));
+        interp_il_win_kernel<false><<<wb, kIwWarps * 32, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
+    } else
     interp_il_kernel<false, kInterpChunk><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
     CU_TRY(cudaGetLastError());
     p->launches++;
@@ -611,6 +668,10 @@ static int run_interp_il_caller(nufft_plan_t p, int batch, const float2* grid, f
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + kInterpChunkCaller - 1) / kInterpChunkCaller), (unsigned)il_groups(batch));
     ProfScope ps(p, "interp", st);
+    if (p->opts.interp_mode != 3) {
+        const dim3 wb((unsigned)((p->M + kIwWarps * 32 - 1) / (kIwWarps * 32)), (unsigned)il_groups(batch));
+        interp_il_win_kernel<true><<<wb, kIwWarps * 32, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
+    } else
     interp_il_kernel<true, kInterpChunkCaller><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
     CU_TRY(cudaGetLastError());
     p->launches++;
@@ -714,10 +775,30 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
     };
     // ---- V order
     std::vector<int32_t> perm_v, bins_v;
+    const int nbr = (K0 + 2) / 3, nbc = (K1 + 2) / 3;     // 3 x 3 blocks of stencil base cells, column-block major
     sort_by([&](uint32_t kp) -> int64_t {
         const int r = row_of(kp), c = col_of(kp);
-        return ((int64_t)(c / kBandW) * K0 + r) * kBandW + (c % kBandW);
-    }, (int64_t)nb * K0 * kBandW, perm_v, bins_v);
+        return ((int64_t)(c / 3) * nbr + r / 3) * 9 + (r % 3) * 3 + (c % 3);
+    }, (int64_t)nbc * nbr * 9, perm_v, bins_v);
+    // window groups of a walk order: maximal runs of consecutive samples whose stencil bases fit a 3 x 3 box (no wrap
+    // inside a group); every sample records the base cell (row | col << 10) of its group
+    auto window_groups = [&](auto kp_at, std::vector<uint32_t>& gb) {
+        gb.resize(M);
+        int64_t i = 0;
+        while (i < M) {
+            int lo0 = row_of(kp_at(i)), hi0 = lo0, lo1 = col_of(kp_at(i)), hi1 = lo1;
+            int64_t j = i + 1;
+            for (; j < M; ++j) {
+                const int r = row_of(kp_at(j)), c = col_of(kp_at(j));
+                const int nlo0 = std::min(lo0, r), nhi0 = std::max(hi0, r), nlo1 = std::min(lo1, c), nhi1 = std::max(hi1, c);
+                if (nhi0 - nlo0 > 2 || nhi1 - nlo1 > 2) break;
+                lo0 = nlo0; hi0 = nhi0; lo1 = nlo1; hi1 = nhi1;
+            }
+            const uint32_t base = (uint32_t)lo0 | ((uint32_t)lo1 << 10);
+            for (int64_t k = i; k < j; ++k) gb[k] = base;
+            i = j;
+        }
+    };
     // ---- V^H order: bins (band, class, row)
     std::vector<int32_t> perm_h, rowptr;
     sort_by([&](uint32_t kp) -> int64_t {
@@ -798,11 +879,19 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
             d0 = std::min(d0, K0 - d0); d1 = std::min(d1, K1 - d1);
             near += (d0 <= 2 && d1 <= 2) ? 1 : 0;
         }
-        p->il_coherent = (M > 1) && (near * 10 >= (M - 1) * 9) && p->opts.interp_mode == 0;
+        p->il_coherent = (M > 1) && (near * 10 >= (M - 1) * 9) && (p->opts.interp_mode == 0 || p->opts.interp_mode == 3);
         if (p->il_coherent) {
+            std::vector<uint32_t> gb_c;
+            window_groups([&](int64_t i) { return kpack[i]; }, gb_c);
             NU_TRY(dev_upload(&p->d_il_kpack_c, kpack, &p->bytes_plan));
             NU_TRY(dev_upload(&p->d_il_delta_c, delta, &p->bytes_plan));
+            NU_TRY(dev_upload(&p->d_il_gbase_c, gb_c, &p->bytes_plan));
         }
+    }
+    {
+        std::vector<uint32_t> gb_v;
+        window_groups([&](int64_t i) { return kp_s[i]; }, gb_v);
+        NU_TRY(dev_upload(&p->d_il_gbase, gb_v, &p->bytes_plan));
     }
     NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_delta, dl_s, &p->bytes_plan));
@@ -865,10 +954,15 @@ static int plan_build(nufft_plan_t p, const double* om) {
     std::vector<uint32_t> kpack(M);
     std::vector<float> delta((size_t)d * M);
     std::vector<double> delta64(p->il_ok ? (size_t)d * M : 0);
-    std::vector<int32_t> tid(M);
+    // 3-D, J = 6, default tile: inside a tile the samples are sorted by pencil (3 x 3 block of stencil base cells on axes
+    // 0, 1) and base pair on axis 2, the order the register-window kernels of win3d.cuh walk
+    p->win3d = (d == 3) && !p->generic_j && p->tile[0] == k3T0 && p->tile[1] == k3T1 && p->tile[2] == k3T2;
+    const int nsub = p->win3d ? kW3SubKeys : 1;
+    std::vector<int64_t> tid(M);        // tile id * nsub + key inside the tile
     for (int64_t m = 0; m < M; ++m) {
         uint32_t kp = 0;
         int64_t t = 0;
+        int c[3] = {0, 0, 0};
         for (int a = 0; a < d; ++a) {
             const double w = om[m * d + a];
             if (!std::isfinite(w)) return NUFFT_ERANGE;
@@ -879,22 +973,22 @@ static int plan_build(nufft_plan_t p, const double* om) {
             kp |= (uint32_t)k0 << (10 * a);
             delta[(size_t)a * M + m] = df;
             t = t * p->ntile[a] + k0 / p->tile[a];
+            c[a] = k0 % p->tile[a];
         }
         kpack[m] = kp;
-        tid[m] = (int32_t)t;
+        tid[m] = t * nsub + (p->win3d ? w3_sub_key(c[0], c[1], c[2]) : 0);
     }
-    // stable counting sort by tile
+    // stable counting sort by (tile, key inside the tile)
     std::vector<int64_t> start(p->n_tiles + 1, 0);
-    for (int64_t m = 0; m < M; ++m) start[tid[m] + 1]++;
-    p->max_tile_samples = 0;
-    for (int64_t t = 0; t < p->n_tiles; ++t) {
-        p->max_tile_samples = std::max<int64_t>(p->max_tile_samples, start[t + 1]);
-        start[t + 1] += start[t];
-    }
     std::vector<int32_t> perm(M);
     {
-        std::vector<int64_t> cur(start.begin(), start.end() - 1);
-        for (int64_t m = 0; m < M; ++m) perm[cur[tid[m]]++] = (int32_t)m;
+        std::vector<int64_t> fine((size_t)p->n_tiles * nsub + 1, 0);
+        for (int64_t m = 0; m < M; ++m) fine[tid[m] + 1]++;
+        for (size_t b = 0; b + 1 < fine.size(); ++b) fine[b + 1] += fine[b];
+        for (int64_t t = 0; t <= p->n_tiles; ++t) start[t] = fine[(size_t)t * nsub];
+        p->max_tile_samples = 0;
+        for (int64_t t = 0; t < p->n_tiles; ++t) p->max_tile_samples = std::max<int64_t>(p->max_tile_samples, start[t + 1] - start[t]);
+        for (int64_t m = 0; m < M; ++m) perm[fine[tid[m]]++] = (int32_t)m;
     }
     std::vector<uint32_t> kpack_s(M);
     std::vector<float> delta_s((size_t)d * M);
@@ -966,8 +1060,8 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     }
     bool generic_sigma = false;
     for (int a = 0; a < d; ++a) generic_sigma = generic_sigma || Kd[a] != 2 * Nd[a];
-    if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 1 || opts->interp_mode < 0 ||
-                 opts->interp_mode > 2 || opts->batch_layout < 0 || opts->batch_layout > 2 || opts->kernel < 0 ||
+    if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 2 || opts->interp_mode < 0 ||
+                 opts->interp_mode > 3 || opts->batch_layout < 0 || opts->batch_layout > 2 || opts->kernel < 0 ||
                  opts->kernel > 1))
         return NUFFT_EINVAL;
     const bool generic_j = Jd[0] != kJ || (opts && opts->interp_mode == 2);
@@ -1018,7 +1112,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_kspace);
     cudaFree(p->d_ones); cudaFree(p->d_that); cudaFree(p->d_dcf_img); cudaFree(p->d_dcf_t);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
-    cudaFree(p->d_il_kpack_c); cudaFree(p->d_il_delta_c);
+    cudaFree(p->d_il_kpack_c); cudaFree(p->d_il_delta_c); cudaFree(p->d_il_gbase); cudaFree(p->d_il_gbase_c);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     if (p->cg_graph) cudaGraphExecDestroy(p->cg_graph);
     for (auto& og : p->op_graphs) cudaGraphExecDestroy(og.exec);
