@@ -26,12 +26,15 @@ Parity pins (tests/test_oracle_next.py):
                            T[-d] = conj(T[d])
     selfadjoint_toeplitz   against the dense matrix A_exact^H A_exact built from the plain non-uniform DFT definition
                            (rel. <= 1e-4) and against adjoint(forward(x)) (same bound)
-    l1tv_lad               PARITY UNPINNED by the paper (eqs. (23)-(33), garbled; reading R23 in its docstring).  Sanity
-                           pins: first inner iteration = L1TV-OLS's, scale equivariance, consistent-data fixed point.
+    l1tv_lad               tests/test_oracle_bregman.py: with A^H A = prod(N) I the converged result is TV-L1 denoising,
+                           contrast invariant for every mu, lambda: a box wider than two rows keeps its full height, a
+                           one-row line is removed; the outer update eq. (33) restores the line (x -> z).  A threshold mu
+                           for 1/mu (or lambda for 1/lambda), a flipped b_f update or a dropped eq. (33) each fail.  Also:
+                           first inner iteration = L1TV-OLS's, scale equivariance, consistent-data fixed point.
     cg_kspace              final step: S^{-1}F^{-1} inverts k = F S x exactly; converged k equals the minimum-norm least
                            squares solution pinv(V) y computed from the dense V (numpy.linalg.lstsq); CG recurrence itself
                            pinned in tests/test_oracle_solvers.py
-No other function here is "parity unpinned".
+No function here is "parity unpinned".
 """
 import numpy as np
 
@@ -101,8 +104,8 @@ def l1tv_lad(AHA, AHy, mu, lam, n_outer, n_inner, n_cg):
         d_a  = shrink(grad_a x + b_a, 1/lam);   b_a += grad_a x - d_a                         (27)-(28), (30)-(31)
         r    = A^H A x - A^H y;   d_f = shrink(r + b_f, 1/mu);   b_f += r - d_f               (29), (32)
         outer: A^H y^{k+1} = A^H y^k + A^H y - A^H A x                                        (33)
-    PARITY UNPINNED by the paper (iterate values are defined only by this code).  Sanity pins: the first inner iteration
-    equals L1TV-OLS's (d_f = b_f = 0); scale equivariance; d_f = b_f = 0 forever when A^H A x = A^H y already holds."""
+    Pins: tests/test_oracle_bregman.py (converged values in closed form on Cartesian sampling, outer update) and
+    tests/test_oracle_next.py (first inner iteration equals L1TV-OLS's, scale equivariance, consistent-data fixed point)."""
     from .solvers_oracle import cg_steps, grad, grad_T, shrink
     AHy = np.asarray(AHy, dtype=np.complex128)
     assert AHy.ndim == 2

@@ -24,9 +24,12 @@ Parity pins (tests/test_oracle_solvers.py):
     shrink          closed-form values; magnitude / phase properties
     cg              tiny dense problem: iterate k equals the minimiser of the A-norm error over the k-th Krylov
                     space (computed by dense linear algebra) and converges to numpy.linalg.lstsq
-    l1tv_ols        PARITY UNPINNED by the paper (its iterate values are defined only by this code; R13-R17).
-                    Sanity pins: with d = b = 0 frozen (threshold -> infinity) and lambda = 0 it reduces to
-                    CG on the normal equation; objective decrease.
+    l1tv_ols        tests/test_oracle_bregman.py: (i) Cartesian full sampling (A^H A = prod(N) I): the converged result is
+                    the closed-form TV-denoising minimiser of a two-level image, for every lambda; (ii) the outer
+                    update eq. (22) drives the iterates to the data-consistent image; (iii) on a small non-Cartesian
+                    dense problem the converged result equals the minimiser of mu/2 ||Ax - y||^2 + w TV(x) computed
+                    by Chambolle-Pock primal-dual iterations.  A threshold lambda instead of 1/lambda, a flipped
+                    Bregman update or a dropped eq. (22) each fail one of them.  Also: lambda = 0 reduces to CG.
 """
 import numpy as np
 

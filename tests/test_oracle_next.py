@@ -110,7 +110,7 @@ def test_selfadjoint_toeplitz_3d_tiny():
     assert rel(nxt.selfadjoint_toeplitz(x, That, Nd), exact) < 1e-4
 
 
-# ---- L1TV-LAD (parity unpinned by the paper: sanity pins only) ----
+# ---- L1TV-LAD: sanity pins (the converged values are pinned in tests/test_oracle_bregman.py) ----
 def _lad_problem(seed=11, N=12, M=500):
     from oracle import solvers_oracle as sol  # noqa: F401
     rng = np.random.default_rng(seed)

@@ -1,4 +1,4 @@
-"""Pins for oracle/solvers_oracle.py: gradient, shrink, CG, and the sanity pins of L1TV-OLS (parity unpinned)."""
+"""Pins for oracle/solvers_oracle.py: gradient, shrink, CG, and sanity pins of L1TV-OLS (its converged values: test_oracle_bregman.py)."""
 import numpy as np
 import pytest
 
