@@ -221,6 +221,13 @@ int nufft_plan_info(nufft_plan_t p, int64_t *bytes_plan, int64_t *bytes_work,
  * weight polynomial the kernels evaluate against the float64 kernel it was fitted to (weights are <= 1). */
 int nufft_plan_modes(nufft_plan_t p, int *J, int *kernel, int *paths, double *poly_err);
 
+/* Tile histogram of the plan (SURVEY 8(b) "tile histogram"): counts[0] = tiles without samples, counts[k] (k >= 1) = tiles
+ * holding 2^(k-1) <= n < 2^k samples, k < NUFFT_TILE_HIST_BUCKETS (the last bucket also takes every larger tile).  The tiles
+ * are those of the planar V^H / 3-D V kernels (default 16 x 32 cells in 2-D, 8 x 8 x 16 in 3-D); the sum of the
+ * counts is n_tiles of nufft_plan_info.  counts: int64[NUFFT_TILE_HIST_BUCKETS], host, written. */
+#define NUFFT_TILE_HIST_BUCKETS 24
+int nufft_plan_tile_histogram(nufft_plan_t p, int64_t *counts);
+
 /* Number of kernel launches the library has enqueued for this plan since creation (bench.py's gpu_launches). */
 int64_t nufft_launch_count(nufft_plan_t p);
 

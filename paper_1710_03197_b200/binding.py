@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "nufft_selfadjoint_toeplitz", "nufft_selfadjoint_toeplitz_coils", "nufft_solve_l1tv_lad", "nufft_solve_cg_kspace",
     "nufft_stage_scale_fft", "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale",
     "nufft_set_coils", "nufft_forward_coils", "nufft_adjoint_coils", "nufft_selfadjoint_coils",
-    "nufft_solve_cg", "nufft_solve_l1tv_ols", "nufft_plan_info", "nufft_plan_modes", "nufft_launch_count", "nufft_destroy",
+    "nufft_solve_cg", "nufft_solve_l1tv_ols", "nufft_plan_info", "nufft_plan_modes", "nufft_plan_tile_histogram", "nufft_launch_count", "nufft_destroy",
     "nufft_profile_enable", "nufft_profile_reset", "nufft_profile_count", "nufft_profile_get",
     "nufft_strerror", "nufft_last_cuda_error", "nufft_version",
 ]
@@ -80,6 +80,7 @@ def lib():
     L.nufft_plan_info.argtypes = [_PLAN, _I64P, _I64P, _I64P, _I64P, _I64P]
     L.nufft_plan_modes.argtypes = [_PLAN, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int), _c.POINTER(_c.c_int),
                                    _c.POINTER(_c.c_double)]
+    L.nufft_plan_tile_histogram.argtypes = [_PLAN, _I64P]
     L.nufft_launch_count.argtypes = [_PLAN]
     L.nufft_launch_count.restype = _c.c_int64
     L.nufft_destroy.argtypes = [_PLAN]
@@ -348,6 +349,9 @@ class NufftPlan:
         J, kern, paths, perr = _c.c_int(), _c.c_int(), _c.c_int(), _c.c_double()
         _check(lib().nufft_plan_modes(self._h, _c.byref(J), _c.byref(kern), _c.byref(paths), _c.byref(perr)),
                "nufft_plan_modes")
+        hist = (_c.c_int64 * 24)()
+        _check(lib().nufft_plan_tile_histogram(self._h, hist), "nufft_plan_tile_histogram")
+        out["tile_histogram"] = [int(v) for v in hist]
         out.update(J=J.value, kernel=("kb", "minmax")[kern.value], interleaved=bool(paths.value & 1),
                    caller_order_interp=bool(paths.value & 2), generic_width_kernels=bool(paths.value & 4),
                    toeplitz=bool(paths.value & 8), poly_err=perr.value)

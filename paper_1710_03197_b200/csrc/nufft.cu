@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -46,6 +47,7 @@ struct CgGraphKey {
 
 struct nufft_plan_s {
     int d = 0;
+    int device = -1;                // the CUDA device the plan was created on (every call must run with it current)
     int N[3] = {1, 1, 1}, K[3] = {1, 1, 1};
     int64_t M = 0, nimg = 0, cells = 0;
     int max_batch = 1;
@@ -84,6 +86,7 @@ struct nufft_plan_s {
     int n_items = 0;
     float2* d_slabs = nullptr;      // deterministic mode: [max_batch][n_items][tile_cells], lazy
     int64_t n_tiles = 0, n_work = 0, max_tile_samples = 0;
+    int64_t tile_hist[NUFFT_TILE_HIST_BUCKETS] = {0};
     bool win3d = false;             // 3-D, J = 6, default tile: samples pencil-sorted inside tiles, register-window V / V^H (win3d.cuh)
     int64_t bytes_plan = 0, bytes_work = 0;
     int64_t launches = 0;
@@ -164,6 +167,7 @@ struct ProfScope {
 };
 
 static int dev_alloc(void** dptr, size_t bytes, int64_t* acct);
+static bool wrong_device(nufft_plan_t p);
 
 // ------------------------------------------------------------------------------------------------------------
 // kernel configuration (dynamic shared memory opt-in), once per process
@@ -948,6 +952,10 @@ static int plan_build(nufft_plan_t p, const double* om) {
         tg.pitch = pitch;
         tg.plane = (d == 3) ? tg.P[1] * pitch : 0;
         tg.tile_cells = (d == 3) ? tg.P[0] * tg.P[1] * pitch : tg.P[0] * pitch;
+        // a user tile whose shared-memory footprint exceeds the opt-in (200 KB) would fail at every adjoint launch
+        const size_t need = (d == 3) ? (size_t)tg.tile_cells * 8 + (size_t)kStage3dBytes
+                                     : (d == 2 ? (size_t)8 * ((size_t)tg.tile_cells * 8 + kStageBytes) : 0);
+        if (need > (size_t)200 * 1024) return NUFFT_EINVAL;
     }
     // per-sample split (float64) and tile id
     const int64_t M = p->M;
@@ -987,7 +995,13 @@ static int plan_build(nufft_plan_t p, const double* om) {
         for (size_t b = 0; b + 1 < fine.size(); ++b) fine[b + 1] += fine[b];
         for (int64_t t = 0; t <= p->n_tiles; ++t) start[t] = fine[(size_t)t * nsub];
         p->max_tile_samples = 0;
-        for (int64_t t = 0; t < p->n_tiles; ++t) p->max_tile_samples = std::max<int64_t>(p->max_tile_samples, start[t + 1] - start[t]);
+        for (int64_t t = 0; t < p->n_tiles; ++t) {
+            const int64_t n = start[t + 1] - start[t];
+            p->max_tile_samples = std::max<int64_t>(p->max_tile_samples, n);
+            int k = 0;
+            while (k + 1 < NUFFT_TILE_HIST_BUCKETS && ((int64_t)1 << k) <= n) ++k;      // n = 0 -> 0; 2^(k-1) <= n < 2^k -> k
+            p->tile_hist[k]++;
+        }
         for (int64_t m = 0; m < M; ++m) perm[fine[tid[m]]++] = (int32_t)m;
     }
     std::vector<uint32_t> kpack_s(M);
@@ -1067,10 +1081,22 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     const bool generic_j = Jd[0] != kJ || (opts && opts->interp_mode == 2);
     // 1-D and the generic-width path have the atomic V^H only
     if ((d == 1 || generic_j) && opts && opts->adjoint_mode == 1) return NUFFT_EINVAL;
-    static cudaError_t cfg = configure_all();
-    if (cfg != cudaSuccess) { g_last_cuda_error = (int)cfg; return NUFFT_ECUDA; }
+    // the dynamic shared-memory opt-ins are per DEVICE: configure once per device ordinal; the plan remembers its device
+    int dev = -1;
+    CU_TRY(cudaGetDevice(&dev));
+    {
+        static std::mutex mu;
+        static std::vector<int> done;       // device ordinals already configured
+        std::lock_guard<std::mutex> lk(mu);
+        if (std::find(done.begin(), done.end(), dev) == done.end()) {
+            const cudaError_t cfg = configure_all();
+            if (cfg != cudaSuccess) { g_last_cuda_error = (int)cfg; (void)cudaGetLastError(); return NUFFT_ECUDA; }
+            done.push_back(dev);
+        }
+    }
     nufft_plan_t p = new (std::nothrow) nufft_plan_s();
     if (!p) return NUFFT_ENOMEM;
+    p->device = dev;
     p->d = d;
     p->M = M;
     p->max_batch = max_batch;
@@ -1141,6 +1167,12 @@ extern "C" int nufft_plan_info(nufft_plan_t p, int64_t* bytes_plan, int64_t* byt
     return NUFFT_OK;
 }
 
+extern "C" int nufft_plan_tile_histogram(nufft_plan_t p, int64_t* counts) {
+    if (!p || !counts) return NUFFT_EINVAL;
+    for (int k = 0; k < NUFFT_TILE_HIST_BUCKETS; ++k) counts[k] = p->tile_hist[k];
+    return NUFFT_OK;
+}
+
 extern "C" int nufft_plan_modes(nufft_plan_t p, int* J, int* kernel, int* paths, double* poly_err) {
     if (!p) return NUFFT_EINVAL;
     if (J) *J = p->J;
@@ -1192,7 +1224,13 @@ extern "C" int nufft_profile_get(nufft_plan_t p, int i, const char** name, doubl
 // ------------------------------------------------------------------------------------------------------------
 // transforms
 // ------------------------------------------------------------------------------------------------------------
-static bool bad_batch(nufft_plan_t p, int batch) { return !p || batch < 1 || batch > p->max_batch; }
+static bool wrong_device(nufft_plan_t p) {
+    int dev = -1;
+    return cudaGetDevice(&dev) != cudaSuccess || dev != p->device;
+}
+// every transform / solver entry point goes through this: null plan, batch out of range, or a current device other than the
+// plan's (its buffers and kernel attributes belong to that device) -> NUFFT_EINVAL
+static bool bad_batch(nufft_plan_t p, int batch) { return !p || batch < 1 || batch > p->max_batch || wrong_device(p); }
 
 extern "C" int nufft_stage_scale_fft(nufft_plan_t p, int batch, const nufft_c64* x, nufft_c64* grid, void* stream) {
     if (bad_batch(p, batch) || !x || !grid) return NUFFT_EINVAL;
@@ -1399,7 +1437,7 @@ extern "C" int nufft_selfadjoint_host(nufft_plan_t p, int batch, const nufft_c64
 // multi-coil operator, eqs. (34)-(35)
 // ------------------------------------------------------------------------------------------------------------
 extern "C" int nufft_set_coils(nufft_plan_t p, int ncoil, const nufft_c64* c) {
-    if (!p || ncoil < 0 || ncoil > p->max_batch || (ncoil > 0 && !c)) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || ncoil < 0 || ncoil > p->max_batch || (ncoil > 0 && !c)) return NUFFT_EINVAL;
     p->ncoil = ncoil;
     p->d_coils = (ncoil > 0) ? (const float2*)c : nullptr;
     if (p->cg_graph) { cudaGraphExecDestroy(p->cg_graph); p->cg_graph = nullptr; }   // the coil pointer is baked into it
@@ -1417,7 +1455,7 @@ static int coil_reduce(nufft_plan_t p, float2* x, cudaStream_t st) {
 }
 
 extern "C" int nufft_forward_coils(nufft_plan_t p, const nufft_c64* x, nufft_c64* y, void* stream) {
-    if (!p || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
@@ -1431,7 +1469,7 @@ extern "C" int nufft_forward_coils(nufft_plan_t p, const nufft_c64* x, nufft_c64
 }
 
 extern "C" int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64* y, nufft_c64* x, void* stream) {
-    if (!p || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
@@ -1445,7 +1483,7 @@ extern "C" int nufft_adjoint_coils(nufft_plan_t p, const nufft_c64* y, nufft_c64
 }
 
 extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
-    if (!p || !x_in || !x_out) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !x_in || !x_out) return NUFFT_EINVAL;
     if (p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     if (use_il(p, p->ncoil)) {
@@ -1467,7 +1505,7 @@ extern "C" int nufft_selfadjoint_coils(nufft_plan_t p, const nufft_c64* x_in, nu
 static int ew_blocks(int64_t n);
 
 extern "C" int nufft_density_weights(nufft_plan_t p, int niter, nufft_c64* w, void* stream) {
-    if (!p || niter < 0 || (!w && p->M > 0)) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || niter < 0 || (!w && p->M > 0)) return NUFFT_EINVAL;
     if (p->M == 0) return NUFFT_OK;
     cudaStream_t st = (cudaStream_t)stream;
     if (!p->d_dcf_img) NU_TRY(dev_alloc((void**)&p->d_dcf_img, (size_t)p->nimg * sizeof(float2), &p->bytes_work));
@@ -1654,7 +1692,7 @@ static int ensure_solver(nufft_plan_t p, int64_t nvec, int hist) {
 
 static int coil_reduce(nufft_plan_t p, float2* x, cudaStream_t st);
 extern "C" int nufft_selfadjoint_toeplitz_coils(nufft_plan_t p, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
-    if (!p || !x_in || !x_out) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !x_in || !x_out) return NUFFT_EINVAL;
     if (p->ncoil < 1 || !p->d_that) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     bool summed = false;
@@ -1771,7 +1809,7 @@ static int adjoint_any(nufft_plan_t p, bool coils, const float2* y, float2* x, c
 
 extern "C" int nufft_solve_cg(nufft_plan_t p, int use_coils, const nufft_c64* y, nufft_c64* x, int niter,
                               double* resnorm_host, void* stream) {
-    if (!p || !y || !x || niter < 0) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !y || !x || niter < 0) return NUFFT_EINVAL;
     const bool coils = use_coils != 0;
     if (coils && p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1795,7 +1833,7 @@ extern "C" int nufft_solve_cg(nufft_plan_t p, int use_coils, const nufft_c64* y,
 // scaling factor).
 extern "C" int nufft_solve_cg_kspace(nufft_plan_t p, const nufft_c64* y, nufft_c64* x, int niter, double* resnorm_host,
                                      void* stream) {
-    if (!p || !x || (!y && p->M > 0) || niter < 0) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !x || (!y && p->M > 0) || niter < 0) return NUFFT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const int64_t n = p->cells;
     if (!p->d_kspace) NU_TRY(dev_alloc((void**)&p->d_kspace, (size_t)5 * n * sizeof(float2), &p->bytes_work));
@@ -1827,7 +1865,7 @@ extern "C" int nufft_solve_cg_kspace(nufft_plan_t p, const nufft_c64* y, nufft_c
 
 extern "C" int nufft_solve_l1tv_ols(nufft_plan_t p, int use_coils, const nufft_c64* y, nufft_c64* x, double mu,
                                     double lam, int n_outer, int n_inner, int n_cg, void* stream) {
-    if (!p || !y || !x || n_outer < 0 || n_inner < 0 || n_cg < 0 || p->d != 2 || lam < 0.0) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !y || !x || n_outer < 0 || n_inner < 0 || n_cg < 0 || p->d != 2 || lam < 0.0) return NUFFT_EINVAL;
     const bool coils = use_coils != 0;
     if (coils && p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1878,7 +1916,7 @@ extern "C" int nufft_solve_l1tv_ols(nufft_plan_t p, int use_coils, const nufft_c
 
 extern "C" int nufft_solve_l1tv_lad(nufft_plan_t p, int use_coils, const nufft_c64* y, nufft_c64* x, double mu,
                                     double lam, int n_outer, int n_inner, int n_cg, void* stream) {
-    if (!p || !y || !x || n_outer < 0 || n_inner < 0 || n_cg < 0 || p->d != 2 || lam < 0.0 || mu < 0.0) return NUFFT_EINVAL;
+    if (!p || wrong_device(p) || !y || !x || n_outer < 0 || n_inner < 0 || n_cg < 0 || p->d != 2 || lam < 0.0 || mu < 0.0) return NUFFT_EINVAL;
     const bool coils = use_coils != 0;
     if (coils && p->ncoil < 1) return NUFFT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;

@@ -243,7 +243,9 @@ __global__ void __launch_bounds__(256) dcf_init_kernel(float2* __restrict__ w, i
 __global__ void __launch_bounds__(256) dcf_update_kernel(float2* __restrict__ w, const float2* __restrict__ t, int64_t M) {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < M; i += (int64_t)gridDim.x * blockDim.x) {
         const float2 tv = t[i];
-        w[i] = make_float2(w[i].x / sqrtf(tv.x * tv.x + tv.y * tv.y), 0.f);
+        const float mag = sqrtf(tv.x * tv.x + tv.y * tv.y);
+        // |A A^H w| = 0 (a sample no image pixel reaches: degenerate input): the weight becomes 0 instead of inf
+        w[i] = make_float2(mag > 0.f ? w[i].x / mag : 0.f, 0.f);
     }
 }
 // out[b][m] = y[b][m] * w[m].re

@@ -21,6 +21,26 @@ def rel(a, b):
     return np.linalg.norm(a - b) / np.linalg.norm(b)
 
 
+def maxabs(a, b):
+    """max |a - b| / max |b|: a single wrong cell or seam row cannot hide in it the way it can in an L2 norm."""
+    a = np.asarray(a).ravel()
+    b = np.asarray(b).ravel()
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+def tol_max(Jd):
+    """Elementwise bound: 50 eps32 sqrt(prod J) of the largest reference value -- 3.6e-5 in 2-D,
+    8.8e-5 in 3-D at J = 6; measured 3e-6 / 4e-7."""
+    return 50.0 * 1.1920929e-07 * float(np.sqrt(np.prod(Jd)))
+
+
+def close(a, ref, Jd, tol=None):
+    """The parity criterion of every transform test: relative L2 AND max-abs."""
+    e2, em = rel(a, ref), maxabs(a, ref)
+    assert e2 < (TOL if tol is None else tol) and em < tol_max(Jd), (e2, em)
+    return e2, em
+
+
 def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.complex64)).cuda()
 
@@ -108,8 +128,7 @@ def check_transforms(cfg, seed=0, **kw):
     yo = orc.forward(x.astype(np.complex128), om, Nd, Kd, Jd)
     xo = orc.adjoint(y.astype(np.complex128), om, Nd, Kd, Jd)
     so = orc.adjoint(yo, om, Nd, Kd, Jd)
-    errs = (rel(yg, yo), rel(xg, xo), rel(sg, so))
-    assert max(errs) < TOL, errs
+    errs = (close(yg, yo, Jd), close(xg, xo, Jd), close(sg, so, Jd))
     p.destroy()
     return errs
 
@@ -134,7 +153,7 @@ def test_config2_phantom_variant():
     x = wl.phantom(cfg["Nd"])
     yg = host(p.forward(dev(x)))[0]
     yo = orc.forward(x.astype(np.complex128), cfg["om"], cfg["Nd"], cfg["Kd"], cfg["Jd"])
-    assert rel(yg, yo) < TOL
+    close(yg, yo, cfg["Jd"])
 
 
 def test_config3_full_spiral_512():
@@ -200,7 +219,7 @@ def test_batch_equals_loop_of_singles():
         assert np.array_equal(yb[b], host(p1.forward(dev(x[b])))[0])
         assert np.array_equal(xb[b], host(p1.adjoint(dev(y[b])))[0])      # deterministic mode: bit-equal
     yo = orc.forward(x[3].astype(np.complex128), cfg["om"], cfg["Nd"], cfg["Kd"], cfg["Jd"])
-    assert rel(yb[3], yo) < TOL
+    close(yb[3], yo, cfg["Jd"])
 
 
 def test_plan_reuse_and_inplace_selfadjoint():
@@ -230,10 +249,11 @@ def test_adjoint_identity_on_gpu():
 # ---------------------------------------------------------------------------------------------------------
 # full-size configs on sampled outputs the oracle (or the plain definition) can compute one by one
 # ---------------------------------------------------------------------------------------------------------
-def test_config4_full_size_sampled():
-    """3-D 128^3 / 256^3 / M = 2,097,152: forward checked on 64 sampled outputs against the oracle's own stencil sum
-    over an oracle grid (float64 FFT of the same image); adjoint checked through the adjoint identity and on sampled
-    image voxels against the plain non-uniform DFT definition (kernel error ~1e-5)."""
+def test_config4_full_size_elementwise():
+    """BASELINE config 4 at full size (3-D 128^3 / 256^3, M = 2,097,152 kooshball): forward, adjoint and A^H A compared
+    with the float64 oracle ELEMENT BY ELEMENT (the oracle takes about 50 s per transform on one host core), plus the
+    adjoint on sampled voxels against the plain non-uniform DFT definition (kernel error ~1e-5).  This is the launch
+    configuration bench.py times: 11 264 work items, hot tiles split, largest tile 73 241 samples."""
     cfg = wl.config(3)
     Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
     p = make_plan(cfg)
@@ -242,16 +262,14 @@ def test_config4_full_size_sampled():
     xd, yd = dev(x), dev(y)
     Ax = host(p.forward(xd))[0]
     AHy = host(p.adjoint(yd))[0]
-    # forward: oracle grid once (float64 FFT), oracle interpolation at a sample subset
-    G = orc.scale_pad_fft(x.astype(np.complex128), Nd, Kd, Jd)
-    rng = np.random.default_rng(9)
-    sel = np.concatenate([rng.integers(0, om.shape[0], 4000), np.arange(250, 262)])   # incl. k-space centre
-    ref = orc.interp(G, om[sel], Nd, Kd, Jd)
-    assert rel(Ax[sel], ref) < TOL
-    # adjoint: identity <Ax, y> = <x, A^H y> with the GPU forward already validated above
-    lhs = np.vdot(Ax.astype(np.complex128), y.astype(np.complex128))
-    rhs = np.vdot(x.astype(np.complex128).ravel(), AHy.astype(np.complex128).ravel())
-    assert abs(lhs - rhs) / abs(lhs) < 2e-5
+    AHAx = host(p.selfadjoint(xd))[0]
+    p.destroy()
+    yo = orc.forward(x.astype(np.complex128), om, Nd, Kd, Jd)
+    close(Ax, yo, Jd)
+    xo = orc.adjoint(y.astype(np.complex128), om, Nd, Kd, Jd)
+    close(AHy, xo, Jd)
+    so = orc.adjoint(yo, om, Nd, Kd, Jd)
+    close(AHAx, so, Jd)
     # adjoint: sampled voxels against the plain definition (brute force over all M samples)
     vox = [(0, 0, 0), (64, 64, 64), (127, 127, 127), (5, 100, 77), (64, 0, 127)]
     for v in vox:
@@ -276,9 +294,9 @@ def test_multicoil_operator():
     yo = orc.forward_coils(x.astype(np.complex128), c128, om, Nd, Kd, Jd)
     xo = orc.adjoint_coils(y.astype(np.complex128), c128, om, Nd, Kd, Jd)
     so = orc.adjoint_coils(yo, c128, om, Nd, Kd, Jd)
-    assert rel(host(p.forward_coils(dev(x))), yo) < TOL
-    assert rel(host(p.adjoint_coils(dev(y))), xo) < TOL
-    assert rel(host(p.selfadjoint_coils(dev(x))), so) < TOL
+    close(host(p.forward_coils(dev(x))), yo, Jd)
+    close(host(p.adjoint_coils(dev(y))), xo, Jd)
+    close(host(p.selfadjoint_coils(dev(x))), so, Jd)
 
 
 @pytest.mark.parametrize("Nd,M,nc", [((16, 16, 16), 5003, 4), ((64,), 301, 3), ((32, 16, 32), 9001, 5)])
@@ -298,9 +316,9 @@ def test_multicoil_operator_3d_and_1d(Nd, M, nc):
     yo = orc.forward_coils(x.astype(np.complex128), c128, om, Nd, Kd, Jd)
     xo = orc.adjoint_coils(y.astype(np.complex128), c128, om, Nd, Kd, Jd)
     so = orc.adjoint_coils(yo, c128, om, Nd, Kd, Jd)
-    assert rel(host(p.forward_coils(dev(x))), yo) < TOL
-    assert rel(host(p.adjoint_coils(dev(y))), xo) < TOL
-    assert rel(host(p.selfadjoint_coils(dev(x))), so) < TOL
+    close(host(p.forward_coils(dev(x))), yo, Jd)
+    close(host(p.adjoint_coils(dev(y))), xo, Jd)
+    close(host(p.selfadjoint_coils(dev(x))), so, Jd)
     AHA = lambda z: orc.selfadjoint_coils(z, c128, om, Nd, Kd, Jd)
     xc, _ = sol.cg(AHA, xo, 3)
     assert rel(host(p.solve_cg(dev(y), 3, use_coils=True)), xc) < 1e-4
@@ -394,8 +412,7 @@ def check_batched(cfg, B, sample_imgs, seed=0):
         yo = orc.forward(x[b].astype(np.complex128), om, Nd, Kd, Jd)
         xo = orc.adjoint(y[b].astype(np.complex128), om, Nd, Kd, Jd)
         so = orc.adjoint(yo, om, Nd, Kd, Jd)
-        errs = (rel(yg[b], yo), rel(xg[b], xo), rel(sg[b], so))
-        assert max(errs) < TOL, (b, errs)
+        errs = (close(yg[b], yo, Jd), close(xg[b], xo, Jd), close(sg[b], so, Jd))
     # gather-form V^H: bit-reproducible run to run
     again = host(p.adjoint(dev(y)))
     assert np.array_equal(xg.view(np.uint32), again.view(np.uint32))
@@ -414,7 +431,7 @@ def test_interleaved_coherent_caller_order_interp_matches_sorted_path():
     yc, ys = host(pc.forward(dev(x))), host(ps.forward(dev(x)))
     assert rel(yc, ys) < 1e-6
     yo = orc.forward(x[39].astype(np.complex128), cfg["om"], cfg["Nd"], cfg["Kd"], cfg["Jd"])
-    assert rel(yc[39], yo) < TOL
+    close(yc[39], yo, cfg["Jd"])
     pc.destroy()
     ps.destroy()
 
@@ -466,9 +483,9 @@ def test_interleaved_multicoil_operator_16_coils():
     yo = orc.forward_coils(x.astype(np.complex128), c128, om, Nd, Kd, Jd)
     xo = orc.adjoint_coils(y.astype(np.complex128), c128, om, Nd, Kd, Jd)
     so = orc.adjoint_coils(yo, c128, om, Nd, Kd, Jd)
-    assert rel(host(p.forward_coils(dev(x))), yo) < TOL
-    assert rel(host(p.adjoint_coils(dev(y))), xo) < TOL
-    assert rel(host(p.selfadjoint_coils(dev(x))), so) < TOL
+    close(host(p.forward_coils(dev(x))), yo, Jd)
+    close(host(p.adjoint_coils(dev(y))), xo, Jd)
+    close(host(p.selfadjoint_coils(dev(x))), so, Jd)
 
 
 def test_host_buffer_pipeline_matches_device_calls():
@@ -489,7 +506,7 @@ def test_host_buffer_pipeline_matches_device_calls():
         assert rel(ax.numpy(), host(p.adjoint(dev(y)))) < 2e-6
         assert rel(sx.numpy(), host(p.selfadjoint(dev(x)))) < 2e-6
     yo = orc.forward(x[37].astype(np.complex128), cfg["om"], cfg["Nd"], cfg["Kd"], cfg["Jd"])
-    assert rel(fy.numpy()[37], yo) < TOL
+    close(fy.numpy()[37], yo, cfg["Jd"])
     # relaxed input ordering (nufft_host_input_ready): back-to-back calls whose copies in overlap the previous copies back
     p.host_input_ready(True)
     ref = host(p.selfadjoint(dev(x)))
@@ -516,9 +533,9 @@ def test_config5_full_size_32_coils_sampled():
     yg = host(p.forward_coils(dev(x)))
     for i in (0, 13, 31):
         yo = orc.forward(c128[i] * x.astype(np.complex128), om, Nd, Kd, Jd)
-        assert rel(yg[i], yo) < TOL
+        close(yg[i], yo, Jd)
     xo = orc.adjoint_coils(y.astype(np.complex128), c128, om, Nd, Kd, Jd)
-    assert rel(host(p.adjoint_coils(dev(y))), xo) < TOL
+    close(host(p.adjoint_coils(dev(y))), xo, Jd)
     p.destroy()
 
 
@@ -558,14 +575,83 @@ def test_l1tv_ols_16_coils_interleaved_path():
     p.destroy()
 
 
-def test_cg_config3_parity_against_the_oracles_own_noise_floor(repo_root):
-    """SURVEY 7.3-3: the VD spiral leaves the k-space corners unsampled, A^H A has a near-null space and CG amplifies any
-    perturbation there.  Measure, on the scaled config 3 (128^2), (i) GPU vs oracle and (ii) the oracle against itself
-    with 1e-12 relative noise injected into every operator application, at iterations 1, 5, 10, 50; the GPU may exceed
-    1e-4 only where the float64 floor itself is within two orders of magnitude of it.  Numbers go to
-    gpurun_out/cg_floor.json (quoted in DESIGN.md)."""
-    import json
+def _coil_ops_threaded(c128, om, Nd, Kd, Jd, with_forward=False):
+    """A_multi^H A_multi and A_multi^H of the oracle, the per-coil transforms (oracle/nufft_oracle.py forward / adjoint,
+    unchanged) evaluated on a thread pool: same arithmetic, same fixed summation order over the coils."""
+    import concurrent.futures as cf
     import os
+    pool = cf.ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1))
+
+    def AHy(y):
+        parts = list(pool.map(lambda i: np.conj(c128[i]) * orc.adjoint(y[i], om, Nd, Kd, Jd), range(len(c128))))
+        out = np.zeros(tuple(Nd), dtype=np.complex128)
+        for q in parts:
+            out += q
+        return out
+
+    def AHA(z):
+        parts = list(pool.map(lambda i: np.conj(c128[i]) * orc.adjoint(orc.forward(c128[i] * z, om, Nd, Kd, Jd), om, Nd, Kd, Jd),
+                              range(len(c128))))
+        out = np.zeros(tuple(Nd), dtype=np.complex128)
+        for q in parts:
+            out += q
+        return out
+
+    def A(z):
+        return np.stack(list(pool.map(lambda i: orc.forward(c128[i] * z, om, Nd, Kd, Jd), range(len(c128)))))
+    return (AHA, AHy, A) if with_forward else (AHA, AHy)
+
+
+def test_l1tv_ols_config5_r17_iteration_counts_128():
+    """BASELINE config 5's solver at reading R17's counts -- n_outer = 4, n_inner = 5 (20 split-Bregman iterations),
+    n_cg = 3, mu = 1, lambda = 0.02 -- on the scaled problem (128^2, 8 coils, radial 64 x 256): solver output vs the
+    float64 oracle <= 1e-4 (north star)."""
+    cfg = wl.config(4, scale=2)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    nc = cfg["ncoil"]
+    c = wl.coil_maps(nc, Nd)
+    c128 = c.astype(np.complex128)
+    xt = wl.phantom(Nd)
+    y = orc.forward_coils(xt.astype(np.complex128), c128, om, Nd, Kd, Jd)
+    y = (y + wl.noise_like(y)).astype(np.complex64)
+    p = make_plan(cfg, max_batch=nc)
+    p.set_coils(dev(c))
+    AHA, AHy = _coil_ops_threaded(c128, om, Nd, Kd, Jd)
+    xo = sol.l1tv_ols(AHA, AHy(y.astype(np.complex128)), 1.0, 0.02, 4, 5, 3)
+    xg = host(p.solve_l1tv_ols(dev(y), 1.0, 0.02, 4, 5, 3, use_coils=True))
+    assert rel(xg, xo) < 1e-4 and maxabs(xg, xo) < 1e-3, (rel(xg, xo), maxabs(xg, xo))
+    p.destroy()
+
+
+def test_l1tv_ols_config5_full_size_32_coils_one_outer_group():
+    """BASELINE config 5 at FULL size (256^2, 32 coils, radial 128 x 512, interleaved path): one outer group of R17's
+    schedule (n_outer = 1, n_inner = 5, n_cg = 3: 5 of the 20 split-Bregman iterations, 21 applications of the 32-coil
+    A^H A) against the float64 oracle, <= 1e-4."""
+    cfg = wl.config(4)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    nc = cfg["ncoil"]
+    assert nc == 32
+    c = wl.coil_maps(nc, Nd)
+    c128 = c.astype(np.complex128)
+    xt = wl.phantom(Nd)
+    AHA, AHy, A = _coil_ops_threaded(c128, om, Nd, Kd, Jd, with_forward=True)
+    p = make_plan(cfg, max_batch=nc)
+    p.set_coils(dev(c))
+    y = A(xt.astype(np.complex128))                         # data from the oracle's forward operator
+    y = (y + wl.noise_like(y)).astype(np.complex64)
+    xo = sol.l1tv_ols(AHA, AHy(y.astype(np.complex128)), 1.0, 0.02, 1, 5, 3)
+    xg = host(p.solve_l1tv_ols(dev(y), 1.0, 0.02, 1, 5, 3, use_coils=True))
+    assert rel(xg, xo) < 1e-4 and maxabs(xg, xo) < 1e-3, (rel(xg, xo), maxabs(xg, xo))
+    p.destroy()
+
+
+def test_cg_config3_parity_against_the_problems_own_amplification():
+    """SURVEY 7.3-3: the VD spiral leaves the k-space corners unsampled, A^H A has a near-null space and CG amplifies any
+    perturbation of the operator.  The GPU operator agrees with the oracle to ~3e-7 per application, so its CG iterates can
+    be no closer to the oracle's than the oracle's own iterates are when ITS operator is perturbed by 3e-7 (relative,
+    random, three seeds).  Asserted at iterations 1, 5, 10 and 50 on the scaled config 3 (128^2):
+        GPU vs oracle  <=  max(1e-4, 3 x the largest perturbed-oracle deviation)
+    (1e-4 = the north star's solver bar; it holds outright at iterations 1 and 5).  DESIGN.md section 3 quotes the numbers."""
     cfg = wl.config(2, scale=4)
     Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
     p = make_plan(cfg)
@@ -574,25 +660,24 @@ def test_cg_config3_parity_against_the_oracles_own_noise_floor(repo_root):
     y = (y + wl.noise_like(y)).astype(np.complex64)
     AHy = orc.adjoint(y.astype(np.complex128), om, Nd, Kd, Jd)
     AHA = lambda z: orc.selfadjoint(z, om, Nd, Kd, Jd)
-    rng = np.random.default_rng(77)
 
-    def AHA_noisy(z):
-        r = AHA(z)
-        return r * (1.0 + 1e-12 * (rng.standard_normal(r.shape) + 1j * rng.standard_normal(r.shape)))
+    def perturbed(seed):
+        rng = np.random.default_rng(seed)
 
-    out = {}
+        def op(z):
+            r = AHA(z)
+            return r * (1.0 + 3e-7 * (rng.standard_normal(r.shape) + 1j * rng.standard_normal(r.shape)))
+        return op
+
+    report = {}
     for niter in (1, 5, 10, 50):
         xo, _ = sol.cg(AHA, AHy, niter)
-        xn, _ = sol.cg(AHA_noisy, AHy, niter)
-        xg = host(p.solve_cg(dev(y), niter))
-        out[niter] = {"gpu_vs_oracle": float(rel(xg, xo)), "oracle_noise_floor_1e-12": float(rel(xn, xo))}
-    d = os.path.join(repo_root, "gpurun_out")
-    if os.path.isdir(d):
-        with open(os.path.join(d, "cg_floor.json"), "w") as f:
-            json.dump(out, f, indent=1)
-    assert out[1]["gpu_vs_oracle"] < 1e-4 and out[5]["gpu_vs_oracle"] < 1e-4
-    for niter, v in out.items():
-        assert v["gpu_vs_oracle"] < max(1e-4, 1e9 * v["oracle_noise_floor_1e-12"]), (niter, v)
+        floor = max(rel(sol.cg(perturbed(seed), AHy, niter)[0], xo) for seed in (77, 78, 79))
+        err = rel(host(p.solve_cg(dev(y), niter)), xo)
+        report[niter] = (float(err), float(floor))
+        assert err < max(1e-4, 3.0 * floor), report
+    assert report[1][0] < 1e-4 and report[5][0] < 1e-4, report
+    print("cg parity (gpu vs oracle, oracle with 3e-7 operator noise):", report)
     p.destroy()
 
 
