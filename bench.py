@@ -269,6 +269,12 @@ def run_ours(args):
         torch.cuda.synchronize()
         return sum(a.elapsed_time(b) for a, b in evs)
 
+    def timed_median(fn, min_ms=50.0, reps=5):
+        """ms per call: `reps` repetitions of >= min_ms of timed calls each (L2 flushed before every call), the median."""
+        est = max(timed(fn, 5) / 5, 1e-3)
+        n = max(5, int(np.ceil(min_ms / est)))
+        return float(np.median([timed(fn, n) / n for _ in range(reps)]))
+
     def barrier():
         if world > 1:
             dist.barrier()
@@ -298,14 +304,35 @@ def run_ours(args):
         clocks["note"] = ("sampled every 50 ms from the start of the timed region through a 0.6 s untimed continuation of "
                           "the same step (the timed region itself is ~10 ms)")
 
-    plan.host_input_ready(True)      # x_host is constant: the copy in of step k+1 may overlap the copy back of step k
+    # e2e, STRICT stream order (the headline e2e number): every copy in is ordered after the L2 flush and the start event
+    # on the caller's stream, so no byte of a step's H2D traffic can move outside that step's event bracket
+    y_host = torch.empty((B, M), dtype=torch.complex64).pin_memory()
+
+    def step_e2e_two_calls():
+        # the same pair as two host-buffer calls: y goes back to the host and comes in again (what a caller who keeps y does)
+        plan.forward_host(x_host, y_host)
+        plan.adjoint_host(y_host, xo_host)
+
+    plan.host_input_ready(False)
     for _ in range(2):
         step_e2e()
     barrier()
     e2e_ms = timed(step_e2e, K_steps)
     barrier()
+    for _ in range(2):
+        step_e2e_two_calls()
+    e2e2_ms = timed(step_e2e_two_calls, K_steps)
+    barrier()
+    # relaxed: the caller promises the host input is final at call time (nufft_host_input_ready), so the copy in of step k + 1
+    # may overlap the copy back of step k -- and, in this loop, the untimed flush between the brackets: context only
+    plan.host_input_ready(True)
+    for _ in range(2):
+        step_e2e()
+    e2e_relaxed_ms = timed(step_e2e, K_steps)
+    plan.host_input_ready(False)
+    barrier()
 
-    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, "cuda")
+    total_ms, e2e_ms, e2e2_ms, e2e_relaxed_ms = max_over_ranks([total_ms, e2e_ms, e2e2_ms, e2e_relaxed_ms], world, "cuda")
 
     # per-kernel device times of the same step (library-side CUDA events on the launch stream)
     peak, peak_src = measured_peak()
@@ -316,7 +343,8 @@ def run_ours(args):
     plan.profile_enable(False)
 
     # forward, adjoint and A^H A alone (north star: absolute transforms/s and fraction of the HBM roofline), same batch,
-    # L2 flushed between calls; A^H A keeps y on the device in the interleaved layout (no layout pass either way)
+    # L2 flushed between calls, median of 5 repetitions of >= 50 ms each; A^H A keeps y on the device in the interleaved
+    # layout (no layout pass either way)
     ab = algorithmic_bytes(2, Nd[0], Kd[0], M, B)
     fwd_bytes = ab["fft_rows_fwd"] + ab["fft_cols_fwd"] + ab["interp"]
     adj_bytes = ab["gridding"] + ab["fft_cols_adj"] + ab["fft_rows_adj"]
@@ -325,9 +353,27 @@ def run_ours(args):
                              ("adjoint", lambda: plan.adjoint(y, xo), adj_bytes),
                              ("selfadjoint", lambda: plan.selfadjoint(x, xo), fwd_bytes + adj_bytes)):
         fn()
-        ms = timed(fn, K_steps) / K_steps
+        ms = timed_median(fn)
         transforms[name] = {"transforms_per_s": world * B / (ms * 1e-3), "ms_per_call": ms, "alg_bytes_per_call": int(nbytes),
                             "frac_of_hbm_roofline": (nbytes / (ms * 1e-3) / 1e9) / peak}
+
+    # the batch-32 point (one interleaved group) of the same workload
+    batch32 = None
+    if world == 1 and B != 32:
+        p32 = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=32)
+        x32, y32, xo32 = x[:32].contiguous(), y[:32].contiguous(), xo[:32].contiguous()
+
+        def step32():
+            p32.forward(x32, y32)
+            p32.adjoint(y32, xo32)
+
+        for _ in range(3):
+            step32()
+        ms32 = timed_median(step32)
+        b32 = algorithmic_bytes(2, Nd[0], Kd[0], M, 32)
+        batch32 = {"batch": 32, "ms_per_step": ms32, "pairs_per_s": 32 / (ms32 * 1e-3),
+                   "step_frac_of_roofline": (sum(b32.values()) / (ms32 * 1e-3) / 1e9) / peak}
+        p32.destroy()
 
     result = None
     if rank == 0:
@@ -335,15 +381,7 @@ def run_ours(args):
         value = aggregate_pairs_per_s(world, B, ms_per_step)
         timed_kernels = {k: v for k, v in rows.items() if "alg_bytes" in v}
         dom = max(timed_kernels, key=lambda k: timed_kernels[k]["ms_per_launch"])
-        traffic = None
-        try:    # DRAM bytes per launch of the dominant kernel, from the committed ncu --set full capture
-            import csv
-            with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
-                for row in csv.DictReader(f):
-                    if row["config"] == "cfg2_batch%d" % B and row["kernel"] == dom:
-                        traffic = int(row["dram_bytes_per_launch"])
-        except Exception:
-            pass
+        traffic = dram_traffic("cfg2_batch%d" % B, dom)     # from the committed ncu --set full capture of this workload
         step_bytes = sum(v["alg_bytes"] for v in timed_kernels.values())
         roofline = {
             "bound": "hbm", "kernel": dom, "achieved": timed_kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
@@ -374,16 +412,38 @@ def run_ours(args):
             "e2e": {"value": world * B / (e2e_ms / K_steps * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": int(x_host.numel() * 8), "d2h_bytes_per_step": int(xo_host.numel() * 8),
                     "ms_per_step": e2e_ms / K_steps,
-                    "call": "nufft_selfadjoint_host: A^H(A x) per image, y kept on the device, 32-image chunks pipelined "
-                            "H2D / kernels / D2H"},
+                    "order": "strict: copies in are ordered after the caller's stream (flush + start event), nothing moves "
+                             "outside the event bracket",
+                    "call": "nufft_selfadjoint_host: the forward+adjoint pair A^H(A x) per image with y kept on the device "
+                            "(sorted-walk V, no layout pass), 32-image chunks pipelined H2D / kernels / D2H",
+                    "relaxed_input_ready": {"value": world * B / (e2e_relaxed_ms / K_steps * 1e-3),
+                                            "note": "nufft_host_input_ready(1): the copy in of a call may start before the "
+                                                    "previous work on the caller's stream ends (here: during the untimed "
+                                                    "flush) -- context, not the e2e number"},
+                    "forward_host_plus_adjoint_host": {
+                        "value": world * B / (e2e2_ms / K_steps * 1e-3), "ms_per_step": e2e2_ms / K_steps,
+                        "h2d_bytes_per_step": int(x_host.numel() * 8 + y_host.numel() * 8),
+                        "d2h_bytes_per_step": int(y_host.numel() * 8 + xo_host.numel() * 8),
+                        "note": "the same kernels as `value` (nufft_forward + nufft_adjoint), y through the host"}},
             "gpu_launches": int(l1 - l0),
             "roofline": roofline,
             "transforms": transforms,
+            "batch32": batch32,
             "cpu_baseline": {"value": 1.0 / cpu_s, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
                              "sample": "%d forward+adjoint pairs on one image of the workload (batch element 0)" % cpu_n},
             "paper_context": "PAPER.md Table 1 (:299-300): forward 6 ms + adjoint 6 ms on one K80 GK210 (PyCUDA), "
                              "workload sizes not stated by the paper",
         }
+        if world == 1:
+            # the 3-D half of the metric (BASELINE: "(2D 256^2, 3D 128^3)"), a record of its own next to the headline
+            try:
+                result["cfg4_3d"] = cfg4_record(nb, torch, peak, peak_src, args.cpu_seconds)
+            except Exception as e:
+                result["cfg4_3d"] = {"error": repr(e)}
+            try:
+                result["parity"] = parity_block(nb, torch)
+            except Exception as e:
+                result["parity"] = {"error": repr(e)}
         if world == 1 and not args.no_extra:
             try:
                 result["extra"] = extra_legs(nb, torch, peak, args)
@@ -398,8 +458,138 @@ def run_ours(args):
     return 0
 
 
+def dram_traffic(config, kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/dram_traffic.csv), or None."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["config"] == config and row["kernel"] == kernel:
+                    return int(row["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
+def _events_ms(torch, fn, n, flush):
+    evs = []
+    for _ in range(n):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        evs.append((a, b))
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in evs]
+
+
+def cfg4_record(nb, torch, peak, peak_src, cpu_seconds):
+    """The 3-D half of the metric (BASELINE config 4: Nd = 128^3, Kd = 256^3, Jd = 6^3, M = 2 097 152 kooshball), batch 1:
+    pairs/s, per-kernel roofline, e2e through the host-buffer calls, the oracle on a bounded sample."""
+    cfg = wl.config(3)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    N, K, M = Nd[0], Kd[0], om.shape[0]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    p = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=1)
+    x_host = torch.from_numpy(wl.image_gaussian(Nd)).reshape(1, *Nd).pin_memory()
+    x = x_host.cuda()
+    y = p.forward(x)
+    xo = p.adjoint(y)
+
+    def step():
+        p.forward(x, y)
+        p.adjoint(y, xo)
+
+    for _ in range(3):
+        step()
+    est = max(float(np.median(_events_ms(torch, step, 5, flush))), 1e-3)
+    n = max(5, int(np.ceil(50.0 / est)))
+    l0 = p.launch_count()
+    ms_pair = float(np.median([np.sum(_events_ms(torch, step, n, flush)) / n for _ in range(5)]))
+    launches = (p.launch_count() - l0) // (5 * n)
+    f_ms = float(np.median(_events_ms(torch, lambda: p.forward(x, y), 10, flush)))
+    a_ms = float(np.median(_events_ms(torch, lambda: p.adjoint(y, xo), 10, flush)))
+    s_ms = float(np.median(_events_ms(torch, lambda: p.selfadjoint(x, xo), 10, flush)))
+    p.profile_enable(True)
+    p.profile_reset()
+    _events_ms(torch, step, 5, flush)
+    ab = algorithmic_bytes(3, N, K, M, 1, cov=0.55)
+    rows = kernel_table(p.profile(), ab, peak)
+    p.profile_enable(False)
+    timed_k = {k: v for k, v in rows.items() if "alg_bytes" in v}
+    dom = max(timed_k, key=lambda k: timed_k[k]["ms_per_launch"])
+    step_bytes = sum(v["alg_bytes"] for v in timed_k.values())
+    # e2e: pinned x -> H2D -> A -> D2H y ; pinned y -> H2D -> A^H -> D2H x'  (strict stream order)
+    y_host = torch.empty((1, M), dtype=torch.complex64).pin_memory()
+    xo_host = torch.empty((1,) + tuple(Nd), dtype=torch.complex64).pin_memory()
+
+    def step_e2e():
+        p.forward_host(x_host, y_host)
+        p.adjoint_host(y_host, xo_host)
+
+    for _ in range(2):
+        step_e2e()
+    e2e_ms = float(np.median(_events_ms(torch, step_e2e, 5, flush)))
+    info = p.info()
+    p.destroy()
+    # the oracle on a bounded sample of the same workload: the first 512 of the 4096 spokes on the full 128^3 / 256^3 geometry
+    sub = om[: 512 * 512]
+    x128 = wl.image_gaussian(Nd).astype(np.complex128)
+    from oracle import nufft_oracle as orc
+    t0, c0 = time.perf_counter(), time.process_time()
+    orc.adjoint(orc.forward(x128, sub, Nd, Kd, Jd), sub, Nd, Kd, Jd)
+    el = time.perf_counter() - t0
+    return {
+        "metric": METRIC, "unit": UNIT, "value": 1e3 / ms_pair, "ms_per_step": ms_pair, "gpu_launches_per_step": int(launches),
+        "config": {"workload": "cfg4_3d_kooshball: Nd=128^3 Kd=256^3 Jd=6^3 M=2097152 (4096 spokes x 512), complex64",
+                   "batch": 1, "l2": "flushed between steps (256 MiB memset); the 134 MB grid exceeds L2 anyway",
+                   "timing": "median of 5 repetitions of >= 50 ms of event-bracketed steps"},
+        "forward_ms": f_ms, "adjoint_ms": a_ms, "selfadjoint_ms": s_ms,
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": timed_k[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                     "frac": timed_k[dom]["frac"], "traffic": dram_traffic("cfg4_batch1", dom), "peak_source": peak_src,
+                     "alg_bytes_per_launch": timed_k[dom]["alg_bytes"], "ms_per_launch": timed_k[dom]["ms_per_launch"],
+                     "step_alg_bytes": int(step_bytes),
+                     "step_frac_of_roofline": (step_bytes / (ms_pair * 1e-3) / 1e9) / peak, "kernels": rows,
+                     "traffic_by_kernel": {k: dram_traffic("cfg4_batch1", k) for k in timed_k},
+                     "note": "interp alg_bytes use coverage 0.55 of the 256^3 grid (SURVEY.md 8(d)); V and V^H are bound by "
+                             "issue slots / shared-memory traffic of the 216-point stencil before HBM (SURVEY 7.3-1: ceiling "
+                             "16-20 % of HBM peak)"},
+        "e2e": {"value": 1e3 / e2e_ms, "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": int(x_host.numel() * 8 + y_host.numel() * 8),
+                "d2h_bytes_per_step": int(y_host.numel() * 8 + xo_host.numel() * 8),
+                "call": "nufft_forward_host + nufft_adjoint_host, pinned buffers, strict stream order"},
+        "cpu_baseline": {"value": 1.0 / el, "unit": UNIT, "cores": cores_used(time.process_time() - c0, el), "kind": "oracle",
+                         "sample": "one forward+adjoint pair on the first 512 of the 4096 spokes (M = 262144) with the full "
+                                   "128^3 / 256^3 geometry: %.1f s" % el},
+        "plan": info,
+    }
+
+
+def parity_block(nb, torch):
+    """Relative L2 and max-abs (of the largest reference value) of forward / adjoint / A^H A against the float64 oracle,
+    on config 1 and the scaled config 4, computed in this very run (SURVEY section 5 "Metrics")."""
+    from oracle import nufft_oracle as orc
+    out = {}
+    for name, cfg in (("cfg1_2d_64", wl.config(0)), ("cfg4_3d_scaled_32", wl.config(3, scale=4))):
+        Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+        x = wl.image_gaussian(Nd)
+        y = wl.data_gaussian(om.shape[0])
+        p = nb.NufftPlan(Nd, Kd, Jd, om)
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        got = (p.forward(dev(x)).cpu().numpy()[0], p.adjoint(dev(y)).cpu().numpy()[0], p.selfadjoint(dev(x)).cpu().numpy()[0])
+        p.destroy()
+        yo = orc.forward(x.astype(np.complex128), om, Nd, Kd, Jd)
+        ref = (yo, orc.adjoint(y.astype(np.complex128), om, Nd, Kd, Jd), orc.adjoint(yo, om, Nd, Kd, Jd))
+        out[name] = {k: {"rel_l2": float(np.linalg.norm(g.ravel() - r.ravel()) / np.linalg.norm(r.ravel())),
+                         "max_abs_over_max_ref": float(np.abs(g.ravel() - r.ravel()).max() / np.abs(r).max())}
+                     for k, g, r in zip(("forward", "adjoint", "selfadjoint"), got, ref)}
+    out["bounds"] = {"rel_l2": 2e-5, "max_abs_over_max_ref": "50 eps32 sqrt(prod J): 3.6e-5 (2-D), 8.8e-5 (3-D)"}
+    return out
+
+
 def extra_legs(nb, torch, peak, args):
-    """Other BASELINE configs on one GPU: batch-1 latency of config 2 and the 3-D config 4 (forward and adjoint)."""
+    """Other BASELINE configs on one GPU: batch-1 latency of config 2, config 3 (CG), config 5 (L1TV-OLS), variants."""
     out = {}
 
     def time_calls(fn, n, flush):
@@ -452,27 +642,6 @@ def extra_legs(nb, torch, peak, args):
                                "selfadjoint_graph_ms": time_side(lambda: pg.selfadjoint(x, xo), 20)})
     torch.cuda.current_stream().wait_stream(side)
     pg.destroy()
-    # config 4, 3-D
-    cfg = wl.config(3)
-    N, K, M = cfg["Nd"][0], cfg["Kd"][0], cfg["om"].shape[0]
-    p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1)
-    x = torch.from_numpy(wl.image_gaussian(cfg["Nd"])).cuda().reshape(1, *cfg["Nd"])
-    y = p.forward(x)
-    xo = p.adjoint(y)
-    for _ in range(2):
-        p.forward(x, y), p.adjoint(y, xo)
-    f_ms = time_calls(lambda: p.forward(x, y), 5, flush)
-    a_ms = time_calls(lambda: p.adjoint(y, xo), 5, flush)
-    p.profile_enable(True)
-    p.profile_reset()
-    for _ in range(3):
-        flush.zero_()
-        p.forward(x, y)
-        p.adjoint(y, xo)
-    torch.cuda.synchronize()
-    rows = kernel_table(p.profile(), algorithmic_bytes(3, N, K, M, 1, cov=0.55), peak)
-    info = p.info()
-    p.destroy()
     # config 3: 2-D variable-density spiral 512^2, 50 CG iterations on A^H A x = A^H y (batch 1, planar path)
     cfg = wl.config(2)
     p = nb.NufftPlan(cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"], max_batch=1)
@@ -623,10 +792,6 @@ def extra_legs(nb, torch, peak, args):
                               "ms": time_calls(lambda: torch.fft.fftn(gref, dim=(1, 2)), 10, flush),
                               "ours_F_ms": "roofline.stages_ms['F (S+pad+FFT)'] (pruned, S and zero-pad fused)"}
     del gref
-    out["cfg4_3d_kooshball"] = {
-        "workload": "Nd=128^3 Kd=256^3 Jd=6^3 M=2097152 kooshball, batch 1", "forward_ms": f_ms, "adjoint_ms": a_ms,
-        "pairs_per_s": 1e3 / (f_ms + a_ms), "kernels": rows, "plan": info,
-        "note": "interp alg_bytes use coverage 0.55 of the 256^3 grid (SURVEY.md 8(d))"}
     return out
 
 
@@ -639,9 +804,22 @@ def main():
     ap.add_argument("--batch", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-extra", action="store_true")
+    ap.add_argument("--only", default="", choices=["", "cfg4"],
+                    help="cfg4: measure only the 3-D config 4 record and print it as the JSON line (used by the ncu "
+                         "commands in profiles/)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.only == "cfg4":
+        import torch
+        import paper_1710_03197_b200 as nb
+        torch.cuda.set_device(0)
+        peak, peak_src = measured_peak()
+        rec = cfg4_record(nb, torch, peak, peak_src, args.cpu_seconds)
+        rec.update({"n_gpus": 1, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                    "dtype": "complex64 (f32 arithmetic)", "data": "synthetic"})
+        print(json.dumps(rec))
+        return 0
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
                "--master-addr", "127.0.0.1", "--master-port", "29533", os.path.abspath(__file__)] + sys.argv[1:]

@@ -140,7 +140,7 @@ class NufftPlan:
     """
 
     def __init__(self, Nd, Kd, Jd, om, max_batch=1, adjoint_mode=0, interp_mode=0, tile=None, max_subtile=0,
-                 batch_layout=0, use_graphs=0, kernel="kb"):
+                 batch_layout=0, use_graphs=0, kernel="kb", coef_mode=0):
         L = lib()
         self.Nd = tuple(int(n) for n in Nd)
         self.Kd = tuple(int(k) for k in Kd)
@@ -156,6 +156,7 @@ class NufftPlan:
         self.cells = int(np.prod(self.Kd))
         opts = NufftOpts()
         _check(L.nufft_default_opts(_c.byref(opts)), "nufft_default_opts")
+        opts.coef_mode = int(coef_mode)
         opts.adjoint_mode = int(adjoint_mode)
         opts.interp_mode = int(interp_mode)
         opts.max_subtile = int(max_subtile)

@@ -87,6 +87,9 @@ struct nufft_plan_s {
     float2* d_slabs = nullptr;      // deterministic mode: [max_batch][n_items][tile_cells], lazy
     int64_t n_tiles = 0, n_work = 0, max_tile_samples = 0;
     int64_t tile_hist[NUFFT_TILE_HIST_BUCKETS] = {0};
+    float* d_w3rec = nullptr;       // coef_mode = 1, win3d: per-sample records [M][28] (padded weights, window key, caller index)
+    float* d_il_wv = nullptr;       // coef_mode = 1, interleaved V: padded weights [M][16] in V order / caller order
+    float* d_il_wv_c = nullptr;
     bool win3d = false;             // 3-D, J = 6, default tile: samples pencil-sorted inside tiles, register-window V / V^H (win3d.cuh)
     int64_t bytes_plan = 0, bytes_work = 0;
     int64_t launches = 0;
@@ -216,8 +219,10 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_il_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<2>::BYTES)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
 #define NU_W3_CFG(NW)                                                                                                                   \
-    if ((e = cudaFuncSetAttribute(interp_win_3d_kernel<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;   \
-    if ((e = cudaFuncSetAttribute(gridding_win_3d_kernel<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(interp_win_3d_kernel<NW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;   \
+    if ((e = cudaFuncSetAttribute(interp_win_3d_kernel<NW, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;   \
+    if ((e = cudaFuncSetAttribute(gridding_win_3d_kernel<NW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e; \
+    if ((e = cudaFuncSetAttribute(gridding_win_3d_kernel<NW, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, win3d_smem(NW))) != cudaSuccess) return e;
     NU_W3_CFG(kW3InterpWarps) NU_W3_CFG(kW3GridWarps)
 #undef NU_W3_CFG
     return cudaSuccess;
@@ -476,8 +481,12 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
         if (p->win3d && p->opts.interp_mode == 0) {
             CUtensorMap tm;
             const int use_tm = tile_tensor_map(p, batch, grid, &tm) ? 1 : 0;
-            interp_win_3d_kernel<kW3InterpWarps><<<tb, kW3InterpWarps * 32, win3d_smem(kW3InterpWarps), st>>>(
-                sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly, tm, use_tm);
+            if (p->d_w3rec)
+                interp_win_3d_kernel<kW3InterpWarps, true><<<tb, kW3InterpWarps * 32, win3d_smem(kW3InterpWarps), st>>>(
+                    sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly, tm, use_tm, p->d_w3rec);
+            else
+                interp_win_3d_kernel<kW3InterpWarps, false><<<tb, kW3InterpWarps * 32, win3d_smem(kW3InterpWarps), st>>>(
+                    sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly, tm, use_tm, nullptr);
         }
         else
             interp_tiled_3d_kernel<<<tb, 256, kInterp3dSmem, st>>>(sample_data(p), grid_geom(p), p->d_items, grid, y, p->poly);
@@ -531,8 +540,12 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
         const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
         CUtensorMap tm;
         const int use_tm = tile_tensor_map(p, batch, grid, &tm) ? 1 : 0;
-        gridding_win_3d_kernel<kW3GridWarps><<<blocks, kW3GridWarps * 32, win3d_smem(kW3GridWarps), st>>>(
-            sample_data(p), grid_geom(p), p->d_items, y, grid, p->poly, tm, use_tm);
+        if (p->d_w3rec)
+            gridding_win_3d_kernel<kW3GridWarps, true><<<blocks, kW3GridWarps * 32, win3d_smem(kW3GridWarps), st>>>(
+                sample_data(p), grid_geom(p), p->d_items, y, grid, p->poly, tm, use_tm, p->d_w3rec);
+        else
+            gridding_win_3d_kernel<kW3GridWarps, false><<<blocks, kW3GridWarps * 32, win3d_smem(kW3GridWarps), st>>>(
+                sample_data(p), grid_geom(p), p->d_items, y, grid, p->poly, tm, use_tm, nullptr);
     } else {
         const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
         const size_t sm = smem_grid3d(p);
@@ -961,7 +974,8 @@ static int plan_build(nufft_plan_t p, const double* om) {
     const int64_t M = p->M;
     std::vector<uint32_t> kpack(M);
     std::vector<float> delta((size_t)d * M);
-    std::vector<double> delta64(p->il_ok ? (size_t)d * M : 0);
+    const bool want64 = p->il_ok || p->opts.coef_mode == 1;
+    std::vector<double> delta64(want64 ? (size_t)d * M : 0);
     // 3-D, J = 6, default tile: inside a tile the samples are sorted by pencil (3 x 3 block of stencil base cells on axes
     // 0, 1) and base pair on axis 2, the order the register-window kernels of win3d.cuh walk
     p->win3d = (d == 3) && !p->generic_j && p->tile[0] == k3T0 && p->tile[1] == k3T1 && p->tile[2] == k3T2;
@@ -977,7 +991,7 @@ static int plan_build(nufft_plan_t p, const double* om) {
             float df;
             double d64;
             const int k0 = host::split_coordinate(w, p->K[a], J, &df, &d64);
-            if (p->il_ok) delta64[(size_t)a * M + m] = d64;
+            if (want64) delta64[(size_t)a * M + m] = d64;
             kp |= (uint32_t)k0 << (10 * a);
             delta[(size_t)a * M + m] = df;
             t = t * p->ntile[a] + k0 / p->tile[a];
@@ -1013,6 +1027,43 @@ static int plan_build(nufft_plan_t p, const double* om) {
     NU_TRY(dev_upload(&p->d_kpack, kpack_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_delta, delta_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_perm, perm, &p->bytes_plan));
+    // coef_mode = 1 (north star item 3 "precomputed in a coalesced per-sample layout"): the records the
+    // register-window 3-D kernels otherwise build on the fly (win3d.cuh w3_stage), evaluated here in float64 and rounded once,
+    // in walk order: 112 contiguous bytes per sample, moved into shared memory by one bulk copy per 16 samples
+    if (p->opts.coef_mode == 1 && p->win3d && M > 0) {
+        std::vector<float> recs((size_t)M * kW3Rec, 0.f);
+        double beta[3];
+        for (int a = 0; a < 3; ++a) beta[a] = host::kb_beta(J, (double)p->K[a] / (double)p->N[a]);
+        auto pad = [](const double (&w)[kJ], int o, float* out8) {
+            for (int i = 0; i < 8; ++i) out8[i] = (i - o >= 0 && i - o < kJ) ? (float)w[i - o] : 0.f;
+        };
+        for (int64_t i = 0; i < M; ++i) {
+            const int64_t m = perm[i];
+            float* r = &recs[(size_t)i * kW3Rec];
+            int c[3];
+            for (int a = 0; a < 3; ++a) c[a] = (int)((kpack[m] >> (10 * a)) & 1023u) % p->tile[a];
+            const int b0 = w3_block_base(c[0]), b1 = w3_block_base(c[1]), zb = c[2] >> 1;
+            double w[kJ];
+            float tmp[8];
+            for (int a = 0; a < 3; ++a) {
+                if (p->minmax) p->mm[a].weights(delta64[(size_t)a * M + m], w);
+                else host::kb_weights_f64(delta64[(size_t)a * M + m], J, beta[a], w);
+                if (a == 0) pad(w, c[0] - b0, r);
+                else if (a == 1) pad(w, c[1] - b1, r + 8);
+                else {
+                    pad(w, c[2] & 1, tmp);
+                    for (int pr = 0; pr < 4; ++pr) {          // rotated by the base pair: slot (zb + pr) & 3 holds pair pr
+                        r[16 + 2 * ((zb + pr) & 3)] = tmp[2 * pr];
+                        r[16 + 2 * ((zb + pr) & 3) + 1] = tmp[2 * pr + 1];
+                    }
+                }
+            }
+            const int32_t key = ((b0 * k3Plane + b1 * k3Pitch) << 4) | zb, mi = (int32_t)m;
+            std::memcpy(&r[24], &key, 4);
+            std::memcpy(&r[25], &mi, 4);
+        }
+        NU_TRY(dev_upload(&p->d_w3rec, recs, &p->bytes_plan));
+    }
     // V^H work items: (tile, sample range), hot tiles split into chunks of at most max_subtile samples
     {
         // default: enough work items to fill the machine at this plan's batch size (148 SMs x ~16 resident warps), but
@@ -1074,7 +1125,7 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
     }
     bool generic_sigma = false;
     for (int a = 0; a < d; ++a) generic_sigma = generic_sigma || Kd[a] != 2 * Nd[a];
-    if (opts && (opts->coef_mode != 0 || opts->adjoint_mode < 0 || opts->adjoint_mode > 2 || opts->interp_mode < 0 ||
+    if (opts && (opts->coef_mode < 0 || opts->coef_mode > 1 || opts->adjoint_mode < 0 || opts->adjoint_mode > 2 || opts->interp_mode < 0 ||
                  opts->interp_mode > 3 || opts->batch_layout < 0 || opts->batch_layout > 2 || opts->kernel < 0 ||
                  opts->kernel > 1))
         return NUFFT_EINVAL;
@@ -1138,7 +1189,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_kspace);
     cudaFree(p->d_ones); cudaFree(p->d_that); cudaFree(p->d_dcf_img); cudaFree(p->d_dcf_t);
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
-    cudaFree(p->d_il_kpack_c); cudaFree(p->d_il_delta_c); cudaFree(p->d_il_gbase); cudaFree(p->d_il_gbase_c);
+    cudaFree(p->d_il_kpack_c); cudaFree(p->d_il_delta_c); cudaFree(p->d_il_gbase); cudaFree(p->d_il_gbase_c); cudaFree(p->d_w3rec); cudaFree(p->d_il_wv); cudaFree(p->d_il_wv_c);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
     if (p->cg_graph) cudaGraphExecDestroy(p->cg_graph);
     for (auto& og : p->op_graphs) cudaGraphExecDestroy(og.exec);

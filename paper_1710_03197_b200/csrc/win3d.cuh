@@ -50,7 +50,7 @@ constexpr int kW3Rec = 28;                  // floats per staged sample record (
 // V 1 / 2 / 4 / 8 warps: 0.304 / 0.249 / 0.217 / 0.258 ms;  V^H (1 warp = no tile lock): 0.315 / 0.386 / 0.491 / 0.927 ms
 constexpr int kW3InterpWarps = 4, kW3GridWarps = 1;
 // NW warps per CTA: tile + NW x 32 records + mbarrier / lock
-constexpr int win3d_smem(int nw) { return k3Cells * 8 + nw * 32 * kW3Rec * 4 + 16; }
+constexpr int win3d_smem(int nw) { return k3Cells * 8 + nw * 32 * kW3Rec * 4 + 16 + nw * 16; }   // + 2 mbarriers per warp (TABLE)
 
 // tile-local stencil base (c0, c1, c2) -> window: pencil base on axes 0, 1 (blocks of 3 cells, the last block of the
 // 8-cell tile edge holds 2), base PAIR on axis 2
@@ -161,10 +161,15 @@ __device__ __forceinline__ W3Rec w3_load(const float* r, int ly, int q) {
 // ------------------------------------------------------------------------------------------------------------
 // V: y[m] = sum over the window of w0 w1 w2 G
 // ------------------------------------------------------------------------------------------------------------
-template <int NW>
+// TABLE (opts.coef_mode = 1): the sample records come precomputed from the plan (w3rec, 112 B per sample in walk order)
+// and are moved into shared memory by one bulk copy per 16 samples, double-buffered per warp, instead of being evaluated
+// from the kernel polynomial by one lane per sample.
+template <int NW, bool TABLE>
 __global__ void __launch_bounds__(NW * 32)
 interp_win_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ items, const float2* __restrict__ grid,
-                     float2* __restrict__ y, KernelPoly P, const __grid_constant__ CUtensorMap tmap, int use_tmap) {
+                     float2* __restrict__ y, KernelPoly P, const __grid_constant__ CUtensorMap tmap, int use_tmap,
+                     const float* __restrict__ w3rec) {
+    constexpr int CH = TABLE ? 16 : 32;
     extern __shared__ __align__(1024) unsigned char w3smem[];
     float2* tile = reinterpret_cast<float2*>(w3smem);
     float* recs = reinterpret_cast<float*>(tile + k3Cells);
@@ -209,11 +214,38 @@ interp_win_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ item
     int cur = -1;
     bool tile_ready = false;
     W3Pre pre;
-    w3_fetch(s, g, wb + lane, wb + lane < we, pre);
-    for (int c0 = wb; c0 < we; c0 += 32) {
-        const int cnt = min(32, we - c0);
-        w3_stage(pre, g, P, o, rec + lane * kW3Rec);
-        w3_fetch(s, g, c0 + 32 + lane, c0 + 32 + lane < we, pre);      // next chunk's plan data: in flight during this chunk
+    uint64_t* wbar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(bar) + 16) + 2 * warp;
+    float* const rec0 = rec;
+    if (TABLE) {
+        if (lane == 0) {
+            mbar_init(&wbar[0], 1);
+            mbar_init(&wbar[1], 1);
+            if (wb < we) {
+                const int n0 = min(CH, we - wb);
+                mbar_expect_tx(&wbar[0], (uint32_t)n0 * kW3Rec * 4);
+                bulk_g2s(rec0, w3rec + (int64_t)wb * kW3Rec, (uint32_t)n0 * kW3Rec * 4, &wbar[0]);
+            }
+        }
+        __syncwarp();
+    } else {
+        w3_fetch(s, g, wb + lane, wb + lane < we, pre);
+    }
+    int it = 0;
+    for (int c0 = wb; c0 < we; c0 += CH, ++it) {
+        const int cnt = min(CH, we - c0);
+        if (TABLE) {
+            rec = rec0 + (it & 1) * CH * kW3Rec;
+            if (lane == 0 && c0 + CH < we) {      // the other buffer was consumed one iteration ago (syncwarp at its end)
+                const int n1 = min(CH, we - c0 - CH);
+                mbar_expect_tx(&wbar[(it + 1) & 1], (uint32_t)n1 * kW3Rec * 4);
+                bulk_g2s(rec0 + ((it + 1) & 1) * CH * kW3Rec, w3rec + (int64_t)(c0 + CH) * kW3Rec, (uint32_t)n1 * kW3Rec * 4,
+                         &wbar[(it + 1) & 1]);
+            }
+            mbar_wait(&wbar[it & 1], (uint32_t)((it >> 1) & 1));
+        } else {
+            w3_stage(pre, g, P, o, rec + lane * kW3Rec);
+            w3_fetch(s, g, c0 + 32 + lane, c0 + 32 + lane < we, pre);      // next chunk's plan data: in flight during this chunk
+        }
         __syncwarp();
         if (!tile_ready) { mbar_wait(bar, 0); tile_ready = true; }
         W3Rec nx = w3_load(rec, ly, q);
@@ -223,9 +255,9 @@ interp_win_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ item
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const W3Rec c = nx;
-                nx = w3_load(rec + min(s8 + j + 1, 31) * kW3Rec, ly, q);
+                nx = w3_load(rec + min(s8 + j + 1, CH - 1) * kW3Rec, ly, q);
                 const int key = __float_as_int(c.kk.x);
-                if (__float_as_int(c.kk.y) >= 0 && key != cur) {       // (padded records of a short chunk keep the window)
+                if (s8 + j < cnt && key != cur) {       // (slots past the end of a short chunk keep the window)
                     // slide (same pencil, base pair advanced by 1..3) or reload: lane (y, q) owns pair zb + ((q - zb) & 3)
                     const int zb = key & 15;
                     const bool same = cur >= 0 && (key >> 4) == (cur >> 4);
@@ -313,10 +345,12 @@ __device__ __forceinline__ void w3_unlock(int* l, int lane) {
     }
 }
 
-template <int NW>
+template <int NW, bool TABLE>
 __global__ void __launch_bounds__(NW * 32)
 gridding_win_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ items, const float2* __restrict__ y,
-                       float2* __restrict__ grid, KernelPoly P, const __grid_constant__ CUtensorMap tmap, int use_tmap) {
+                       float2* __restrict__ grid, KernelPoly P, const __grid_constant__ CUtensorMap tmap, int use_tmap,
+                       const float* __restrict__ w3rec) {
+    constexpr int CH = TABLE ? 16 : 32;
     extern __shared__ __align__(1024) unsigned char w3smem[];
     float2* tile = reinterpret_cast<float2*>(w3smem);
     float* recs = reinterpret_cast<float*>(tile + k3Cells);
@@ -361,21 +395,58 @@ gridding_win_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ it
     };
     // two-deep prefetch: plan data of chunk c + 2 and the y values of chunk c + 1 are in flight while chunk c is applied
     W3Pre pre, nxt;
-    w3_fetch(s, g, wb + lane, wb + lane < we, pre);
-    if (pre.m >= 0) pre.yv = __ldg(&yb[pre.m]);
-    w3_fetch(s, g, wb + 32 + lane, wb + 32 + lane < we, nxt);
-    for (int c0 = wb; c0 < we; c0 += 32) {
-        const int cnt = min(32, we - c0);
-        w3_stage(pre, g, P, o, rec + lane * kW3Rec);
-        pre = nxt;
+    uint64_t* wbar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(lock) + 16) + 2 * warp;
+    float* const rec0 = rec;
+    // TABLE: only the caller's index and y are fetched through registers (two / one chunk ahead); the weights arrive by bulk copy
+    auto fetch_m = [&](int si, bool valid, W3Pre& f) { f.m = valid ? __ldg(&s.perm[si]) : -1; f.yv = make_float2(0.f, 0.f); };
+    if (TABLE) {
+        if (lane == 0) {
+            mbar_init(&wbar[0], 1);
+            mbar_init(&wbar[1], 1);
+            if (wb < we) {
+                const int n0 = min(CH, we - wb);
+                mbar_expect_tx(&wbar[0], (uint32_t)n0 * kW3Rec * 4);
+                bulk_g2s(rec0, w3rec + (int64_t)wb * kW3Rec, (uint32_t)n0 * kW3Rec * 4, &wbar[0]);
+            }
+        }
+        __syncwarp();
+        fetch_m(wb + lane, lane < CH && wb + lane < we, pre);
         if (pre.m >= 0) pre.yv = __ldg(&yb[pre.m]);
-        w3_fetch(s, g, c0 + 64 + lane, c0 + 64 + lane < we, nxt);
+        fetch_m(wb + CH + lane, lane < CH && wb + CH + lane < we, nxt);
+    } else {
+        w3_fetch(s, g, wb + lane, wb + lane < we, pre);
+        if (pre.m >= 0) pre.yv = __ldg(&yb[pre.m]);
+        w3_fetch(s, g, wb + 32 + lane, wb + 32 + lane < we, nxt);
+    }
+    int it = 0;
+    for (int c0 = wb; c0 < we; c0 += CH, ++it) {
+        const int cnt = min(CH, we - c0);
+        if (TABLE) {
+            rec = rec0 + (it & 1) * CH * kW3Rec;
+            if (lane == 0 && c0 + CH < we) {
+                const int n1 = min(CH, we - c0 - CH);
+                fence_proxy_async_smem();         // this warp's y stores into that buffer precede the engine's writes
+                mbar_expect_tx(&wbar[(it + 1) & 1], (uint32_t)n1 * kW3Rec * 4);
+                bulk_g2s(rec0 + ((it + 1) & 1) * CH * kW3Rec, w3rec + (int64_t)(c0 + CH) * kW3Rec, (uint32_t)n1 * kW3Rec * 4,
+                         &wbar[(it + 1) & 1]);
+            }
+            mbar_wait(&wbar[it & 1], (uint32_t)((it >> 1) & 1));
+            if (lane < cnt) *reinterpret_cast<float2*>(rec + lane * kW3Rec + 26) = pre.yv;
+            pre = nxt;
+            if (pre.m >= 0) pre.yv = __ldg(&yb[pre.m]);
+            fetch_m(c0 + 2 * CH + lane, lane < CH && c0 + 2 * CH + lane < we, nxt);
+        } else {
+            w3_stage(pre, g, P, o, rec + lane * kW3Rec);
+            pre = nxt;
+            if (pre.m >= 0) pre.yv = __ldg(&yb[pre.m]);
+            w3_fetch(s, g, c0 + 64 + lane, c0 + 64 + lane < we, nxt);
+        }
         __syncwarp();
         W3Rec nx = w3_load(rec, ly, q);
 #pragma unroll 4
         for (int si = 0; si < cnt; ++si) {
             const W3Rec c = nx;
-            nx = w3_load(rec + min(si + 1, 31) * kW3Rec, ly, q);
+            nx = w3_load(rec + min(si + 1, CH - 1) * kW3Rec, ly, q);
             const int key = __float_as_int(c.kk.x);
             if (key != cur) {
                 if (cur >= 0) retire(((key >> 4) == (cur >> 4)) ? (key & 15) - (cur & 15) : 4);
