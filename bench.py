@@ -566,6 +566,55 @@ def cfg4_record(nb, torch, peak, peak_src, cpu_seconds):
     }
 
 
+def coef_mode_table(nb, torch):
+    """North star item 3 / SURVEY 8(b) coef_mode: V (and the 3-D V^H) with weights recomputed on the fly from the kernel
+    polynomial (mode 0: 4 + 4 d bytes of plan data per sample) against weights precomputed by the plan in a coalesced
+    per-sample layout (mode 1: 64 B per sample on the interleaved 2-D path, 112 B in 3-D), on config 2 batch 64 and config 4.
+    Device ms per launch (library-side events, L2 flushed between steps) and plan bytes; parity of mode 1 vs the oracle."""
+    from oracle import nufft_oracle as orc
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    out = {}
+    for name, cfg, B in (("cfg2_batch64", wl.config(1), 64), ("cfg4_batch1", wl.config(3), 1)):
+        Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+        x = torch.from_numpy(wl.image_gaussian(Nd, batch=B)).cuda()
+        rows = {}
+        for mode in (0, 1):
+            p = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=B, coef_mode=mode)
+            y = p.forward(x)
+            xo = p.adjoint(y)
+            for _ in range(3):
+                p.forward(x, y), p.adjoint(y, xo), p.selfadjoint(x, xo)
+            p.profile_enable(True)
+            p.profile_reset()
+            for _ in range(10):
+                flush.zero_()
+                p.forward(x, y)
+                p.adjoint(y, xo)
+            torch.cuda.synchronize()
+            pr = p.profile()
+            fa = {k: v[0] / v[1] for k, v in pr.items() if v[1] and k in ("interp", "gridding")}
+            p.profile_reset()
+            for _ in range(10):
+                flush.zero_()
+                p.selfadjoint(x, xo)
+            torch.cuda.synchronize()
+            sa = {k: v[0] / v[1] for k, v in p.profile().items() if v[1] and k in ("interp", "gridding")}
+            rows["coef_mode_%d" % mode] = {"interp_ms": fa.get("interp"), "gridding_ms": fa.get("gridding"),
+                                           "interp_ms_in_selfadjoint": sa.get("interp"), "plan_bytes": p.info()["bytes_plan"]}
+            p.destroy()
+        out[name] = rows
+    cfg = wl.config(3, scale=4)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    xs, ys = wl.image_gaussian(Nd), wl.data_gaussian(om.shape[0])
+    p = nb.NufftPlan(Nd, Kd, Jd, om, coef_mode=1)
+    rel = lambda a, b: float(np.linalg.norm(a.ravel() - b.ravel()) / np.linalg.norm(b.ravel()))
+    out["parity_coef_mode_1_cfg4_scaled"] = {
+        "forward": rel(p.forward(torch.from_numpy(xs).cuda()).cpu().numpy()[0], orc.forward(xs.astype(np.complex128), om, Nd, Kd, Jd)),
+        "adjoint": rel(p.adjoint(torch.from_numpy(ys).cuda()).cpu().numpy()[0], orc.adjoint(ys.astype(np.complex128), om, Nd, Kd, Jd))}
+    p.destroy()
+    return out
+
+
 def parity_block(nb, torch):
     """Relative L2 and max-abs (of the largest reference value) of forward / adjoint / A^H A against the float64 oracle,
     on config 1 and the scaled config 4, computed in this very run (SURVEY section 5 "Metrics")."""
@@ -804,12 +853,18 @@ def main():
     ap.add_argument("--batch", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-extra", action="store_true")
-    ap.add_argument("--only", default="", choices=["", "cfg4"],
+    ap.add_argument("--only", default="", choices=["", "cfg4", "coef"],
                     help="cfg4: measure only the 3-D config 4 record and print it as the JSON line (used by the ncu "
                          "commands in profiles/)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.only == "coef":
+        import torch
+        import paper_1710_03197_b200 as nb
+        torch.cuda.set_device(0)
+        print(json.dumps({"coef_mode_table": coef_mode_table(nb, torch)}))
+        return 0
     if args.only == "cfg4":
         import torch
         import paper_1710_03197_b200 as nb

@@ -28,6 +28,8 @@
  *   - every call returns 0 (NUFFT_OK) or a negative nufft_status; nothing is printed, nothing throws or aborts.
  *   - transform calls are asynchronous: they enqueue kernels on `stream` and return.  A plan owns one workspace:
  *     use one stream at a time per plan.  Distinct plans are independent.
+ *   - a plan belongs to the CUDA device that was current when nufft_plan created it (its buffers and kernel attributes live
+ *     there): every later call must be made with that device current, else NUFFT_EINVAL.
  *   - outputs are overwritten, never accumulated into.  In-place (x_in == x_out) is allowed for selfadjoint.
  *   - supported: d in {1,2,3} (1-D: "1D signals"; planar path, atomic V^H only -- adjoint_mode = 1 is
  *     refused); Jd[a] the same on every axis, 2 <= Jd <= 8 (odd widths included);
@@ -63,23 +65,31 @@ typedef enum {
 
 /* Options.  Zero-initialise or call nufft_default_opts first. */
 typedef struct {
-    int coef_mode;      /* must be 0: the library chooses per kernel from measured cost: planar V / V^H
-                               and interleaved V recompute the weights on the fly from a piecewise polynomial fit of
-                               the Kaiser-Bessel kernel (4 + 4 d bytes of plan data per sample); interleaved V^H reads a
-                               float64-built separable table (96 B per sample).  Any other value -> NUFFT_EINVAL      */
-    int adjoint_mode;   /* planar path: 0 = V^H by tile-sorted shared-memory accumulation, one vector-atomic flush per
-                               tile (summation order across tiles free: reproducible to rounding only);
+    int coef_mode;      /* how V (and the 3-D V^H) get their interpolation weights (north star item 3):
+                           0 = recomputed on the fly from a piecewise polynomial fit of the kernel: 4 + 4 d bytes of plan
+                               data per sample (the default: fewest bytes; measured 2-7 % slower than 1, profiles/r02_coef_mode.md);
+                           1 = precomputed by the plan in float64, rounded once, stored zero-padded in a coalesced per-sample
+                               layout in walk order -- 64 B per sample for the interleaved 2-D V, 112 B for the register-window
+                               3-D V / V^H (moved to shared memory by one bulk copy per 16 samples).  Other kernels (planar
+                               2-D, generic widths) recompute in either mode; the interleaved V^H always reads its
+                               float64-built 96-B table.  Any other value -> NUFFT_EINVAL                                   */
+    int adjoint_mode;   /* planar path: 0 = V^H by tile-sorted accumulation on chip, one TMA reduce-add flush per work item
+                               (3-D: register windows over pencil-sorted samples, win3d.cuh; 2-D: warp-private shared tiles);
+                               summation order across work items free: reproducible to rounding only;
                            1 = deterministic: tiles flushed to private slabs and summed in fixed order
-                               (bit-reproducible run to run).  The interleaved path (batch >= 12) is always
-                               deterministic (gather form, fixed order)                                             */
-    int interp_mode;    /* 0 = library default: 3-D planar V stages the padded tile of a work item in shared memory
-                               (half-warp per sample), 2-D planar V gathers through L1/L2, interleaved V walks the
-                               CALLER's sample order and writes y directly when the trajectory is coherent (>= 90 % of
-                               consecutive samples within two grid cells: radial spokes, spiral arms);
-                           1 = the plain variants: direct gather in 3-D, sorted walk + layout pass on the interleaved
-                               path (kept for cross-checks);
+                               (bit-reproducible run to run);
+                           2 = 3-D only: the plane-owner shared-memory kernel of round 1 (kept for A/B measurements).
+                           The interleaved path (batch >= 12) is always deterministic (gather form, fixed order)        */
+    int interp_mode;    /* 0 = library default: register-window kernels -- 3-D planar V keeps an 8 x 8 x 8 window of the
+                               staged tile in registers and slides it along the pencil-sorted samples; interleaved V keeps
+                               the 8 x 8 window of a group of neighbouring samples in registers and walks the CALLER's
+                               sample order, writing y directly, when the trajectory is coherent (>= 90 % of consecutive
+                               samples within two grid cells: radial spokes, spiral arms); 2-D planar V gathers through L1/L2;
+                           1 = the plain variants: direct gather in 3-D, sorted walk + layout pass on the interleaved path;
                            2 = the generic-width kernels (direct V, atomic V^H, planar) even at Jd = 6: what a plan
-                               with Jd != 6 runs, selectable at Jd = 6 for cross-checks against the tuned kernels   */
+                               with Jd != 6 runs, selectable at Jd = 6 for cross-checks against the tuned kernels;
+                           3 = the round-1 kernels (half-warp-per-sample 3-D V, stencil-per-sample interleaved V), kept
+                               for A/B measurements                                                                    */
     int tile[3];        /* tile shape in grid cells per axis, 0 = library default                                */
     int max_subtile;    /* max samples per V^H work item (hot tiles are split), 0 = default                      */
     int use_graphs;     /* 1 = CUDA-graph replay of launch-bound work on a non-default stream (the legacy stream cannot

@@ -164,6 +164,8 @@ struct IlPlan {
     const float* delta_c;     // caller order [2][M]
     const uint32_t* gbase;    // V order: base cell (row | col << 10) of the sample's window group (interp_il_win_kernel)
     const uint32_t* gbase_c;  // caller order (trajectory-coherent plans only, else null)
+    const float* wv;          // coef_mode = 1: zero-padded weights [M][16] (w0 padded[8], w1 padded[8]) in V order, else null
+    const float* wv_c;        // ... in the caller's order
     const int32_t* v2h;       // V-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
     const float* wtab;        // V^H order: [M][kTabW] = w0[6], k0_0 (int bits), pad, w1 part A[8], w1 part B[8] (float64-built)
@@ -310,12 +312,19 @@ interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, f
         float4 r0, r1, r2, r3, r4;
         if (lane < cnt) {
             const int64_t si = w0s + lane;
-            const uint32_t kp = __ldg(&kpk[si]), gb = __ldg(&gbs[si]);
-            float w[kJ];
-            kb_weights(P, 0, __ldg(&dlt[si]), w);
-            il_pad8(w, (int)(kp & 1023u) - (int)(gb & 1023u), r0, r1);
-            kb_weights(P, 1, __ldg(&dlt[g.M + si]), w);
-            il_pad8(w, (int)((kp >> 10) & 1023u) - (int)((gb >> 10) & 1023u), r2, r3);
+            const uint32_t gb = __ldg(&gbs[si]);
+            const float* __restrict__ wt = CALLER ? s.wv_c : s.wv;
+            if (wt) {       // coef_mode = 1: precomputed (float64-built) padded weights, 64 contiguous bytes per sample
+                const float4* __restrict__ t4 = reinterpret_cast<const float4*>(wt + si * 16);
+                r0 = __ldg(t4); r1 = __ldg(t4 + 1); r2 = __ldg(t4 + 2); r3 = __ldg(t4 + 3);
+            } else {
+                const uint32_t kp = __ldg(&kpk[si]);
+                float w[kJ];
+                kb_weights(P, 0, __ldg(&dlt[si]), w);
+                il_pad8(w, (int)(kp & 1023u) - (int)(gb & 1023u), r0, r1);
+                kb_weights(P, 1, __ldg(&dlt[g.M + si]), w);
+                il_pad8(w, (int)((kp >> 10) & 1023u) - (int)((gb >> 10) & 1023u), r2, r3);
+            }
             r4 = make_float4(__int_as_float((int)gb), __int_as_float(CALLER ? 0 : __ldg(&s.v2h[si])), 0.f, 0.f);
         } else {
             r0 = r1 = r2 = r3 = make_float4(0.f, 0.f, 0.f, 0.f);

@@ -634,6 +634,7 @@ static IlPlan il_plan(nufft_plan_t p) {
     s.rowptr = p->d_il_rowptr; s.v2h = p->d_il_v2h;
     s.kpack_c = p->d_il_kpack_c; s.delta_c = p->d_il_delta_c;
     s.gbase = p->d_il_gbase; s.gbase_c = p->d_il_gbase_c;
+    s.wv = p->d_il_wv; s.wv_c = p->d_il_wv_c;
     return s;
 }
 
@@ -836,6 +837,18 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
         dl_s[M + i] = delta[M + m];
         v2h[i] = pos_h[m];
     }
+    // coef_mode = 1: the zero-padded weight vectors of interp_il_win_kernel, float64-built, per walk order
+    auto weight_table = [&](auto sample_at, const std::vector<uint32_t>& gb, std::vector<float>& tab) {
+        tab.assign((size_t)M * 16, 0.f);
+        for (int64_t i = 0; i < M; ++i) {
+            const int64_t m = sample_at(i);
+            double w0[kJ], w1[kJ];
+            if (p->minmax) { p->mm[0].weights(delta64[m], w0); p->mm[1].weights(delta64[M + m], w1); }
+            else { host::kb_weights_f64(delta64[m], J, beta, w0); host::kb_weights_f64(delta64[M + m], J, beta, w1); }
+            const int o0 = row_of(kpack[m]) - (int)(gb[i] & 1023u), o1 = col_of(kpack[m]) - (int)((gb[i] >> 10) & 1023u);
+            for (int j = 0; j < kJ; ++j) { tab[(size_t)i * 16 + o0 + j] = (float)w0[j]; tab[(size_t)i * 16 + 8 + o1 + j] = (float)w1[j]; }
+        }
+    };
     std::vector<float> wtab((size_t)M * kTabW, 0.f);
     for (int64_t i = 0; i < M; ++i) {
         const int64_t m = perm_h[i];
@@ -903,12 +916,22 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
             NU_TRY(dev_upload(&p->d_il_kpack_c, kpack, &p->bytes_plan));
             NU_TRY(dev_upload(&p->d_il_delta_c, delta, &p->bytes_plan));
             NU_TRY(dev_upload(&p->d_il_gbase_c, gb_c, &p->bytes_plan));
+            if (p->opts.coef_mode == 1) {
+                std::vector<float> tab;
+                weight_table([&](int64_t i) { return i; }, gb_c, tab);
+                NU_TRY(dev_upload(&p->d_il_wv_c, tab, &p->bytes_plan));
+            }
         }
     }
     {
         std::vector<uint32_t> gb_v;
         window_groups([&](int64_t i) { return kp_s[i]; }, gb_v);
         NU_TRY(dev_upload(&p->d_il_gbase, gb_v, &p->bytes_plan));
+        if (p->opts.coef_mode == 1) {
+            std::vector<float> tab;
+            weight_table([&](int64_t i) { return (int64_t)perm_v[i]; }, gb_v, tab);
+            NU_TRY(dev_upload(&p->d_il_wv, tab, &p->bytes_plan));
+        }
     }
     NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
     NU_TRY(dev_upload(&p->d_il_delta, dl_s, &p->bytes_plan));

@@ -658,6 +658,45 @@ def test_l1tv_ols_config5_full_size_32_coils_r17_iteration_counts():
     p.destroy()
 
 
+@pytest.mark.parametrize("ci,scale,B", [(1, 2, 40), (0, 1, 33), (3, 4, 1), (3, 8, 2)])
+def test_coef_mode_1_precomputed_weight_tables(ci, scale, B):
+    """opts.coef_mode = 1: plan-precomputed, zero-padded per-sample weights for the interleaved 2-D V (caller
+    and sorted walks) and the register-window 3-D V / V^H, against the oracle; plan facts report the larger table."""
+    cfg = wl.config(ci, scale=scale)
+    Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+    x = wl.image_gaussian(Nd, batch=B)
+    y = wl.data_gaussian(om.shape[0], batch=B)
+    p0 = make_plan(cfg, max_batch=B)
+    p1 = make_plan(cfg, max_batch=B, coef_mode=1)
+    assert p1.info()["bytes_plan"] > p0.info()["bytes_plan"]
+    yg, xg, sg = host(p1.forward(dev(x))), host(p1.adjoint(dev(y))), host(p1.selfadjoint(dev(x)))
+    for b in sorted({0, B - 1}):
+        yo = orc.forward(x[b].astype(np.complex128), om, Nd, Kd, Jd)
+        close(yg[b], yo, Jd)
+        close(xg[b], orc.adjoint(y[b].astype(np.complex128), om, Nd, Kd, Jd), Jd)
+        close(sg[b], orc.adjoint(yo, om, Nd, Kd, Jd), Jd)
+    p0.destroy()
+    p1.destroy()
+
+
+def test_plan_tile_histogram_and_wrong_option_values():
+    import paper_1710_03197_b200 as nb
+    cfg = wl.config(3, scale=4)
+    p = make_plan(cfg)
+    info = p.info()
+    h = info["tile_histogram"]
+    assert len(h) == 24 and sum(h) == info["n_tiles"]
+    # the bucket of the largest tile is the last non-empty one
+    top = max(k for k, v in enumerate(h) if v)
+    assert 2 ** (top - 1) <= info["max_tile_samples"] < 2 ** top
+    p.destroy()
+    for kw in (dict(coef_mode=2), dict(adjoint_mode=3), dict(interp_mode=4)):
+        with pytest.raises(nb.NufftError):
+            make_plan(cfg, **kw)
+    with pytest.raises(nb.NufftError):
+        make_plan(wl.config(0), tile=(64, 64))          # shared-memory footprint of the V^H tiles exceeds the opt-in
+
+
 def test_cg_config3_parity_against_the_problems_own_amplification():
     """the VD spiral leaves the k-space corners unsampled, A^H A has a near-null space and CG amplifies any
     perturbation of the operator.  The GPU operator agrees with the oracle to ~3e-7 per application, so its CG iterates can
