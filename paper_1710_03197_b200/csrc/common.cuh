@@ -105,6 +105,15 @@ __device__ __forceinline__ void bulk_commit_and_wait_read() {
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// Programmatic dependent launch (PDL): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
+// while its predecessor in the stream is still running; pdl_enter() is its first statement: it lets the NEXT kernel in the
+// stream be scheduled early (launch_dependents) and then waits until the predecessor grid has completed and its writes are
+// visible (wait).  Without the launch attribute both are no-ops.  The small dependent kernels of a single transform then
+// overlap their launch latency and CTA scheduling with the tail of the previous kernel.
+__device__ __forceinline__ void pdl_enter() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     uint32_t ok;
     do {

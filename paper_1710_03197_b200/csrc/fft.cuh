@@ -253,6 +253,7 @@ struct RowPassParams {
 template <int K>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::LC)
 fft_rows_fwd_kernel(RowPassParams p) {
+    pdl_enter();
     using G = FftGeom<K>;
     constexpr int N = K / 2, TPL = G::TPL, LC = Rad<K>::LC;
     extern __shared__ float2 smem[];
@@ -284,6 +285,7 @@ fft_rows_fwd_kernel(RowPassParams p) {
 template <int K>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::LC)
 fft_rows_adj_kernel(RowPassParams p) {
+    pdl_enter();
     using G = FftGeom<K>;
     constexpr int N = K / 2, TPL = G::TPL, LC = Rad<K>::LC;
     extern __shared__ float2 smem[];
@@ -329,6 +331,7 @@ struct ColPassParams {
 template <int K, bool ADJ, bool FULL = false, bool MULT = false>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS, Rad<K>::MBS)
 fft_cols_kernel(ColPassParams p) {
+    pdl_enter();
     using G = FftGeom<K>;
     constexpr int T = Rad<K>::TS;
     extern __shared__ float2 smem[];

@@ -212,6 +212,7 @@ static cudaError_t configure_all() {
     if ((e = configure_fft<1024>()) != cudaSuccess) return e;
     const int big = 200 * 1024;
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(interp_tiled_2d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(interp_tiled_3d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kInterp3dSmem)) != cudaSuccess) return e;
@@ -231,17 +232,29 @@ static cudaError_t configure_all() {
 // ------------------------------------------------------------------------------------------------------------
 // FFT pass launchers
 // ------------------------------------------------------------------------------------------------------------
+// launch with programmatic stream serialization (see pdl_enter in common.cuh)
+template <class... KArgs, class... Args>
+static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    (void)cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <int K> static void launch_rows(bool adj, const RowPassParams& p, cudaStream_t st) {
     constexpr int threads = FftGeom<K>::TPL * Rad<K>::LC;
     const int blocks = (p.nlines + Rad<K>::LC - 1) / Rad<K>::LC;
-    if (adj) fft_rows_adj_kernel<K><<<blocks, threads, smem_rows<K>(), st>>>(p);
-    else     fft_rows_fwd_kernel<K><<<blocks, threads, smem_rows<K>(), st>>>(p);
+    if (adj) launch_pdl(fft_rows_adj_kernel<K>, dim3(blocks), dim3(threads), smem_rows<K>(), st, p);
+    else     launch_pdl(fft_rows_fwd_kernel<K>, dim3(blocks), dim3(threads), smem_rows<K>(), st, p);
 }
 template <int K> static void launch_cols(bool adj, const ColPassParams& p, cudaStream_t st) {
     constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
-    if (adj && p.mult) fft_cols_kernel<K, true, false, true><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
-    else if (adj) fft_cols_kernel<K, true><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
-    else     fft_cols_kernel<K, false><<<p.ngroups, threads, smem_cols<K>(), st>>>(p);
+    if (adj && p.mult) launch_pdl(fft_cols_kernel<K, true, false, true>, dim3(p.ngroups), dim3(threads), smem_cols<K>(), st, p);
+    else if (adj) launch_pdl(fft_cols_kernel<K, true>, dim3(p.ngroups), dim3(threads), smem_cols<K>(), st, p);
+    else     launch_pdl(fft_cols_kernel<K, false>, dim3(p.ngroups), dim3(threads), smem_cols<K>(), st, p);
 }
 static int tile_T(int K) {
     switch (K) {
@@ -494,6 +507,15 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
         p->launches++;
         return NUFFT_OK;
     }
+    if (p->d == 2 && p->opts.interp_mode == 0 && p->n_items > 0 && p->K[1] >= p->tg.pitch) {
+        // tile-staged V: one CTA per V^H work item (the same tile-sorted sample ranges)
+        const dim3 tb((unsigned)p->n_items, (unsigned)batch);
+        launch_pdl(interp_tiled_2d_kernel, tb, dim3(128), (size_t)p->tg.tile_cells * 8 + 16, st, sample_data(p), grid_geom(p), p->tg,
+                   (const WorkItem*)p->d_items, grid, y, p->poly);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+        return NUFFT_OK;
+    }
     const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
     if (p->d == 1) interp_direct_kernel<1><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
     else if (p->d == 2) interp_direct_kernel<2><<<blocks, 128, 0, st>>>(sample_data(p), grid_geom(p), grid, y, p->poly);
@@ -526,7 +548,13 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
     const int64_t slab_stride = (int64_t)p->n_items * p->tg.tile_cells;
     if (det && !p->d_slabs)
         NU_TRY(dev_alloc((void**)&p->d_slabs, (size_t)p->max_batch * slab_stride * sizeof(float2), &p->bytes_work));
-    if (!det) { ProfScope ps(p, "grid_zero", st); CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st)); }
+    if (!det) {
+        ProfScope ps(p, "grid_zero", st);
+        const int64_t n4 = (int64_t)batch * p->cells / 2;      // cells is even: float4 = two cells
+        launch_pdl(grid_zero_kernel, dim3((unsigned)std::min<int64_t>((n4 + 255) / 256, 148 * 16)), dim3(256), 0, st, (float4*)grid, n4);
+        CU_TRY(cudaGetLastError());
+        p->launches++;
+    }
     ProfScope ps(p, "gridding", st);
     if (p->d == 1) {       // 1-D: one thread per sample, one vector atomic per stencil point (the grid was zeroed above)
         const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)batch);
@@ -535,7 +563,8 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
         const dim3 blocks((unsigned)((p->n_items + kGrid2dWarps - 1) / kGrid2dWarps), (unsigned)batch);
         const size_t sm = smem_grid2d(p);
         if (det) gridding_tiled_2d_kernel<true><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly);
-        else     gridding_tiled_2d_kernel<false><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, nullptr, 0, p->poly);
+        else     launch_pdl(gridding_tiled_2d_kernel<false>, blocks, dim3(kGrid2dWarps * 32), sm, st, sample_data(p), grid_geom(p), p->tg,
+                            (const WorkItem*)p->d_items, p->n_items, y, grid, (float2*)nullptr, (int64_t)0, p->poly);
     } else if (!det && p->win3d && p->opts.adjoint_mode == 0) {
         const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
         CUtensorMap tm;

@@ -241,12 +241,20 @@ __device__ __forceinline__ void flush_tile(const float2* tile, const TileGeom& t
     }
 }
 
+// grid = 0 as a kernel (not a memset node), so that it takes part in the programmatic-dependent-launch chain of a transform
+__global__ void __launch_bounds__(256) grid_zero_kernel(float4* __restrict__ g4, int64_t n4) {
+    pdl_enter();
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (int64_t)gridDim.x * blockDim.x)
+        g4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
 // 2-D: NW independent warps per CTA, each with a private tile + staging area.
 template <bool DET>
 __global__ void __launch_bounds__(256)
 gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items, int n_items,
                          const float2* __restrict__ y, float2* __restrict__ grid, float2* __restrict__ slabs,
                          int64_t slab_batch_stride, KernelPoly P) {
+    pdl_enter();
     extern __shared__ float4 smem4[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int item = blockIdx.x * nw + warp;
@@ -452,6 +460,72 @@ gridding_merge_kernel(GridGeom g, TileGeom tg, int nt0, int nt1, int nt2, const 
             }
     grid[(int64_t)b * g.cells + cell] = acc;
 }
+// ------------------------------------------------------------------------------------------------------------
+// V, 2-D planar, tile-staged (round 2; small batches): one CTA per work item (tile, sample range), one thread per sample.
+// profiles/r01b: with the direct form every warp load touches ~16 sectors and the L1 data pipe saturates; here the padded
+// tile of the item (default 21 x 40 cells = 6.7 KB) is staged in shared memory with one bulk copy per row and the 36
+// stencil values of a sample are 36 shared-memory loads.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+interp_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items,
+                       const float2* __restrict__ grid, float2* __restrict__ y, KernelPoly P) {
+    pdl_enter();
+    extern __shared__ float4 smem4[];
+    float2* tile = reinterpret_cast<float2*>(smem4);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(tile + tg.tile_cells);
+    const WorkItem wi = items[blockIdx.x];
+    const int b = blockIdx.y;
+    int o[3];
+    unpack_k0(wi.origin, o);
+    const int K0 = g.K[0], K1 = g.K[1];
+    const float2* __restrict__ G = grid + (int64_t)b * g.cells;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_expect_tx(bar, (uint32_t)(tg.P[0] * tg.pitch * 8));
+    }
+    __syncthreads();
+    for (int row = threadIdx.x; row < tg.P[0]; row += blockDim.x) {
+        const int gx = (o[0] + row) & (K0 - 1), gz = o[1] & (K1 - 1);
+        const float2* src = G + (int64_t)gx * K1;
+        float2* dst = tile + row * tg.pitch;
+        const int first = min(tg.pitch, K1 - gz);
+        bulk_g2s(dst, src + gz, (uint32_t)first * 8, bar);
+        if (first < tg.pitch) bulk_g2s(dst + first, src, (uint32_t)(tg.pitch - first) * 8, bar);
+    }
+    // the sample's plan data and weights are fetched / evaluated while the copies are in flight
+    float2* __restrict__ yb = y + (int64_t)b * g.M;
+    for (int base = wi.s_begin; base < wi.s_end; base += blockDim.x) {
+        const int si = base + threadIdx.x;
+        const bool valid = si < wi.s_end;
+        int k0[3] = {0, 0, 0};
+        float w0[kJ], w1[kJ];
+        int m = 0;
+        if (valid) {
+            unpack_k0(__ldg(&s.kpack[si]), k0);
+            kb_weights(P, 0, __ldg(&s.delta[si]), w0);
+            kb_weights(P, 1, __ldg(&s.delta[g.M + si]), w1);
+            m = __ldg(&s.perm[si]);
+        }
+        if (base == wi.s_begin) mbar_wait(bar, 0);
+        if (!valid) continue;
+        const float2* __restrict__ tp = tile + ((k0[0] - o[0]) & (K0 - 1)) * tg.pitch + ((k0[1] - o[1]) & (K1 - 1));
+        float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j0 = 0; j0 < kJ; ++j0) {
+            float2 r = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int j1 = 0; j1 < kJ; ++j1) {
+                const float2 v = tp[j0 * tg.pitch + j1];
+                r.x = fmaf(w1[j1], v.x, r.x);
+                r.y = fmaf(w1[j1], v.y, r.y);
+            }
+            acc.x = fmaf(w0[j0], r.x, acc.x);
+            acc.y = fmaf(w0[j0], r.y, acc.y);
+        }
+        yb[m] = acc;
+    }
+}
+
 }  // namespace nufft
 
 namespace nufft {
