@@ -359,7 +359,7 @@ def run_ours(args):
 
     # the batch-32 point (one interleaved group) of the same workload
     batch32 = None
-    if world == 1 and B != 32:
+    if world == 1 and B != 32 and not args.no_extra:
         p32 = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=32)
         x32, y32, xo32 = x[:32].contiguous(), y[:32].contiguous(), xo[:32].contiguous()
 
@@ -434,7 +434,7 @@ def run_ours(args):
             "paper_context": "PAPER.md Table 1 (:299-300): forward 6 ms + adjoint 6 ms on one K80 GK210 (PyCUDA), "
                              "workload sizes not stated by the paper",
         }
-        if world == 1:
+        if world == 1 and not args.no_extra:
             # the 3-D half of the metric (BASELINE: "(2D 256^2, 3D 128^3)"), a record of its own next to the headline
             try:
                 result["cfg4_3d"] = cfg4_record(nb, torch, peak, peak_src, args.cpu_seconds)
@@ -852,7 +852,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
-    ap.add_argument("--no-extra", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="headline workload only: skip the cfg4_3d record, the parity block, the batch-32 point and the extra "
+                         "legs (used by the ncu commands in profiles/)")
     ap.add_argument("--only", default="", choices=["", "cfg4", "coef"],
                     help="cfg4: measure only the 3-D config 4 record and print it as the JSON line (used by the ncu "
                          "commands in profiles/)")
