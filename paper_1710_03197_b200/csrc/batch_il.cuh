@@ -164,7 +164,7 @@ struct IlPlan {
     const float* delta_c;     // caller order [2][M]
     const uint32_t* gbase;    // V order: base cell (row | col << 10) of the sample's window group (interp_il_win_kernel)
     const uint32_t* gbase_c;  // caller order (trajectory-coherent plans only, else null)
-    const float* wv;          // coef_mode = 1: zero-padded weights [M][16] (w0 padded[8], w1 padded[8]) in V order, else null
+    const float* wv;          // coef_mode = 1: zero-padded weights [M][24] (w0 padded[10], 2 pad, w1 padded[10], 2 pad) in V order, else null
     const float* wv_c;        // ... in the caller's order
     const int32_t* v2h;       // V-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
@@ -277,19 +277,72 @@ interp_il_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float
 // memory; all per-sample loads are warp-uniform broadcasts.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kIwWarps = 4;          // warps per CTA, 32 consecutive samples of the walk order each
-constexpr int kIwRec = 20;           // floats per staged sample: w0 padded [8], w1 padded [8], base, output index, 2 pad
-                                     // (5 float4: 5 s mod 8 is a permutation -> conflict-free 128-bit stores)
+constexpr int kIwRec = 28;           // floats per staged sample: w0 padded [10], 2 pad, w1 padded [10], 2 pad, key, output index, 2 pad
+                                     // (7 float4: 7 s mod 8 is a permutation -> conflict-free 128-bit stores)
+// Window shapes (rows x columns of grid cells, <= 64 cells = 128 registers per lane).  A readout that runs along the grid
+// columns stays in ONE stencil base row for many samples: a 6 x 10 window then serves five samples where the 8 x 8 one
+// serves three.  The plan picks, group by group, the shape with the fewest window cells per sample (config 2, caller's
+// order: 20.1 cells per sample with 8 x 8 alone, 15.9 with the five shapes).  shape id -> (rows, columns):
+constexpr int kIwShapes = 5;
+__host__ __device__ __forceinline__ constexpr int iw_rows(int sh) { return sh == 0 ? 8 : (sh == 1 ? 6 : (sh == 2 ? 10 : (sh == 3 ? 7 : 9))); }
+__host__ __device__ __forceinline__ constexpr int iw_cols(int sh) { return sh == 0 ? 8 : (sh == 1 ? 10 : (sh == 2 ? 6 : (sh == 3 ? 9 : 7))); }
+// group key (plan, per sample): base row | base column << 10 | shape << 20
 
-__device__ __forceinline__ void il_pad8(const float (&w)[kJ], int o, float4& a, float4& b) {
-    const bool o0 = o == 0, o1 = o == 1;
-    a.x = o0 ? w[0] : 0.f;
-    a.y = o0 ? w[1] : (o1 ? w[0] : 0.f);
-    a.z = o0 ? w[2] : (o1 ? w[1] : w[0]);
-    a.w = o0 ? w[3] : (o1 ? w[2] : w[1]);
-    b.x = o0 ? w[4] : (o1 ? w[3] : w[2]);
-    b.y = o0 ? w[5] : (o1 ? w[4] : w[3]);
-    b.z = o0 ? 0.f : (o1 ? w[5] : w[4]);
-    b.w = (o0 || o1) ? 0.f : w[5];
+// zero-padded weight vector of up to 10 entries: p[i] = w[i - o], 0 <= i - o < 6, else 0   (o in 0..4)
+__device__ __forceinline__ void il_pad10(const float (&w)[kJ], int o, float (&p)[12]) {
+#pragma unroll
+    for (int i = 0; i < 12; ++i) {
+        float v = 0.f;
+#pragma unroll
+        for (int oo = 0; oo < 5; ++oo)
+            if (i - oo >= 0 && i - oo < kJ) v = (o == oo) ? w[i - oo] : v;
+        p[i] = v;
+    }
+}
+
+// one group of the walk: load its R x C window once, then interpolate its samples t, t + 1, ... while the key stays the same
+template <int R, int C, bool CALLER>
+__device__ __forceinline__ int iw_group(const float* __restrict__ recw, int t, int cnt, int key, const float2* __restrict__ G,
+                                        int K0, int K1, float2 (*otile)[33], int obase, float2* __restrict__ y_il_grp, int lane) {
+    float2 win[R][C];
+    const int br = key & 1023, bc = (key >> 10) & 1023;
+    if (bc + C <= K1) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const float2* __restrict__ pr = G + ((int64_t)((br + i) & (K0 - 1)) * K1 + bc) * kIL;
+#pragma unroll
+            for (int j = 0; j < C; ++j) win[i][j] = __ldg(pr + j * kIL);
+        }
+    } else {      // the window crosses the periodic seam of axis 1
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const float2* __restrict__ pr = G + (int64_t)((br + i) & (K0 - 1)) * K1 * kIL;
+#pragma unroll
+            for (int j = 0; j < C; ++j) win[i][j] = __ldg(pr + (int64_t)((bc + j) & (K1 - 1)) * kIL);
+        }
+    }
+    do {
+        const float* r = recw + t * kIwRec;
+        float w0[12], w1[12];
+#pragma unroll
+        for (int v4 = 0; v4 < 3; ++v4) {
+            const float4 a = *reinterpret_cast<const float4*>(r + 4 * v4), b = *reinterpret_cast<const float4*>(r + 12 + 4 * v4);
+            w0[4 * v4] = a.x; w0[4 * v4 + 1] = a.y; w0[4 * v4 + 2] = a.z; w0[4 * v4 + 3] = a.w;
+            w1[4 * v4] = b.x; w1[4 * v4 + 1] = b.y; w1[4 * v4 + 2] = b.z; w1[4 * v4 + 3] = b.w;
+        }
+        float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            float2 rs = __fmul2_rn(make_float2(w1[0], w1[0]), win[i][0]);
+#pragma unroll
+            for (int j = 1; j < C; ++j) rs = __ffma2_rn(make_float2(w1[j], w1[j]), win[i][j], rs);
+            acc = __ffma2_rn(make_float2(w0[i], w0[i]), rs, acc);
+        }
+        if (CALLER) otile[obase + t][lane] = acc;
+        else y_il_grp[(int64_t)__float_as_int(r[25]) * kIL + lane] = acc;
+        ++t;
+    } while (t < cnt && __float_as_int(recw[t * kIwRec + 24]) == key);
+    return t;
 }
 
 template <bool CALLER>
@@ -308,76 +361,43 @@ interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, f
     const float2* __restrict__ G = grid_il + (int64_t)grp * g.cells * kIL + lane;
     const int64_t w0s = s0 + warp * 32;
     const int cnt = (int)max((int64_t)0, min((int64_t)32, g.M - w0s));
-    {   // stage: lane = sample
-        float4 r0, r1, r2, r3, r4;
-        if (lane < cnt) {
-            const int64_t si = w0s + lane;
-            const uint32_t gb = __ldg(&gbs[si]);
-            const float* __restrict__ wt = CALLER ? s.wv_c : s.wv;
-            if (wt) {       // coef_mode = 1: precomputed (float64-built) padded weights, 64 contiguous bytes per sample
-                const float4* __restrict__ t4 = reinterpret_cast<const float4*>(wt + si * 16);
-                r0 = __ldg(t4); r1 = __ldg(t4 + 1); r2 = __ldg(t4 + 2); r3 = __ldg(t4 + 3);
-            } else {
-                const uint32_t kp = __ldg(&kpk[si]);
-                float w[kJ];
-                kb_weights(P, 0, __ldg(&dlt[si]), w);
-                il_pad8(w, (int)(kp & 1023u) - (int)(gb & 1023u), r0, r1);
-                kb_weights(P, 1, __ldg(&dlt[g.M + si]), w);
-                il_pad8(w, (int)((kp >> 10) & 1023u) - (int)((gb >> 10) & 1023u), r2, r3);
-            }
-            r4 = make_float4(__int_as_float((int)gb), __int_as_float(CALLER ? 0 : __ldg(&s.v2h[si])), 0.f, 0.f);
+    if (lane < cnt) {   // stage: lane = sample
+        const int64_t si = w0s + lane;
+        const uint32_t gb = __ldg(&gbs[si]);
+        float* r = &recs[warp][lane][0];
+        const float* __restrict__ wt = CALLER ? s.wv_c : s.wv;
+        if (wt) {       // coef_mode = 1: precomputed (float64-built) padded weights, 96 contiguous bytes per sample
+            const float4* __restrict__ t4 = reinterpret_cast<const float4*>(wt + si * 24);
+#pragma unroll
+            for (int v4 = 0; v4 < 6; ++v4) reinterpret_cast<float4*>(r)[v4] = __ldg(t4 + v4);
         } else {
-            r0 = r1 = r2 = r3 = make_float4(0.f, 0.f, 0.f, 0.f);
-            r4 = make_float4(__int_as_float(-1), __int_as_float(0), 0.f, 0.f);
+            const uint32_t kp = __ldg(&kpk[si]);
+            float w[kJ], pd[12];
+            kb_weights(P, 0, __ldg(&dlt[si]), w);
+            il_pad10(w, (int)(kp & 1023u) - (int)(gb & 1023u), pd);
+#pragma unroll
+            for (int v4 = 0; v4 < 3; ++v4) reinterpret_cast<float4*>(r)[v4] = make_float4(pd[4 * v4], pd[4 * v4 + 1], pd[4 * v4 + 2], pd[4 * v4 + 3]);
+            kb_weights(P, 1, __ldg(&dlt[g.M + si]), w);
+            il_pad10(w, (int)((kp >> 10) & 1023u) - (int)((gb >> 10) & 1023u), pd);
+#pragma unroll
+            for (int v4 = 0; v4 < 3; ++v4) reinterpret_cast<float4*>(r)[3 + v4] = make_float4(pd[4 * v4], pd[4 * v4 + 1], pd[4 * v4 + 2], pd[4 * v4 + 3]);
         }
-        float4* r = reinterpret_cast<float4*>(&recs[warp][lane][0]);
-        r[0] = r0; r[1] = r1; r[2] = r2; r[3] = r3; r[4] = r4;
+        reinterpret_cast<float4*>(r)[6] = make_float4(__int_as_float((int)gb), __int_as_float(CALLER ? 0 : __ldg(&s.v2h[si])), 0.f, 0.f);
     }
     __syncwarp();
-    float2 win[8][8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-#pragma unroll
-        for (int j = 0; j < 8; ++j) win[i][j] = make_float2(0.f, 0.f);
-    int cur = -1;
+    const float* recw = &recs[warp][0][0];
+    float2* __restrict__ yg = CALLER ? nullptr : y_out + (int64_t)grp * g.M * kIL;
+    int t = 0;
 #pragma unroll 1
-    for (int t = 0; t < cnt; ++t) {
-        const float* r = &recs[warp][t][0];
-        const float4 a0 = *reinterpret_cast<const float4*>(r), a1 = *reinterpret_cast<const float4*>(r + 4);
-        const float4 b0 = *reinterpret_cast<const float4*>(r + 8), b1 = *reinterpret_cast<const float4*>(r + 12);
-        const float2 mm = *reinterpret_cast<const float2*>(r + 16);
-        const int key = __float_as_int(mm.x);
-        if (key != cur) {       // new group: load its 8 x 8 window (rows and columns wrap periodically)
-            cur = key;
-            const int br = key & 1023, bc = (key >> 10) & 1023;
-            if (bc + 8 <= K1) {
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float2* __restrict__ pr = G + ((int64_t)((br + i) & (K0 - 1)) * K1 + bc) * kIL;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) win[i][j] = __ldg(pr + j * kIL);
-                }
-            } else {
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float2* __restrict__ pr = G + (int64_t)((br + i) & (K0 - 1)) * K1 * kIL;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) win[i][j] = __ldg(pr + (int64_t)((bc + j) & (K1 - 1)) * kIL);
-                }
-            }
+    while (t < cnt) {
+        const int key = __float_as_int(recw[t * kIwRec + 24]);
+        switch ((key >> 20) & 7) {       // warp-uniform
+            case 1: t = iw_group<iw_rows(1), iw_cols(1), CALLER>(recw, t, cnt, key, G, K0, K1, otile, warp * 32, yg, lane); break;
+            case 2: t = iw_group<iw_rows(2), iw_cols(2), CALLER>(recw, t, cnt, key, G, K0, K1, otile, warp * 32, yg, lane); break;
+            case 3: t = iw_group<iw_rows(3), iw_cols(3), CALLER>(recw, t, cnt, key, G, K0, K1, otile, warp * 32, yg, lane); break;
+            case 4: t = iw_group<iw_rows(4), iw_cols(4), CALLER>(recw, t, cnt, key, G, K0, K1, otile, warp * 32, yg, lane); break;
+            default: t = iw_group<iw_rows(0), iw_cols(0), CALLER>(recw, t, cnt, key, G, K0, K1, otile, warp * 32, yg, lane); break;
         }
-        const float w0[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-        const float w1[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
-        float2 acc = make_float2(0.f, 0.f);
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            float2 rs = __fmul2_rn(make_float2(w1[0], w1[0]), win[i][0]);
-#pragma unroll
-            for (int j = 1; j < 8; ++j) rs = __ffma2_rn(make_float2(w1[j], w1[j]), win[i][j], rs);
-            acc = __ffma2_rn(make_float2(w0[i], w0[i]), rs, acc);
-        }
-        if (CALLER) otile[warp * 32 + t][lane] = acc;
-        else y_out[((int64_t)grp * g.M + __float_as_int(mm.y)) * kIL + lane] = acc;
     }
     if (CALLER) {     // y_out is the caller's y[batch][M]: warp w writes images 8 w .. 8 w + 7, 128 consecutive samples each
         __syncthreads();
@@ -386,7 +406,7 @@ interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, f
         for (int li = 0; li < kIL / kIwWarps; ++li) {
             const int l = warp * (kIL / kIwWarps) + li, b = grp * kIL + l;
             if (b >= batch) continue;
-            for (int t = lane; t < tot; t += 32) y_out[(int64_t)b * g.M + s0 + t] = otile[t][l];
+            for (int tt = lane; tt < tot; tt += 32) y_out[(int64_t)b * g.M + s0 + tt] = otile[tt][l];
         }
     }
 }

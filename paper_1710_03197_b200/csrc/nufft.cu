@@ -827,23 +827,36 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
         const int r = row_of(kp), c = col_of(kp);
         return ((int64_t)(c / 3) * nbr + r / 3) * 9 + (r % 3) * 3 + (c % 3);
     }, (int64_t)nbc * nbr * 9, perm_v, bins_v);
-    // window groups of a walk order: maximal runs of consecutive samples whose stencil bases fit a 3 x 3 box (no wrap
-    // inside a group); every sample records the base cell (row | col << 10) of its group
+    // window groups of a walk order (interp_il_win_kernel): the order is cut into runs of consecutive samples whose stencil
+    // bases fit the span of a window shape (rows x columns of cells: 8x8, 6x10, 10x6, 7x9, 9x7 -> base spans 2x2, 0x4, 4x0,
+    // 1x3, 3x1); greedily, the shape with the fewest window cells per sample wins.  Runs never cross a 32-sample boundary
+    // (one warp walks 32 consecutive samples) and never wrap.  Every sample records base row | base column << 10 | shape << 20.
     auto window_groups = [&](auto kp_at, std::vector<uint32_t>& gb) {
         gb.resize(M);
         int64_t i = 0;
         while (i < M) {
-            int lo0 = row_of(kp_at(i)), hi0 = lo0, lo1 = col_of(kp_at(i)), hi1 = lo1;
-            int64_t j = i + 1;
-            for (; j < M; ++j) {
-                const int r = row_of(kp_at(j)), c = col_of(kp_at(j));
-                const int nlo0 = std::min(lo0, r), nhi0 = std::max(hi0, r), nlo1 = std::min(lo1, c), nhi1 = std::max(hi1, c);
-                if (nhi0 - nlo0 > 2 || nhi1 - nlo1 > 2) break;
-                lo0 = nlo0; hi0 = nhi0; lo1 = nlo1; hi1 = nhi1;
+            const int64_t cap = 32 - (i % 32);
+            int best_sh = 0, best_lo0 = 0, best_lo1 = 0;
+            int64_t best_n = 0;
+            for (int sh = 0; sh < kIwShapes; ++sh) {
+                const int sp0 = iw_rows(sh) - kJ, sp1 = iw_cols(sh) - kJ;
+                int lo0 = row_of(kp_at(i)), hi0 = lo0, lo1 = col_of(kp_at(i)), hi1 = lo1;
+                int64_t j = i + 1;
+                for (; j < M && j - i < cap; ++j) {
+                    const int r = row_of(kp_at(j)), c = col_of(kp_at(j));
+                    const int nlo0 = std::min(lo0, r), nhi0 = std::max(hi0, r), nlo1 = std::min(lo1, c), nhi1 = std::max(hi1, c);
+                    if (nhi0 - nlo0 > sp0 || nhi1 - nlo1 > sp1) break;
+                    lo0 = nlo0; hi0 = nhi0; lo1 = nlo1; hi1 = nhi1;
+                }
+                const int64_t n = j - i;
+                // cells per sample: rows * cols / n, compared by cross-multiplication (all shapes hold 60-64 cells)
+                if (best_n == 0 || (int64_t)iw_rows(sh) * iw_cols(sh) * best_n < (int64_t)iw_rows(best_sh) * iw_cols(best_sh) * n) {
+                    best_n = n; best_sh = sh; best_lo0 = lo0; best_lo1 = lo1;
+                }
             }
-            const uint32_t base = (uint32_t)lo0 | ((uint32_t)lo1 << 10);
-            for (int64_t k = i; k < j; ++k) gb[k] = base;
-            i = j;
+            const uint32_t base = (uint32_t)best_lo0 | ((uint32_t)best_lo1 << 10) | ((uint32_t)best_sh << 20);
+            for (int64_t k = i; k < i + best_n; ++k) gb[k] = base;
+            i += best_n;
         }
     };
     // ---- V^H order: bins (band, class, row)
@@ -868,14 +881,14 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
     }
     // coef_mode = 1: the zero-padded weight vectors of interp_il_win_kernel, float64-built, per walk order
     auto weight_table = [&](auto sample_at, const std::vector<uint32_t>& gb, std::vector<float>& tab) {
-        tab.assign((size_t)M * 16, 0.f);
+        tab.assign((size_t)M * 24, 0.f);
         for (int64_t i = 0; i < M; ++i) {
             const int64_t m = sample_at(i);
             double w0[kJ], w1[kJ];
             if (p->minmax) { p->mm[0].weights(delta64[m], w0); p->mm[1].weights(delta64[M + m], w1); }
             else { host::kb_weights_f64(delta64[m], J, beta, w0); host::kb_weights_f64(delta64[M + m], J, beta, w1); }
             const int o0 = row_of(kpack[m]) - (int)(gb[i] & 1023u), o1 = col_of(kpack[m]) - (int)((gb[i] >> 10) & 1023u);
-            for (int j = 0; j < kJ; ++j) { tab[(size_t)i * 16 + o0 + j] = (float)w0[j]; tab[(size_t)i * 16 + 8 + o1 + j] = (float)w1[j]; }
+            for (int j = 0; j < kJ; ++j) { tab[(size_t)i * 24 + o0 + j] = (float)w0[j]; tab[(size_t)i * 24 + 12 + o1 + j] = (float)w1[j]; }
         }
     };
     std::vector<float> wtab((size_t)M * kTabW, 0.f);
