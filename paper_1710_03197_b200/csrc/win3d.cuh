@@ -330,19 +330,21 @@ interp_win_3d_kernel(SampleData s, GridGeom g, const WorkItem* __restrict__ item
 // ------------------------------------------------------------------------------------------------------------
 // V^H: G += w0 w1 w2 y, window accumulators in registers, flushed to the shared tile under a lock
 // ------------------------------------------------------------------------------------------------------------
+// Tile lock of a CTA with more than one warp.  Everything it orders is SHARED memory touched by warps of one SM: the
+// shared-memory pipe executes a warp's LDS / STS / ATOMS in issue order, so the read-modify-writes of the critical section
+// lie between the warp's own CAS and EXCH without a fence.  The asm clobbers stop the compiler from moving shared-memory
+// accesses across the lock.  (Measured, config 4: 2 / 4 warps per CTA under this lock 0.363 / 0.481 ms against 0.315 ms for
+// one warp per CTA and no lock -- with or without fences the shared tile does not pay; kW3GridWarps = 1 is the default.)
 __device__ __forceinline__ void w3_lock(int* l, int lane) {
-    if (lane == 0) {
-        while (atomicCAS(l, 0, 1) != 0) __nanosleep(20);
-        __threadfence_block();
-    }
+    if (lane == 0)
+        while (atomicCAS(l, 0, 1) != 0) {}
     __syncwarp();
+    asm volatile("" ::: "memory");
 }
 __device__ __forceinline__ void w3_unlock(int* l, int lane) {
+    asm volatile("" ::: "memory");
     __syncwarp();
-    if (lane == 0) {
-        __threadfence_block();
-        atomicExch(l, 0);
-    }
+    if (lane == 0) atomicExch(l, 0);
 }
 
 template <int NW, bool TABLE>
