@@ -1,6 +1,7 @@
 // common.cuh -- small shared helpers of the CUDA path (complex arithmetic, error plumbing).
 // Part of the product path; shares nothing with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -105,6 +106,32 @@ __device__ __forceinline__ void bulk_commit_and_wait_read() {
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// ---- tensor-map TMA (cp.async.bulk.tensor, SASS UTMALDG / UTMAREDG): ONE copy moves the whole padded tile
+// (24 x 13 x 13 cells) between the grid and shared memory.  round 2: with one 192-byte cp.async.bulk per padded row
+// (169 per CTA, 1.9 M per launch) the per-SM TMA issue rate, not bandwidth, bounded both 3-D kernels at ~0.24 ms.
+// The map views the planar grid [B][K0][K1][K2] complex64 as float32 [B][K0][K1][2 K2]; box = {48, 13, 13, 1}.  Tiles
+// whose padded box crosses the periodic seam keep the row-copy path (a tensor box cannot wrap).
+__device__ __forceinline__ void tma_load_tile_4d(void* smem_dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3,
+                                                 uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_tile_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3,
+                                                       const void* smem_src) {
+    asm volatile("cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(smem_src)) : "memory");
+}
+
+// 2-D planar grid [B][K0][K1] complex64 seen as float32 [B][K0][2 K1]; box = {2 pitch, P0, 1}
+__device__ __forceinline__ void tma_load_tile_3d(void* smem_dst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_tile_3d(const CUtensorMap* tm, int c0, int c1, int c2, const void* smem_src) {
+    asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2, %3}], [%4];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(smem_src)) : "memory");
+}
+
 // Programmatic dependent launch (PDL): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
 // while its predecessor in the stream is still running; pdl_enter() is its first statement: it lets the NEXT kernel in the
 // stream be scheduled early (launch_dependents) and then waits until the predecessor grid has completed and its writes are

@@ -450,13 +450,24 @@ static tmap_encode_fn tmap_encoder() {
 static bool tile_tensor_map(nufft_plan_t p, int batch, const float2* grid, CUtensorMap* tm) {
     std::memset(tm, 0, sizeof(*tm));
     tmap_encode_fn enc = tmap_encoder();
-    if (!enc || p->d != 3) return false;
-    const cuuint64_t gdim[4] = {(cuuint64_t)2 * p->K[2], (cuuint64_t)p->K[1], (cuuint64_t)p->K[0], (cuuint64_t)batch};
-    const cuuint64_t gstr[3] = {(cuuint64_t)p->K[2] * 8, (cuuint64_t)p->K[1] * p->K[2] * 8, (cuuint64_t)p->cells * 8};
-    const cuuint32_t box[4] = {2 * k3Pitch, k3P1, k3P0, 1};
+    if (!enc) return false;
     const cuuint32_t est[4] = {1, 1, 1, 1};
-    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)grid, gdim, gstr, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    if (p->d == 3) {
+        const cuuint64_t gdim[4] = {(cuuint64_t)2 * p->K[2], (cuuint64_t)p->K[1], (cuuint64_t)p->K[0], (cuuint64_t)batch};
+        const cuuint64_t gstr[3] = {(cuuint64_t)p->K[2] * 8, (cuuint64_t)p->K[1] * p->K[2] * 8, (cuuint64_t)p->cells * 8};
+        const cuuint32_t box[4] = {2 * k3Pitch, k3P1, k3P0, 1};
+        return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)grid, gdim, gstr, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    }
+    if (p->d == 2) {      // planar 2-D grid [batch][K0][K1] as float32 [batch][K0][2 K1]; box = one padded V / V^H tile
+        if (2 * p->tg.pitch > 256 || p->tg.P[0] > 256) return false;
+        const cuuint64_t gdim[3] = {(cuuint64_t)2 * p->K[1], (cuuint64_t)p->K[0], (cuuint64_t)batch};
+        const cuuint64_t gstr[2] = {(cuuint64_t)p->K[1] * 8, (cuuint64_t)p->cells * 8};
+        const cuuint32_t box[3] = {(cuuint32_t)(2 * p->tg.pitch), (cuuint32_t)p->tg.P[0], 1};
+        return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)grid, gdim, gstr, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    }
+    return false;
 }
 
 // Widths other than kJ: direct V and atomic V^H, one instantiation per (d, J)
@@ -510,8 +521,10 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
     if (p->d == 2 && p->opts.interp_mode == 0 && p->n_items > 0 && p->K[1] >= p->tg.pitch) {
         // tile-staged V: one CTA per V^H work item (the same tile-sorted sample ranges)
         const dim3 tb((unsigned)p->n_items, (unsigned)batch);
+        CUtensorMap tm;
+        const int use_tm = tile_tensor_map(p, batch, grid, &tm) ? 1 : 0;
         launch_pdl(interp_tiled_2d_kernel, tb, dim3(128), (size_t)p->tg.tile_cells * 8 + 16, st, sample_data(p), grid_geom(p), p->tg,
-                   (const WorkItem*)p->d_items, grid, y, p->poly);
+                   (const WorkItem*)p->d_items, grid, y, p->poly, tm, use_tm);
         CU_TRY(cudaGetLastError());
         p->launches++;
         return NUFFT_OK;
@@ -527,7 +540,7 @@ static int run_interp(nufft_plan_t p, int batch, const float2* grid, float2* y, 
 
 // a4: grid = V^H y
 static constexpr int kGrid2dWarps = 8;
-static size_t smem_grid2d(nufft_plan_t p) { return (size_t)kGrid2dWarps * ((size_t)p->tg.tile_cells * 8 + kStageBytes); }
+static size_t smem_grid2d(nufft_plan_t p) { return (size_t)kGrid2dWarps * (size_t)grid2d_warp_bytes(p->tg.tile_cells); }
 static size_t smem_grid3d(nufft_plan_t p) { return (size_t)p->tg.tile_cells * 8 + (size_t)kStage3dBytes; }
 
 static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid, cudaStream_t st) {
@@ -562,9 +575,11 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
     } else if (p->d == 2) {
         const dim3 blocks((unsigned)((p->n_items + kGrid2dWarps - 1) / kGrid2dWarps), (unsigned)batch);
         const size_t sm = smem_grid2d(p);
-        if (det) gridding_tiled_2d_kernel<true><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly);
+        CUtensorMap tm;
+        const int use_tm = (!det && tile_tensor_map(p, batch, grid, &tm)) ? 1 : 0;
+        if (det) { std::memset(&tm, 0, sizeof(tm)); gridding_tiled_2d_kernel<true><<<blocks, kGrid2dWarps * 32, sm, st>>>(sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->d_slabs, slab_stride, p->poly, tm, 0); }
         else     launch_pdl(gridding_tiled_2d_kernel<false>, blocks, dim3(kGrid2dWarps * 32), sm, st, sample_data(p), grid_geom(p), p->tg,
-                            (const WorkItem*)p->d_items, p->n_items, y, grid, (float2*)nullptr, (int64_t)0, p->poly);
+                            (const WorkItem*)p->d_items, p->n_items, y, grid, (float2*)nullptr, (int64_t)0, p->poly, tm, use_tm);
     } else if (!det && p->win3d && p->opts.adjoint_mode == 0) {
         const dim3 blocks((unsigned)p->n_items, (unsigned)batch);
         CUtensorMap tm;
@@ -1032,7 +1047,7 @@ static int plan_build(nufft_plan_t p, const double* om) {
         tg.tile_cells = (d == 3) ? tg.P[0] * tg.P[1] * pitch : tg.P[0] * pitch;
         // a user tile whose shared-memory footprint exceeds the opt-in (200 KB) would fail at every adjoint launch
         const size_t need = (d == 3) ? (size_t)tg.tile_cells * 8 + (size_t)kStage3dBytes
-                                     : (d == 2 ? (size_t)8 * ((size_t)tg.tile_cells * 8 + kStageBytes) : 0);
+                                     : (d == 2 ? (size_t)8 * (size_t)grid2d_warp_bytes(tg.tile_cells) : 0);
         if (need > (size_t)200 * 1024) return NUFFT_EINVAL;
     }
     // per-sample split (float64) and tile id

@@ -178,6 +178,8 @@ struct TileGeom {
 constexpr int kStageRow = 7;   // float4 slots per sample in rowrec (6 used; 7 keeps 8-lane phases conflict-free)
 constexpr int kStageCol = 5;   // float2 slots per sample in colrec (4 used)
 constexpr int kStageBytes = 32 * (kStageRow * 16 + kStageCol * 8);
+// shared memory of one warp of gridding_tiled_2d_kernel: padded tile + staging, rounded up to 128 bytes
+__host__ __device__ __forceinline__ int grid2d_warp_bytes(int tile_cells) { return ((tile_cells * 8 + kStageBytes + 127) / 128) * 128; }
 
 // One lane prepares one sample of a 2-D work item.
 __device__ __forceinline__ void stage_sample_2d(const KernelPoly& P, float4* rowrec, float2* colrec, int lane,
@@ -253,14 +255,14 @@ template <bool DET>
 __global__ void __launch_bounds__(256)
 gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items, int n_items,
                          const float2* __restrict__ y, float2* __restrict__ grid, float2* __restrict__ slabs,
-                         int64_t slab_batch_stride, KernelPoly P) {
+                         int64_t slab_batch_stride, KernelPoly P, const __grid_constant__ CUtensorMap tmap, int use_tmap) {
     pdl_enter();
     extern __shared__ float4 smem4[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int item = blockIdx.x * nw + warp;
     if (item >= n_items) return;
     const int b = blockIdx.y;
-    const int per_warp4 = (tg.tile_cells * 8 + kStageBytes) / 16;
+    const int per_warp4 = grid2d_warp_bytes(tg.tile_cells) / 16;          // 128-byte multiple: every warp's tile is TMA-aligned
     float2* tile = reinterpret_cast<float2*>(smem4 + (size_t)warp * per_warp4);
     float4* rowrec = reinterpret_cast<float4*>(tile + tg.tile_cells);
     float2* colrec = reinterpret_cast<float2*>(rowrec + 32 * kStageRow);
@@ -287,6 +289,14 @@ gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
     }
     if (!DET) {       // flush by the TMA engine: one bulk f32 reduce-add per padded row (split at the seam of axis 1)
         fence_proxy_async_smem();
+        if (use_tmap && o[0] + tg.P[0] <= g.K[0] && o[1] + tg.pitch <= g.K[1]) {      // one tensor-map reduce-add per item
+            __syncwarp();
+            if (lane == 0) {
+                tma_reduce_add_tile_3d(&tmap, 2 * o[1], o[0], b, tile);
+                bulk_commit_and_wait_read();
+            }
+            return;
+        }
         float2* __restrict__ Gb = grid + (int64_t)b * g.cells;
         for (int row = lane; row < tg.P[0]; row += 32) {
             const int gx = (o[0] + row) & (g.K[0] - 1), gz = o[1] & (g.K[1] - 1);
@@ -468,7 +478,8 @@ gridding_merge_kernel(GridGeom g, TileGeom tg, int nt0, int nt1, int nt2, const 
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 interp_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items,
-                       const float2* __restrict__ grid, float2* __restrict__ y, KernelPoly P) {
+                       const float2* __restrict__ grid, float2* __restrict__ y, KernelPoly P,
+                       const __grid_constant__ CUtensorMap tmap, int use_tmap) {
     pdl_enter();
     extern __shared__ float4 smem4[];
     float2* tile = reinterpret_cast<float2*>(smem4);
@@ -484,13 +495,17 @@ interp_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __
         mbar_expect_tx(bar, (uint32_t)(tg.P[0] * tg.pitch * 8));
     }
     __syncthreads();
-    for (int row = threadIdx.x; row < tg.P[0]; row += blockDim.x) {
-        const int gx = (o[0] + row) & (K0 - 1), gz = o[1] & (K1 - 1);
-        const float2* src = G + (int64_t)gx * K1;
-        float2* dst = tile + row * tg.pitch;
-        const int first = min(tg.pitch, K1 - gz);
-        bulk_g2s(dst, src + gz, (uint32_t)first * 8, bar);
-        if (first < tg.pitch) bulk_g2s(dst + first, src, (uint32_t)(tg.pitch - first) * 8, bar);
+    if (use_tmap && o[0] + tg.P[0] <= K0 && o[1] + tg.pitch <= K1) {      // one tensor-map copy for the whole padded tile
+        if (threadIdx.x == 0) tma_load_tile_3d(tile, &tmap, 2 * o[1], o[0], b, bar);
+    } else {                                                              // seam tiles: one bulk copy per row, split at the seam
+        for (int row = threadIdx.x; row < tg.P[0]; row += blockDim.x) {
+            const int gx = (o[0] + row) & (K0 - 1), gz = o[1] & (K1 - 1);
+            const float2* src = G + (int64_t)gx * K1;
+            float2* dst = tile + row * tg.pitch;
+            const int first = min(tg.pitch, K1 - gz);
+            bulk_g2s(dst, src + gz, (uint32_t)first * 8, bar);
+            if (first < tg.pitch) bulk_g2s(dst + first, src, (uint32_t)(tg.pitch - first) * 8, bar);
+        }
     }
     // the sample's plan data and weights are fetched / evaluated while the copies are in flight
     float2* __restrict__ yb = y + (int64_t)b * g.M;

@@ -21,28 +21,10 @@
 //
 // The weights outside a sample's 6-cell support are exact zeros, so the arithmetic is that of the plain stencil sum.
 #pragma once
-#include <cuda.h>
-
 #include "common.cuh"
 #include "spread_interp.cuh"
 
 namespace nufft {
-
-// ---- tensor-map TMA (cp.async.bulk.tensor, SASS UTMALDG / UTMAREDG): ONE copy moves the whole padded tile
-// (24 x 13 x 13 cells) between the grid and shared memory.  profiles/r02a: with one 192-byte cp.async.bulk per padded row
-// (169 per CTA, 1.9 M per launch) the per-SM TMA issue rate, not bandwidth, bounded both 3-D kernels at ~0.24 ms.
-// The map views the planar grid [B][K0][K1][K2] complex64 as float32 [B][K0][K1][2 K2]; box = {48, 13, 13, 1}.  Tiles
-// whose padded box crosses the periodic seam keep the row-copy path (a tensor box cannot wrap).
-__device__ __forceinline__ void tma_load_tile_4d(void* smem_dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3,
-                                                 uint64_t* bar) {
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tma_reduce_add_tile_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3,
-                                                       const void* smem_src) {
-    asm volatile("cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
-                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(smem_src)) : "memory");
-}
 
 constexpr int kW3Rec = 28;                  // floats per staged sample record (7 float4; 7 s mod 8 is a permutation:
                                             // the 128-bit stores of 8 consecutive lanes fall into distinct bank quads)
