@@ -48,6 +48,7 @@ struct IlRowParams {
 template <int K>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS, (K == 512) ? 4 : 1)
 fft_il_rows_fwd_kernel(IlRowParams p) {
+    pdl_enter();
     constexpr int N = K / 2, T = Rad<K>::TS;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x % T, q0 = threadIdx.x / T;
@@ -76,6 +77,7 @@ fft_il_rows_fwd_kernel(IlRowParams p) {
 template <int K>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
 fft_il_rows_adj_kernel(IlRowParams p) {
+    pdl_enter();
     constexpr int N = K / 2, T = Rad<K>::TS;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x % T, q0 = threadIdx.x / T;
@@ -107,6 +109,7 @@ fft_il_rows_adj_kernel(IlRowParams p) {
 template <int K>
 __global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::TS)
 fft_il_rows_adj_coilsum_kernel(IlRowParams p) {
+    pdl_enter();
     constexpr int N = K / 2, T = Rad<K>::TS, E = Rad<K>::E;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x % T, q0 = threadIdx.x / T;
@@ -349,6 +352,7 @@ template <bool CALLER>
 __global__ void __launch_bounds__(kIwWarps * 32, 3)
 interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, float2* __restrict__ y_out, int batch,
                      KernelPoly P) {
+    pdl_enter();
     __shared__ __align__(16) float recs[kIwWarps][32][kIwRec];
     __shared__ float2 otile[CALLER ? kIwWarps * 32 : 1][33];
     const uint32_t* __restrict__ kpk = CALLER ? s.kpack_c : s.kpack;
@@ -417,6 +421,7 @@ interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, f
 __global__ void __launch_bounds__(128)
 y_to_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y, float2* __restrict__ y_il, int64_t M,
                int batch) {
+    pdl_enter();
     __shared__ float2 tile[4][32][33];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = blockIdx.y;
@@ -444,6 +449,7 @@ y_to_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y, fl
 __global__ void __launch_bounds__(128)
 y_from_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y_il, float2* __restrict__ y, int64_t M,
                  int batch) {
+    pdl_enter();
     __shared__ float2 tile[4][32][33];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = blockIdx.y;
@@ -549,6 +555,7 @@ template <int NG>
 __global__ void __launch_bounds__(256)
 gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const float2* __restrict__ y_il,
                    float2* __restrict__ grid_il, int group0) {
+    pdl_enter();
     constexpr int CAP = GridStage<NG>::CAP;
     extern __shared__ __align__(128) unsigned char gsm[];
     float2* y_s = reinterpret_cast<float2*>(gsm);                                           // [NG][3][CAP][32]

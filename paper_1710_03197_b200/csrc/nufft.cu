@@ -232,7 +232,16 @@ static cudaError_t configure_all() {
 // ------------------------------------------------------------------------------------------------------------
 // FFT pass launchers
 // ------------------------------------------------------------------------------------------------------------
-// launch with programmatic stream serialization (see pdl_enter in common.cuh)
+// launch with programmatic stream serialization (see pdl_enter in common.cuh).  Measured (cfg2 batch 64): it shortens the
+// forward chain of the interleaved path (0.1905 -> 0.1827 ms) but LENGTHENS its adjoint chain (0.2059 -> 0.2205 ms: the
+// early-resident CTAs of the next kernel take shared memory from the tail of gridding_il), so the interleaved adjoint runners
+// switch it off (PdlOff); the planar path keeps it in both directions (batch-1 adjoint 34.8 -> 27.7 us).
+static thread_local bool t_pdl = true;
+struct PdlOff {
+    bool prev;
+    PdlOff() : prev(t_pdl) { t_pdl = false; }
+    ~PdlOff() { t_pdl = prev; }
+};
 template <class... KArgs, class... Args>
 static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
     cudaLaunchConfig_t cfg{};
@@ -240,7 +249,7 @@ static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+    cfg.attrs = at; cfg.numAttrs = t_pdl ? 1 : 0;
     (void)cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
@@ -619,8 +628,8 @@ static int il_groups(int batch) { return (batch + kIL - 1) / kIL; }
 
 template <int K> static void launch_il_rows(bool adj, const IlRowParams& p, int blocks, cudaStream_t st) {
     constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
-    if (adj) fft_il_rows_adj_kernel<K><<<blocks, threads, smem_cols<K>(), st>>>(p);
-    else     fft_il_rows_fwd_kernel<K><<<blocks, threads, smem_cols<K>(), st>>>(p);
+    if (adj) launch_pdl(fft_il_rows_adj_kernel<K>, dim3(blocks), dim3(threads), smem_cols<K>(), st, p);
+    else     launch_pdl(fft_il_rows_fwd_kernel<K>, dim3(blocks), dim3(threads), smem_cols<K>(), st, p);
 }
 static int dispatch_il_rows(int K, bool adj, const IlRowParams& p, cudaStream_t st) {
     const int T = tile_T(K);
@@ -640,7 +649,7 @@ static int dispatch_il_rows(int K, bool adj, const IlRowParams& p, cudaStream_t 
 }
 template <int K> static void launch_il_rows_coilsum(const IlRowParams& p, cudaStream_t st) {
     constexpr int threads = FftGeom<K>::TPL * Rad<K>::TS;
-    fft_il_rows_adj_coilsum_kernel<K><<<p.n_outer, threads, smem_cols<K>(), st>>>(p);
+    launch_pdl(fft_il_rows_adj_coilsum_kernel<K>, dim3(p.n_outer), dim3(threads), smem_cols<K>(), st, p);
 }
 static int dispatch_il_rows_coilsum(int K, const IlRowParams& p, cudaStream_t st) {
     switch (K) {
@@ -694,6 +703,7 @@ static int run_scale_fft_il(nufft_plan_t p, int batch, const float2* x, float2* 
 // a5 + a6 on the interleaved grid
 static int run_fft_scale_il(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st,
                             bool coil_sum = false) {
+    PdlOff no_pdl;
     {
         ColPassParams c = il_col_params(p, batch, grid);
         c.mult = p->cur_mult; c.mult_shift = 5;
@@ -718,7 +728,7 @@ static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* 
     ProfScope ps(p, "interp", st);
     if (p->opts.interp_mode != 3) {     // register windows over the block-sorted walk (interp_mode = 3: round-1 kernel)
         const dim3 wb((unsigned)((p->M + kIwWarps * 32 - 1) / (kIwWarps * 32)), (unsigned)il_groups(batch));
-        interp_il_win_kernel<false><<<wb, kIwWarps * 32, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
+        launch_pdl(interp_il_win_kernel<false>, wb, dim3(kIwWarps * 32), 0, st, il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
     } else
     interp_il_kernel<false, kInterpChunk><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
     CU_TRY(cudaGetLastError());
@@ -732,7 +742,7 @@ static int run_interp_il_caller(nufft_plan_t p, int batch, const float2* grid, f
     ProfScope ps(p, "interp", st);
     if (p->opts.interp_mode != 3) {
         const dim3 wb((unsigned)((p->M + kIwWarps * 32 - 1) / (kIwWarps * 32)), (unsigned)il_groups(batch));
-        interp_il_win_kernel<true><<<wb, kIwWarps * 32, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
+        launch_pdl(interp_il_win_kernel<true>, wb, dim3(kIwWarps * 32), 0, st, il_plan(p), grid_geom(p), grid, y, batch, p->poly);
     } else
     interp_il_kernel<true, kInterpChunkCaller><<<blocks, 256, 0, st>>>(il_plan(p), grid_geom(p), grid, y, batch, p->poly);
     CU_TRY(cudaGetLastError());
@@ -741,12 +751,13 @@ static int run_interp_il_caller(nufft_plan_t p, int batch, const float2* grid, f
 }
 // caller's y[batch][M] -> d_yil
 static int run_y_to_il(nufft_plan_t p, int batch, const float2* y, cudaStream_t st) {
+    PdlOff no_pdl;
     if (p->M == 0) return NUFFT_OK;
     if (!p->d_yil)
         NU_TRY(dev_alloc((void**)&p->d_yil, (size_t)p->batch_pad * p->M * sizeof(float2), &p->bytes_work));
     const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)il_groups(batch));
     ProfScope ps(p, "y_to_il", st);
-    y_to_il_kernel<<<blocks, 128, 0, st>>>(p->d_il_pos, y, p->d_yil, p->M, batch);
+    launch_pdl(y_to_il_kernel, blocks, dim3(128), 0, st, (const int32_t*)p->d_il_pos, y, p->d_yil, p->M, batch);
     CU_TRY(cudaGetLastError());
     p->launches++;
     return NUFFT_OK;
@@ -756,13 +767,14 @@ static int run_y_from_il(nufft_plan_t p, int batch, const float2* y_il, float2* 
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + 127) / 128), (unsigned)il_groups(batch));
     ProfScope ps(p, "y_from_il", st);
-    y_from_il_kernel<<<blocks, 128, 0, st>>>(p->d_il_pos, y_il, y, p->M, batch);
+    launch_pdl(y_from_il_kernel, blocks, dim3(128), 0, st, (const int32_t*)p->d_il_pos, y_il, y, p->M, batch);
     CU_TRY(cudaGetLastError());
     p->launches++;
     return NUFFT_OK;
 }
 // a4 from y_il
 static int run_gridding_il(nufft_plan_t p, int batch, const float2* y_il, float2* grid, cudaStream_t st) {
+    PdlOff no_pdl;
     if (p->M == 0) {
         CU_TRY(cudaMemsetAsync(grid, 0, (size_t)il_groups(batch) * kIL * p->cells * sizeof(float2), st));
         return NUFFT_OK;
@@ -772,12 +784,12 @@ static int run_gridding_il(nufft_plan_t p, int batch, const float2* y_il, float2
     // CTAs handle two groups (64 images) at a time: the staged weight records and row lookups are shared
     if (ng >= 2) {
         const dim3 blocks((unsigned)p->n_il_items, (unsigned)(ng / 2));
-        gridding_il_kernel<2><<<blocks, 256, GridStage<2>::BYTES, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid, 0);
+        launch_pdl(gridding_il_kernel<2>, blocks, dim3(256), GridStage<2>::BYTES, st, il_plan(p), grid_geom(p), (const IlItem*)p->d_il_items, y_il, grid, 0);
         p->launches++;
     }
     if (ng & 1) {
         const dim3 blocks((unsigned)p->n_il_items, 1u);
-        gridding_il_kernel<1><<<blocks, 256, GridStage<1>::BYTES, st>>>(il_plan(p), grid_geom(p), p->d_il_items, y_il, grid, ng - 1);
+        launch_pdl(gridding_il_kernel<1>, blocks, dim3(256), GridStage<1>::BYTES, st, il_plan(p), grid_geom(p), (const IlItem*)p->d_il_items, y_il, grid, ng - 1);
         p->launches++;
     }
     CU_TRY(cudaGetLastError());
