@@ -385,9 +385,9 @@ fft_rows_full_kernel(float2* __restrict__ data, const float2* __restrict__ tw, i
 
 // ------------------------------------------------------------------------------------------------------------
 // Oversampling ratios other than 2 (SURVEY 8(f)-4 "other sigma"): any even N < K.  The pruned passes above hard-wire
-// K = 2 N (the zero half is a radix digit), so these plans run S + zero-pad and crop + S^H as separate elementwise
-// kernels around the UNPRUNED in-place FFT (fft_rows_full_kernel, fft_cols_kernel<K, false, true>).  Functional, not
-// tuned.  F^H needs no conjugation pass: sum_k g_k e^{+i gamma k p} = FFT(g)[(-p) mod K].
+// K = 2 N (the zero half is a radix digit), so these plans run the UNPRUNED FFT (fft_cols_kernel<K, false, true> for the
+// strided axes) with S + zero-pad and crop + S^H fused into the contiguous-axis pass (fft_rows_pad_kernel /
+// fft_rows_crop_kernel below).  F^H needs no conjugation pass: sum_k g_k e^{+i gamma k p} = FFT(g)[(-p) mod K].
 // ------------------------------------------------------------------------------------------------------------
 struct PadGeom {
     int d;
@@ -395,55 +395,114 @@ struct PadGeom {
     const float* s[3];       // scaling vectors per axis (length N[a])
 };
 
-// a1: grid[b][k] = prod_a s_a[n_a] (c_b[n]) x[n] at k_a = (n_a - N_a/2) mod K_a, zero elsewhere (every cell is written)
-__global__ void __launch_bounds__(256)
-pad_scale_kernel(PadGeom P, const float2* __restrict__ x, const float2* __restrict__ coil, float2* __restrict__ grid,
-                 int64_t cells, int64_t nimg, int same_image) {
-    const int b = blockIdx.y;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cells; i += (int64_t)gridDim.x * blockDim.x) {
-        int64_t r = i, idx = 0, mul = 1;
-        float sc = 1.0f;
-        bool inside = true;
-        for (int a = P.d - 1; a >= 0; --a) {
-            const int k = (int)(r % P.K[a]);
-            r /= P.K[a];
-            const int h = P.N[a] / 2;
-            const int n = (k < h) ? k + h : ((k >= P.K[a] - h) ? k - P.K[a] + h : -1);
-            if (n < 0) { inside = false; break; }
-            sc *= __ldg(&P.s[a][n]);
-            idx += (int64_t)n * mul;
-            mul *= P.N[a];
-        }
-        float2 v = make_float2(0.f, 0.f);
-        if (inside) {
-            v = __ldg(&x[(same_image ? 0 : (int64_t)b * nimg) + idx]);
-            if (coil) v = cmul(v, __ldg(&coil[(int64_t)b * nimg + idx]));
-            v = cscale(v, sc);
-        }
-        grid[(int64_t)b * cells + i] = v;
-    }
+// ------------------------------------------------------------------------------------------------------------
+// sigma != 2 with S + zero-pad and crop + S^H FUSED into the contiguous-axis pass (round 2): the padded grid is never
+// written by a separate pass and the cropped image never read back from one.
+//   forward: fft_rows_pad_kernel runs over ALL grid lines; the loader maps the line's grid coordinates to image samples
+//            (zero outside the image: such lines come out as zeros) and scales; unpruned FFT along the line.
+//   adjoint: the strided passes run first (unpruned, in place); fft_rows_crop_kernel then transforms only the lines the crop
+//            keeps and stores only the N kept outputs of each, at the reversed index (F^H through the forward FFT), scaled.
+// ------------------------------------------------------------------------------------------------------------
+struct SigmaRowParams {
+    PadGeom g;
+    const float2* img_in;     // forward: x [batch][prod N]
+    float2* img_out;          // adjoint: x out
+    float2* grid;             // [batch][prod K]
+    const float2* coil;       // optional [batch][prod N]
+    const float2* tw;         // twiddles of the line axis
+    int64_t cells, nimg;
+    int same_image;           // forward: every batch item reads image 0
+    int nlines;               // forward: batch * prod(K outer);  adjoint: batch * prod(N outer)
+};
+
+// image index of grid coordinate k on an axis of size (N, K), or -1 in the zero-padded part
+__device__ __forceinline__ int pad_map(int k, int N, int K) {
+    const int h = N / 2;
+    return (k < h) ? k + h : ((k >= K - h) ? k - K + h : -1);
 }
 
-// a6 after the forward FFT of the gridded data: x[b][n] = prod_a s_a[n_a] conj(c_b[n]) G[b][(-(n - N/2)) mod K]
-__global__ void __launch_bounds__(256)
-crop_scale_kernel(PadGeom P, const float2* __restrict__ G, const float2* __restrict__ coil, float2* __restrict__ x,
-                  int64_t cells, int64_t nimg) {
-    const int b = blockIdx.y;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nimg; i += (int64_t)gridDim.x * blockDim.x) {
-        int64_t r = i, cell = 0, mul = 1;
-        float sc = 1.0f;
-        for (int a = P.d - 1; a >= 0; --a) {
-            const int n = (int)(r % P.N[a]);
-            r /= P.N[a];
-            const int k = (P.N[a] / 2 - n) & (P.K[a] - 1);       // (-(n - N/2)) mod K, K a power of two
-            sc *= __ldg(&P.s[a][n]);
-            cell += (int64_t)k * mul;
-            mul *= P.K[a];
-        }
-        float2 v = cscale(G[(int64_t)b * cells + cell], sc);
-        if (coil) v = cmul(v, cconj(__ldg(&coil[(int64_t)b * nimg + i])));
-        x[(int64_t)b * nimg + i] = v;
+template <int K>
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::LC)
+fft_rows_pad_kernel(SigmaRowParams p) {
+    pdl_enter();
+    using G = FftGeom<K>;
+    constexpr int TPL = G::TPL, LC = Rad<K>::LC;
+    extern __shared__ float2 smem[];
+    const int lt = threadIdx.x / TPL, q0 = threadIdx.x % TPL;
+    const int line = blockIdx.x * LC + lt;
+    const bool active = line < p.nlines;
+    const int d = p.g.d, NL = p.g.N[d - 1];
+    // line -> (b, outer grid coordinates) -> outer image coordinates (or a zero line)
+    int r = active ? line : 0;
+    int64_t img_off = 0, mul = NL;
+    float so = 1.0f;
+    bool zero_line = false;
+    for (int a = d - 2; a >= 0; --a) {
+        const int k = r % p.g.K[a];
+        r /= p.g.K[a];
+        const int n = pad_map(k, p.g.N[a], p.g.K[a]);
+        if (n < 0) zero_line = true;
+        else { so *= __ldg(&p.g.s[a][n]); img_off += (int64_t)n * mul; }
+        mul *= p.g.N[a];
     }
+    const int b = r;
+    const float2* __restrict__ src = p.img_in + (p.same_image ? 0 : (int64_t)b * p.nimg) + img_off;
+    const float2* __restrict__ csrc = p.coil ? p.coil + (int64_t)b * p.nimg + img_off : nullptr;
+    float2* __restrict__ dst = p.grid + (int64_t)(active ? line : 0) * K;
+    const float* __restrict__ sl = p.g.s[d - 1];
+    LayContig<K> lay{smem + lt * G::PITCH_C};
+    auto ld = [&](int i) -> float2 {
+        const int n = pad_map(i, NL, K);
+        if (zero_line || n < 0) return make_float2(0.f, 0.f);
+        float2 xv = __ldg(&src[n]);
+        if (csrc) xv = cmul(xv, __ldg(&csrc[n]));
+        return cscale(xv, so * __ldg(&sl[n]));
+    };
+    auto st = [&](int i, float2 v) { dst[i] = v; };
+    fft_line<K, false, false>(q0, active, lay, p.tw, ld, st);
+}
+
+template <int K>
+__global__ void __launch_bounds__(FftGeom<K>::TPL * Rad<K>::LC)
+fft_rows_crop_kernel(SigmaRowParams p) {
+    pdl_enter();
+    using G = FftGeom<K>;
+    constexpr int TPL = G::TPL, LC = Rad<K>::LC;
+    extern __shared__ float2 smem[];
+    const int lt = threadIdx.x / TPL, q0 = threadIdx.x % TPL;
+    const int line = blockIdx.x * LC + lt;
+    const bool active = line < p.nlines;
+    const int d = p.g.d, NL = p.g.N[d - 1];
+    // line -> (b, outer image coordinates) -> outer grid coordinates at the reversed index (-(n - N/2)) mod K
+    int r = active ? line : 0;
+    int64_t img_off = 0, imul = NL, cell_off = 0, cmul_ = K;
+    float so = 1.0f;
+    for (int a = d - 2; a >= 0; --a) {
+        const int n = r % p.g.N[a];
+        r /= p.g.N[a];
+        const int k = (p.g.N[a] / 2 - n) & (p.g.K[a] - 1);
+        so *= __ldg(&p.g.s[a][n]);
+        img_off += (int64_t)n * imul;
+        cell_off += (int64_t)k * cmul_;
+        imul *= p.g.N[a];
+        cmul_ *= p.g.K[a];
+    }
+    const int b = r;
+    const float2* __restrict__ src = p.grid + (int64_t)b * p.cells + cell_off;
+    float2* __restrict__ dst = p.img_out + (int64_t)b * p.nimg + img_off;
+    const float2* __restrict__ csrc = p.coil ? p.coil + (int64_t)b * p.nimg + img_off : nullptr;
+    const float* __restrict__ sl = p.g.s[d - 1];
+    LayContig<K> lay{smem + lt * G::PITCH_C};
+    auto ld = [&](int i) -> float2 { return src[i]; };
+    auto st = [&](int i, float2 v) {
+        const int n = (NL / 2 - i) & (K - 1);        // output i of the forward FFT is image sample n = (N/2 - i) mod K
+        if (n < NL) {
+            float2 o = cscale(v, so * __ldg(&sl[n]));
+            if (csrc) o = cmul(o, cconj(__ldg(&csrc[n])));
+            dst[n] = o;
+        }
+    };
+    fft_line<K, false, false>(q0, active, lay, p.tw, ld, st);
 }
 
 }  // namespace nufft

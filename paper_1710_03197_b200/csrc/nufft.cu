@@ -199,6 +199,10 @@ template <int K> static cudaError_t configure_fft() {
     e = cudaFuncSetAttribute(fft_cols_kernel<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols<K>());
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(fft_rows_full_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_rows_pad_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fft_rows_crop_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows<K>());
     return e;
 }
 
@@ -322,7 +326,7 @@ static RowPassParams row_params(nufft_plan_t p, int batch, const float2* img_in,
     return r;
 }
 
-static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int batch = 1);
+static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int batch = 1, bool do_rows = true);
 static PadGeom pad_geom(nufft_plan_t p) {
     PadGeom g{};
     g.d = p->d;
@@ -334,19 +338,46 @@ static PadGeom pad_geom(nufft_plan_t p) {
 }
 static int ew_blocks(int64_t n);
 
+// sigma != 2: contiguous-axis pass with S + zero-pad (forward) / crop + S^H (adjoint) fused (fft.cuh)
+template <int K> static void launch_rows_sigma(bool adj, const SigmaRowParams& sp, cudaStream_t st) {
+    constexpr int threads = FftGeom<K>::TPL * Rad<K>::LC;
+    const int blocks = (sp.nlines + Rad<K>::LC - 1) / Rad<K>::LC;
+    if (adj) launch_pdl(fft_rows_crop_kernel<K>, dim3(blocks), dim3(threads), smem_rows<K>(), st, sp);
+    else     launch_pdl(fft_rows_pad_kernel<K>, dim3(blocks), dim3(threads), smem_rows<K>(), st, sp);
+}
+static int dispatch_rows_sigma(nufft_plan_t p, bool adj, int batch, const float2* x_in, float2* x_out, float2* grid,
+                               const float2* coil, bool same_image, cudaStream_t st) {
+    SigmaRowParams sp{};
+    sp.g = pad_geom(p);
+    sp.img_in = x_in; sp.img_out = x_out; sp.grid = grid; sp.coil = coil;
+    sp.tw = p->d_tw[p->d - 1];
+    sp.cells = p->cells; sp.nimg = p->nimg; sp.same_image = same_image ? 1 : 0;
+    int64_t lines = batch;
+    for (int a = 0; a + 1 < p->d; ++a) lines *= adj ? p->N[a] : p->K[a];
+    sp.nlines = (int)lines;
+    switch (p->K[p->d - 1]) {
+        case 32: launch_rows_sigma<32>(adj, sp, st); break;
+        case 64: launch_rows_sigma<64>(adj, sp, st); break;
+        case 128: launch_rows_sigma<128>(adj, sp, st); break;
+        case 256: launch_rows_sigma<256>(adj, sp, st); break;
+        case 512: launch_rows_sigma<512>(adj, sp, st); break;
+        case 1024: launch_rows_sigma<1024>(adj, sp, st); break;
+        default: return NUFFT_EINVAL;
+    }
+    CU_TRY(cudaGetLastError());
+    p->launches++;
+    return NUFFT_OK;
+}
+
 // a1 + a2: grid = F S x  (coil != nullptr: grid_b = F S (c_b . x))
 static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* grid, const float2* coil,
                          bool same_image, cudaStream_t st) {
     const int d = p->d;
-    if (p->generic_sigma) {      // sigma != 2: pad kernel + unpruned FFT
-        {
-            ProfScope ps(p, "pad_scale", st);
-            pad_scale_kernel<<<dim3((unsigned)ew_blocks(p->cells), (unsigned)batch), 256, 0, st>>>(pad_geom(p), x, coil, grid, p->cells, p->nimg, same_image ? 1 : 0);
-            CU_TRY(cudaGetLastError());
-            p->launches++;
-        }
+    if (p->generic_sigma) {      // sigma != 2: S + zero-pad fused into the unpruned contiguous-axis pass, then the strided passes
+        { ProfScope ps(p, "fft_rows_fwd", st); NU_TRY(dispatch_rows_sigma(p, false, batch, x, nullptr, grid, coil, same_image, st)); }
+        if (d == 1) return NUFFT_OK;
         ProfScope ps(p, "fft_full_fwd", st);
-        return fft_full_inplace(p, grid, st, batch);
+        return fft_full_inplace(p, grid, st, batch, false);
     }
     RowPassParams r = row_params(p, batch, x, nullptr, grid, coil, same_image);
     { ProfScope ps(p, "fft_rows_fwd", st); NU_TRY(dispatch_rows(p->K[d - 1], false, r, st)); }
@@ -381,13 +412,10 @@ static int run_scale_fft(nufft_plan_t p, int batch, const float2* x, float2* gri
 // a5 + a6: x = S^H F^H grid  (grid destroyed; coil != nullptr: x_b = conj(c_b) . S^H F^H grid_b)
 static int run_fft_scale(nufft_plan_t p, int batch, float2* grid, float2* x, const float2* coil, cudaStream_t st) {
     const int d = p->d;
-    if (p->generic_sigma) {      // sigma != 2: unpruned FFT, then crop at the reversed index (= F^H) + S^H
-        { ProfScope ps(p, "fft_full_adj", st); NU_TRY(fft_full_inplace(p, grid, st, batch)); }
-        ProfScope ps(p, "crop_scale", st);
-        crop_scale_kernel<<<dim3((unsigned)ew_blocks(p->nimg), (unsigned)batch), 256, 0, st>>>(pad_geom(p), grid, coil, x, p->cells, p->nimg);
-        CU_TRY(cudaGetLastError());
-        p->launches++;
-        return NUFFT_OK;
+    if (p->generic_sigma) {      // sigma != 2: unpruned strided passes, then the contiguous-axis pass on the kept lines only with
+        if (d > 1) { ProfScope ps(p, "fft_full_adj", st); NU_TRY(fft_full_inplace(p, grid, st, batch, false)); }   // crop (reversed index = F^H) + S^H fused
+        ProfScope ps(p, "fft_rows_adj", st);
+        return dispatch_rows_sigma(p, true, batch, nullptr, x, grid, coil, false, st);
     }
     if (d == 1) {
         // the Toeplitz spectrum multiply normally rides on the first adjoint column pass; 1-D has none
@@ -1694,10 +1722,10 @@ template <int K> static void launch_cols_full(const ColPassParams& c, cudaStream
     }
 
 // in-place unpruned forward FFT of a planar K^d array (used once per plan for the Toeplitz spectrum)
-static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int batch) {
+static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int batch, bool do_rows) {
     const int d = p->d;
     const int64_t cells = p->cells;
-    {
+    if (do_rows) {
         const int Kl = p->K[d - 1];
         const int nlines = (int)(cells / Kl) * batch;
 #define CALL_ROWS(KK) launch_rows_full<KK>(data, p->d_tw[d - 1], nlines, st)
@@ -1719,7 +1747,7 @@ static int fft_full_inplace(nufft_plan_t p, float2* data, cudaStream_t st, int b
 #undef CALL_COLS
     }
     CU_TRY(cudaGetLastError());
-    p->launches += d;
+    p->launches += do_rows ? d : d - 1;
     return NUFFT_OK;
 }
 
