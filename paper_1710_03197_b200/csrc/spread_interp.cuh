@@ -269,20 +269,33 @@ gridding_tiled_2d_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* 
     const WorkItem wi = items[item];
     int o[3];
     unpack_k0(wi.origin, o);
+    const float2* __restrict__ yb = y + (int64_t)b * g.M;
+    // plan data of chunk c + 2 and y of chunk c + 1 travel through registers while chunk c is applied: a warp walks its item
+    // alone, so an unhidden load is two DRAM round trips per 32 samples (the whole batch-1 adjoint was paced by them)
+    struct Pre { uint32_t kp; float d0, d1; int m; float2 yv; };
+    auto fetch = [&](int si, Pre& f) {
+        f.m = -1; f.kp = 0; f.d0 = f.d1 = 0.f; f.yv = make_float2(0.f, 0.f);
+        if (si < wi.s_end) {
+            f.kp = __ldg(&s.kpack[si]); f.d0 = __ldg(&s.delta[si]); f.d1 = __ldg(&s.delta[g.M + si]); f.m = __ldg(&s.perm[si]);
+        }
+    };
+    Pre cur, nxt;
+    fetch(wi.s_begin + lane, cur);
+    if (cur.m >= 0) cur.yv = __ldg(&yb[cur.m]);
+    fetch(wi.s_begin + 32 + lane, nxt);
     for (int i = lane; i < tg.tile_cells / 2; i += 32) reinterpret_cast<float4*>(tile)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncwarp();
-    const float2* __restrict__ yb = y + (int64_t)b * g.M;
     for (int s0 = wi.s_begin; s0 < wi.s_end; s0 += 32) {
-        const int si = s0 + lane;
         const int cnt = min(32, wi.s_end - s0);
-        if (si < wi.s_end) {
+        if (cur.m >= 0) {
             int k0[3];
-            unpack_k0(__ldg(&s.kpack[si]), k0);
-            const float d0 = __ldg(&s.delta[si]), d1 = __ldg(&s.delta[g.M + si]);
-            const float2 yv = __ldg(&yb[__ldg(&s.perm[si])]);
-            stage_sample_2d(P, rowrec, colrec, lane, (k0[0] - o[0]) & (g.K[0] - 1), (k0[1] - o[1]) & (g.K[1] - 1), d0, d1,
-                            yv, tg.pitch, 0);
+            unpack_k0(cur.kp, k0);
+            stage_sample_2d(P, rowrec, colrec, lane, (k0[0] - o[0]) & (g.K[0] - 1), (k0[1] - o[1]) & (g.K[1] - 1), cur.d0, cur.d1,
+                            cur.yv, tg.pitch, 0);
         }
+        cur = nxt;
+        if (cur.m >= 0) cur.yv = __ldg(&yb[cur.m]);
+        fetch(s0 + 64 + lane, nxt);
         __syncwarp();
         apply_staged(tile, rowrec, colrec, cnt, lane);
         __syncwarp();
