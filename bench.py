@@ -832,7 +832,7 @@ def extra_legs(nb, torch, peak, args):
                      "adjoint_ms": time_calls(lambda: pv.adjoint(yv, xov), 10, flush)}
         pv.destroy()
     var["note"] = ("Kd=512^2, radial 256x512; min-max runs the same kernels as Kaiser-Bessel; J != 6 runs the direct V / atomic "
-                   "V^H kernels; sigma != 2 (Nd=320^2) runs pad / crop kernels around the unpruned FFT")
+                   "V^H kernels; sigma != 2 (Nd=320^2) runs the unpruned FFT with pad / crop fused into its contiguous-axis pass")
     out["variants_cfg2_batch1"] = var
     # cuFFT reference point for F alone (never linked into the product): full 512^2 FFT of 64 grids via torch.fft
     gref = torch.randn(64, 512, 512, dtype=torch.complex64, device="cuda")
