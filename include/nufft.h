@@ -37,9 +37,9 @@
  *     1 <= batch <= max_batch.  Kd == 2 Nd (the paper's and every BASELINE config's ratio) runs the pruned, fused FFT passes;
  *     any other ratio runs S + zero-pad and crop + S^H as separate kernels around the unpruned FFT, planar layout, and has
  *     no Toeplitz form (nufft_toeplitz_build -> NUFFT_EINVAL); everything else works unchanged.  Jd == 6 runs the tiled / batch-interleaved kernels;
- *     every other width runs the direct V (one thread per sample, prod(J) gathered loads) and the atomic V^H (one
- *     vector atomic per stencil point into a zeroed grid), planar layout at every batch size, adjoint_mode = 1
- *     refused; all transforms, solvers, density weights and the Toeplitz form work on such plans.
+ *     every other width runs the direct V (one thread per sample, prod(J) gathered loads) and, in 2-D, a tiled V^H with the
+ *     lane map derived from J (warp-private shared tiles, one TMA reduce-add flush per work item; 1-D / 3-D: one vector
+ *     atomic per stencil point into a zeroed grid), planar layout at every batch size, adjoint_mode = 1 refused; all transforms, solvers, density weights and the Toeplitz form work on such plans.
  *     Anything else -> NUFFT_EINVAL (there is no CPU fallback).
  */
 #ifndef NUFFT_B200_H

@@ -218,6 +218,9 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(interp_tiled_2d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_2d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+#define NU_TILED_J_CFG(JJ) if ((e = cudaFuncSetAttribute(gridding_tiled_2d_j_kernel<JJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
+    NU_TILED_J_CFG(2) NU_TILED_J_CFG(3) NU_TILED_J_CFG(4) NU_TILED_J_CFG(5) NU_TILED_J_CFG(6) NU_TILED_J_CFG(7) NU_TILED_J_CFG(8)
+#undef NU_TILED_J_CFG
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(interp_tiled_3d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kInterp3dSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_il_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<1>::BYTES)) != cudaSuccess) return e;
@@ -584,6 +587,22 @@ static int run_gridding(nufft_plan_t p, int batch, const float2* y, float2* grid
     const bool det = p->opts.adjoint_mode == 1;
     if (p->M == 0 || p->n_items == 0) {
         CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st));
+        return NUFFT_OK;
+    }
+    if (p->generic_j && p->d == 2 && p->opts.adjoint_mode == 0 && p->K[1] >= p->tg.pitch) {
+        // any width, 2-D: warp-private shared tiles + one TMA reduce-add flush per work item (gridding_tiled_2d_j_kernel)
+        { ProfScope pz(p, "grid_zero", st); CU_TRY(cudaMemsetAsync(grid, 0, (size_t)batch * p->cells * sizeof(float2), st)); }
+        ProfScope ps(p, "gridding", st);
+        const dim3 blocks((unsigned)((p->n_items + kGrid2dWarps - 1) / kGrid2dWarps), (unsigned)batch);
+#define NU_TILED_J(JJ) case JJ: gridding_tiled_2d_j_kernel<JJ><<<blocks, kGrid2dWarps * 32, (size_t)kGrid2dWarps * Tile2dJ<JJ>::warp_bytes(p->tg.tile_cells), st>>>( \
+            sample_data(p), grid_geom(p), p->tg, p->d_items, p->n_items, y, grid, p->polyg); break;
+        switch (p->J) {
+            NU_TILED_J(2) NU_TILED_J(3) NU_TILED_J(4) NU_TILED_J(5) NU_TILED_J(6) NU_TILED_J(7) NU_TILED_J(8)
+            default: return NUFFT_EINVAL;
+        }
+#undef NU_TILED_J
+        CU_TRY(cudaGetLastError());
+        p->launches++;
         return NUFFT_OK;
     }
     if (p->generic_j) {
@@ -1077,10 +1096,12 @@ static int plan_build(nufft_plan_t p, const double* om) {
     p->n_tiles = (int64_t)p->ntile[0] * p->ntile[1] * p->ntile[2];
     {
         TileGeom& tg = p->tg;
-        for (int a = 0; a < 3; ++a) { tg.T[a] = p->tile[a]; tg.P[a] = (a < d) ? p->tile[a] + kJ - 1 : 1; }
+        // halo of J - 1 cells: the plan's own width on 2-D generic-width plans (gridding_tiled_2d_j_kernel), kJ otherwise
+        const int Jt = (p->generic_j && d == 2) ? p->J : kJ;
+        for (int a = 0; a < 3; ++a) { tg.T[a] = p->tile[a]; tg.P[a] = (a < d) ? p->tile[a] + Jt - 1 : 1; }
         // row pitch: >= T + J (8-cell aligned windows reach one cell past the halo) and = 8 (mod 16) cells, so that the
         // two stencil rows of an 8-lane shared-memory phase fall into different 64-byte bank halves
-        int pitch = p->tile[d - 1] + kJ;
+        int pitch = p->tile[d - 1] + Jt;
         pitch += ((8 - pitch % 16) + 16) % 16;
         tg.pitch = pitch;
         tg.plane = (d == 3) ? tg.P[1] * pitch : 0;

@@ -243,6 +243,106 @@ __device__ __forceinline__ void flush_tile(const float2* tile, const TileGeom& t
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Tiled V^H for any kernel width J in [kJmin, kJmax], 2-D (round 2; SURVEY 8(f)-4 "other Jd").  Same scheme as
+// gridding_tiled_2d_kernel -- warp-private padded tile in shared memory, 32 samples staged at a time, one 16-byte
+// read-modify-write per lane and sample, one TMA reduce-add flush per work item -- with the lane map derived from J:
+// NP = (J + 2) / 2 cell pairs cover the (J + 1)-cell window aligned to an even column; a lane handles RPL stencil rows
+// (J = 8: 5 pairs x 4 lane rows = 20 lanes, two rows each; J <= 7: one row per lane).  Replaces one global red.add per stencil point.
+// ------------------------------------------------------------------------------------------------------------
+template <int J> struct Tile2dJ {
+    static constexpr int NP = (J + 2) / 2;
+    static constexpr int RPL = (J + (32 / NP) - 1) / (32 / NP);      // stencil rows per lane (J = 8: 2, else 1)
+    static constexpr int RL = (J + RPL - 1) / RPL;                  // lane rows: lane (rl, q) handles rows rl, rl + RL, ...
+    static constexpr int ROWSLOTS = J | 1;            // float4 slots per sample (odd: 8-lane phases conflict-free)
+    static constexpr int COLSLOTS = NP | 1;           // float2 slots per sample
+    static constexpr int STAGE_BYTES = 32 * (ROWSLOTS * 16 + COLSLOTS * 8);
+    __host__ __device__ static constexpr int warp_bytes(int tile_cells) { return ((tile_cells * 8 + STAGE_BYTES + 127) / 128) * 128; }
+};
+
+template <int J>
+__global__ void __launch_bounds__(256)
+gridding_tiled_2d_j_kernel(SampleData s, GridGeom g, TileGeom tg, const WorkItem* __restrict__ items, int n_items,
+                           const float2* __restrict__ y, float2* __restrict__ grid, KernelPolyG P) {
+    pdl_enter();
+    using C = Tile2dJ<J>;
+    extern __shared__ float4 smem4[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int item = blockIdx.x * nw + warp;
+    if (item >= n_items) return;
+    const int b = blockIdx.y;
+    float2* tile = reinterpret_cast<float2*>(smem4 + (size_t)warp * (C::warp_bytes(tg.tile_cells) / 16));
+    float4* rowrec = reinterpret_cast<float4*>(tile + tg.tile_cells);
+    float2* colrec = reinterpret_cast<float2*>(rowrec + 32 * C::ROWSLOTS);
+    const WorkItem wi = items[item];
+    int o[3];
+    unpack_k0(wi.origin, o);
+    for (int i = lane; i < tg.tile_cells / 2; i += 32) reinterpret_cast<float4*>(tile)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+    const float2* __restrict__ yb = y + (int64_t)b * g.M;
+    for (int s0 = wi.s_begin; s0 < wi.s_end; s0 += 32) {
+        const int si = s0 + lane;
+        const int cnt = min(32, wi.s_end - s0);
+        if (si < wi.s_end) {
+            int k0[3];
+            unpack_k0(__ldg(&s.kpack[si]), k0);
+            float w0[J], w1[J];
+            kb_weights_j<J>(P, 0, __ldg(&s.delta[si]), w0);
+            kb_weights_j<J>(P, 1, __ldg(&s.delta[g.M + si]), w1);
+            const float2 yv = __ldg(&yb[__ldg(&s.perm[si])]);
+            const int c0 = (k0[0] - o[0]) & (g.K[0] - 1), c1 = (k0[1] - o[1]) & (g.K[1] - 1);
+            const int par = c1 & 1, base = c0 * tg.pitch + (c1 - par);
+#pragma unroll
+            for (int r = 0; r < J; ++r)
+                rowrec[lane * C::ROWSLOTS + r] = make_float4(w0[r] * yv.x, w0[r] * yv.y, __int_as_float(base + r * tg.pitch), 0.f);
+#pragma unroll
+            for (int q = 0; q < C::NP; ++q) {       // pair q = columns 2 q, 2 q + 1 of the aligned window = weights 2 q - par, + 1
+                const int ja = 2 * q - par, jb = ja + 1;
+                float wa = 0.f, wb = 0.f;
+#pragma unroll
+                for (int j = 0; j < J; ++j) { wa = (j == ja) ? w1[j] : wa; wb = (j == jb) ? w1[j] : wb; }
+                colrec[lane * C::COLSLOTS + q] = make_float2(wa, wb);
+            }
+        }
+        __syncwarp();
+        {
+            const int rl = lane / C::NP, q = lane % C::NP;
+            if (lane < C::RL * C::NP) {
+                for (int t = 0; t < cnt; ++t) {
+                    const float2 cc = colrec[t * C::COLSLOTS + q];
+#pragma unroll
+                    for (int i = 0; i < C::RPL; ++i) {
+                        const int r = rl + i * C::RL;
+                        if (r < J) {
+                            const float4 rr = rowrec[t * C::ROWSLOTS + r];
+                            float4* cell = reinterpret_cast<float4*>(tile + __float_as_int(rr.z) + 2 * q);
+                            float4 a = *cell;
+                            a.x = fmaf(rr.x, cc.x, a.x);
+                            a.y = fmaf(rr.y, cc.x, a.y);
+                            a.z = fmaf(rr.x, cc.y, a.z);
+                            a.w = fmaf(rr.y, cc.y, a.w);
+                            *cell = a;
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    }
+    // flush by the TMA engine: one bulk f32 reduce-add per padded row (split at the seam of axis 1)
+    fence_proxy_async_smem();
+    float2* __restrict__ Gb = grid + (int64_t)b * g.cells;
+    for (int row = lane; row < tg.P[0]; row += 32) {
+        const int gx = (o[0] + row) & (g.K[0] - 1), gz = o[1] & (g.K[1] - 1);
+        float2* dst = Gb + (int64_t)gx * g.K[1];
+        const float2* src = tile + row * tg.pitch;
+        const int first = min(tg.pitch, g.K[1] - gz);
+        bulk_s2g_add_f32(dst + gz, src, (uint32_t)first * 8);
+        if (first < tg.pitch) bulk_s2g_add_f32(dst, src + first, (uint32_t)(tg.pitch - first) * 8);
+    }
+    bulk_commit_and_wait_read();
+}
+
 // grid = 0 as a kernel (not a memset node), so that it takes part in the programmatic-dependent-launch chain of a transform
 __global__ void __launch_bounds__(256) grid_zero_kernel(float4* __restrict__ g4, int64_t n4) {
     pdl_enter();
