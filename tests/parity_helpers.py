@@ -34,3 +34,30 @@ def check_density_weights(wg, wo, om, Nd, Kd, Jd, niter, tol):
     floor = max(rel(noisy_density_weights(om, Nd, Kd, Jd, niter, 2e-7, seed=s), wo) for s in (0, 1, 2))
     assert np.all(np.isfinite(wg)) and err < max(tol, 3.0 * floor), (err, floor)
     return err, floor
+
+
+def coil_ops_threaded(c128, om, Nd, Kd, Jd, with_forward=False):
+    """A_multi^H A_multi and A_multi^H of the oracle, the per-coil transforms (oracle/nufft_oracle.py forward / adjoint,
+    unchanged) evaluated on a thread pool: same arithmetic, same fixed summation order over the coils."""
+    import concurrent.futures as cf
+    import os
+    pool = cf.ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1))
+
+    def AHy(y):
+        parts = list(pool.map(lambda i: np.conj(c128[i]) * orc.adjoint(y[i], om, Nd, Kd, Jd), range(len(c128))))
+        out = np.zeros(tuple(Nd), dtype=np.complex128)
+        for q in parts:
+            out += q
+        return out
+
+    def AHA(z):
+        parts = list(pool.map(lambda i: np.conj(c128[i]) * orc.adjoint(orc.forward(c128[i] * z, om, Nd, Kd, Jd), om, Nd, Kd, Jd),
+                              range(len(c128))))
+        out = np.zeros(tuple(Nd), dtype=np.complex128)
+        for q in parts:
+            out += q
+        return out
+
+    def A(z):
+        return np.stack(list(pool.map(lambda i: orc.forward(c128[i] * z, om, Nd, Kd, Jd), range(len(c128)))))
+    return (AHA, AHy, A) if with_forward else (AHA, AHy)

@@ -174,6 +174,27 @@ def test_l1tv_lad(ncoil):
     p.destroy()
 
 
+def test_l1tv_lad_config5_r17_iteration_counts_128():
+    """L1TV-LAD (eqs. 23-33) at reading R17's full schedule (n_outer = 4, n_inner = 5, n_cg = 3, mu = 1, lambda = 0.02) on the
+    scaled config 5 (128^2, 8 coils, radial 64 x 256), and one outer group of it at FULL size (256^2, 32 coils): <= 1e-4."""
+    from parity_helpers import coil_ops_threaded
+    for scale, sched in ((2, (4, 5, 3)), (1, (1, 5, 3))):
+        cfg = wl.config(4, scale=scale)
+        Nd, Kd, Jd, om = cfg["Nd"], cfg["Kd"], cfg["Jd"], cfg["om"]
+        nc = cfg["ncoil"]
+        c = wl.coil_maps(nc, Nd)
+        c128 = c.astype(np.complex128)
+        AHA, AHy, A = coil_ops_threaded(c128, om, Nd, Kd, Jd, with_forward=True)
+        y = A(wl.phantom(Nd).astype(np.complex128))
+        y = (y + wl.noise_like(y)).astype(np.complex64)
+        p = make_plan(cfg, max_batch=nc)
+        p.set_coils(dev(c))
+        xo = nxt.l1tv_lad(AHA, AHy(y.astype(np.complex128)), 1.0, 0.02, *sched)
+        xg = host(p.solve_l1tv_lad(dev(y), 1.0, 0.02, *sched, use_coils=True))
+        assert rel(xg, xo) < 1e-4, (scale, rel(xg, xo))
+        p.destroy()
+
+
 @pytest.mark.parametrize("ci,scale", [(0, 1), (1, 4), (3, 8)])
 def test_cg_kspace(ci, scale):
     """The paper's k-space CG (eqs. 8-11): iterates 1 and 4 against the oracle (<= 1e-4; V^H V is singular on the

@@ -10,6 +10,8 @@ import workloads as wl
 from oracle import nufft_oracle as orc
 from oracle import solvers_oracle as sol
 
+from parity_helpers import coil_ops_threaded as _coil_ops_threaded
+
 pytestmark = pytest.mark.gpu
 
 TOL = 2e-5
@@ -594,33 +596,6 @@ def test_l1tv_ols_16_coils_interleaved_path():
     xg = p.solve_l1tv_ols(dev(y), 1.0, 0.02, 1, 2, 2, use_coils=True)
     assert rel(host(xg), xo) < 1e-4
     p.destroy()
-
-
-def _coil_ops_threaded(c128, om, Nd, Kd, Jd, with_forward=False):
-    """A_multi^H A_multi and A_multi^H of the oracle, the per-coil transforms (oracle/nufft_oracle.py forward / adjoint,
-    unchanged) evaluated on a thread pool: same arithmetic, same fixed summation order over the coils."""
-    import concurrent.futures as cf
-    import os
-    pool = cf.ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1))
-
-    def AHy(y):
-        parts = list(pool.map(lambda i: np.conj(c128[i]) * orc.adjoint(y[i], om, Nd, Kd, Jd), range(len(c128))))
-        out = np.zeros(tuple(Nd), dtype=np.complex128)
-        for q in parts:
-            out += q
-        return out
-
-    def AHA(z):
-        parts = list(pool.map(lambda i: np.conj(c128[i]) * orc.adjoint(orc.forward(c128[i] * z, om, Nd, Kd, Jd), om, Nd, Kd, Jd),
-                              range(len(c128))))
-        out = np.zeros(tuple(Nd), dtype=np.complex128)
-        for q in parts:
-            out += q
-        return out
-
-    def A(z):
-        return np.stack(list(pool.map(lambda i: orc.forward(c128[i] * z, om, Nd, Kd, Jd), range(len(c128)))))
-    return (AHA, AHy, A) if with_forward else (AHA, AHy)
 
 
 def test_l1tv_ols_config5_r17_iteration_counts_128():
