@@ -35,7 +35,7 @@
  *     refused); Jd[a] the same on every axis, 2 <= Jd <= 8 (odd widths included);
  *     Kd[a] in {32,64,128,256,512,1024}; Nd[a] even, 2 <= Nd[a] < Kd[a] (the ratio Kd[a]/Nd[a] may differ per axis);
  *     1 <= batch <= max_batch.  Kd == 2 Nd (the paper's and every BASELINE config's ratio) runs the pruned, fused FFT passes;
- *     any other ratio runs S + zero-pad and crop + S^H as separate kernels around the unpruned FFT, planar layout, and has
+ *     any other ratio runs the unpruned FFT with S + zero-pad and crop + S^H fused into its contiguous-axis pass, planar layout, and has
  *     no Toeplitz form (nufft_toeplitz_build -> NUFFT_EINVAL); everything else works unchanged.  Jd == 6 runs the tiled / batch-interleaved kernels;
  *     every other width runs the direct V (one thread per sample, prod(J) gathered loads) and, in 2-D, a tiled V^H with the
  *     lane map derived from J (warp-private shared tiles, one TMA reduce-add flush per work item; 1-D / 3-D: one vector
