@@ -60,7 +60,8 @@ typedef enum {
     NUFFT_ENOMEM  = -2,   /* host or device allocation failed                                             */
     NUFFT_ECUDA   = -3,   /* a CUDA runtime call failed; nufft_last_cuda_error() gives the cudaError_t    */
     NUFFT_ERANGE  = -4,   /* om contains a non-finite value                                               */
-    NUFFT_ESTATE  = -5    /* call needs something not set (e.g. coil maps)                                */
+    NUFFT_ESTATE  = -5,   /* call needs something not set (e.g. coil maps)                                */
+    NUFFT_ETOOBIG = -6    /* nufft_adjoint_noalloc: prod(Kd) exceeds NUFFT_NOALLOC_MAX_CELLS                 */
 } nufft_status;
 
 /* Options.  Zero-initialise or call nufft_default_opts first. */
@@ -132,6 +133,24 @@ int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64 *y, nufft_c64 *x, v
 
 /* x_out[b] = A^H A x_in[b], the intermediate samples stay in the plan's workspace.   eq.(5), R8 */
 int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64 *x_in, nufft_c64 *x_out, void *stream);
+
+/* x = A^H y for ONE image (eq.(2), the same kernels as nufft_adjoint at batch 1 on the planar path) for callers that
+ * cannot tolerate an allocation: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating library routine: the oversampled grid that V^H
+ * accumulates into and F^H transforms (the scratch of a5 / a4) lives in a file-scope `static __device__` array of the
+ * library, NUFFT_NOALLOC_MAX_CELLS complex64 cells = 2 MiB, which every GPU that loads the library holds until the
+ * process exits (its device address is taken once per device, at plan creation, with cudaGetSymbolAddress).
+ *   y: device [M];  x: device [prod Nd], caller-owned.  Asynchronous on `stream` like nufft_adjoint.
+ *   prod(Kd) > NUFFT_NOALLOC_MAX_CELLS -> NUFFT_ETOOBIG (e.g. 512 x 512 and 64^3 grids fit, 1024^2 and 256^3 do not);
+ *   plans with adjoint_mode = 1 (their slabs are allocated on first use) and calls made while nufft_profile_enable is
+ *   on (events are created) -> NUFFT_EINVAL;  the static array could not be located at plan creation -> NUFFT_ESTATE.
+ * The array is SHARED by every plan, stream and thread of the process on that GPU and keeps the last call's contents:
+ * the call zero-fills the part it uses before accumulating (the same grid_zero pass as nufft_adjoint), so a call never
+ * sees stale data, but two calls that overlap on the GPU (different streams, or different host threads on unordered
+ * streams) race on it -- order them on one stream or with events.  The result is that of nufft_adjoint up to the
+ * summation order of the tile flushes (adjoint_mode = 0: reproducible to rounding only). */
+#define NUFFT_NOALLOC_MAX_CELLS 262144
+int nufft_adjoint_noalloc(nufft_plan_t p, const nufft_c64 *y, nufft_c64 *x, void *stream);
 
 /* The same three transforms on HOST buffers (bench.py's end-to-end leg).  x / y are host pointers, read / written
  * asynchronously: they must stay valid until `stream` has passed this call, and should be page-locked (pinned) --

@@ -15,7 +15,7 @@ _PTR = _c.c_void_p
 _I64P = _c.POINTER(_c.c_int64)
 
 EXPORTED_SYMBOLS = [
-    "nufft_default_opts", "nufft_plan", "nufft_forward", "nufft_adjoint", "nufft_selfadjoint",
+    "nufft_default_opts", "nufft_plan", "nufft_forward", "nufft_adjoint", "nufft_selfadjoint", "nufft_adjoint_noalloc",
     "nufft_forward_host", "nufft_adjoint_host", "nufft_selfadjoint_host", "nufft_host_input_ready",
     "nufft_density_weights", "nufft_adjoint_dcf", "nufft_toeplitz_build", "nufft_toeplitz_enable",
     "nufft_selfadjoint_toeplitz", "nufft_selfadjoint_toeplitz_coils", "nufft_solve_l1tv_lad", "nufft_solve_cg_kspace",
@@ -62,6 +62,7 @@ def lib():
                  "nufft_selfadjoint_host", "nufft_stage_scale_fft",
                  "nufft_stage_interp", "nufft_stage_gridding", "nufft_stage_fft_scale"):
         getattr(L, name).argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR]
+    L.nufft_adjoint_noalloc.argtypes = [_PLAN, _PTR, _PTR, _PTR]
     L.nufft_host_input_ready.argtypes = [_PLAN, _c.c_int]
     L.nufft_density_weights.argtypes = [_PLAN, _c.c_int, _PTR, _PTR]
     L.nufft_adjoint_dcf.argtypes = [_PLAN, _c.c_int, _PTR, _PTR, _PTR, _PTR]
@@ -212,6 +213,12 @@ class NufftPlan:
         x = self._new(b, *self.Nd) if x is None else x
         _check(lib().nufft_adjoint(self._h, b, _dev(y, "y") if self.M else None, _dev(x, "x", b * self.nimg), _stream()),
                "nufft_adjoint")
+        return x
+
+    def adjoint_noalloc(self, y, x):
+        """nufft_adjoint_noalloc: one image, caller-owned output, workspace in the library's static device array."""
+        _check(lib().nufft_adjoint_noalloc(self._h, _dev(y, "y", self.M) if self.M else None, _dev(x, "x", self.nimg), _stream()),
+               "nufft_adjoint_noalloc")
         return x
 
     def selfadjoint(self, x, out=None):

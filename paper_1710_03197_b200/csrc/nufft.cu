@@ -110,6 +110,7 @@ struct nufft_plan_s {
     bool il_coherent = false;
     IlItem* d_il_items = nullptr;
     int n_il_items = 0;
+    float2* noalloc_grid = nullptr;     // device address of g_noalloc_grid on the plan's device (nufft_adjoint_noalloc), or null
     float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
     // "next" rows: density compensation and Toeplitz A^H A
     std::vector<double> om_host;    // copy of the trajectory (the Toeplitz build plans a second, 2N transform)
@@ -1255,6 +1256,25 @@ static int plan_build(nufft_plan_t p, const double* om) {
     return NUFFT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// nufft_adjoint_noalloc: the workspace grid as a file-scope device array (include/nufft.h).  In host code the NAME of a
+// __device__ variable is a host-side stand-in, not a device address: the address a kernel can use comes from
+// cudaGetSymbolAddress, asked once per device with that device current (every device that loads this module holds its
+// own copy of the array).
+// ------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) float2 g_noalloc_grid[NUFFT_NOALLOC_MAX_CELLS];
+// device ordinal -> address (null: the lookup failed; the entry point then returns NUFFT_ESTATE).  Called under the
+// per-device configuration mutex of nufft_plan.
+static float2* noalloc_grid_of_device(int dev) {
+    static std::vector<std::pair<int, float2*>> known;
+    for (const auto& k : known) if (k.first == dev) return k.second;
+    float2* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_grid);
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); ptr = nullptr; }
+    known.emplace_back(dev, ptr);
+    return ptr;
+}
+
 extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int* Jd, int64_t M, const double* om,
                           int max_batch, const nufft_opts* opts, nufft_plan_t* out) {
     if (out) *out = nullptr;
@@ -1286,9 +1306,16 @@ extern "C" int nufft_plan(int d, const int64_t* Nd, const int64_t* Kd, const int
             done.push_back(dev);
         }
     }
+    float2* noalloc_grid = nullptr;
+    {
+        static std::mutex mu_na;
+        std::lock_guard<std::mutex> lk(mu_na);
+        noalloc_grid = noalloc_grid_of_device(dev);
+    }
     nufft_plan_t p = new (std::nothrow) nufft_plan_s();
     if (!p) return NUFFT_ENOMEM;
     p->device = dev;
+    p->noalloc_grid = noalloc_grid;
     p->d = d;
     p->M = M;
     p->max_batch = max_batch;
@@ -1535,6 +1562,18 @@ extern "C" int nufft_adjoint(nufft_plan_t p, int batch, const nufft_c64* y, nuff
     if (bad_batch(p, batch) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     return run_graphed(p, 1, batch, y, x, st, [&]() { return adjoint_impl(p, batch, y, x, st); });
+}
+// x = A^H y, one image, with the workspace grid in the library's static device array: no allocation of any kind on this path
+// (run_gridding zero-fills the cells it accumulates into; adjoint_mode = 1 would allocate its slabs on first use and the
+// profiler creates events, so both are refused).
+extern "C" int nufft_adjoint_noalloc(nufft_plan_t p, const nufft_c64* y, nufft_c64* x, void* stream) {
+    if (bad_batch(p, 1) || !x || (!y && p->M > 0)) return NUFFT_EINVAL;
+    if (p->cells > (int64_t)NUFFT_NOALLOC_MAX_CELLS) return NUFFT_ETOOBIG;
+    if (p->opts.adjoint_mode == 1 || p->prof_on) return NUFFT_EINVAL;
+    if (!p->noalloc_grid) return NUFFT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    NU_TRY(run_gridding(p, 1, (const float2*)y, p->noalloc_grid, st));
+    return run_fft_scale(p, 1, p->noalloc_grid, (float2*)x, nullptr, st);
 }
 extern "C" int nufft_selfadjoint(nufft_plan_t p, int batch, const nufft_c64* x_in, nufft_c64* x_out, void* stream) {
     if (bad_batch(p, batch) || !x_in || !x_out) return NUFFT_EINVAL;
@@ -2167,6 +2206,7 @@ extern "C" const char* nufft_strerror(int code) {
         case NUFFT_ECUDA: return "CUDA runtime error (see nufft_last_cuda_error)";
         case NUFFT_ERANGE: return "non-finite sample location";
         case NUFFT_ESTATE: return "missing state (coil maps not set)";
+        case NUFFT_ETOOBIG: return "oversampled grid larger than the static scratch of nufft_adjoint_noalloc (NUFFT_NOALLOC_MAX_CELLS cells)";
     }
     return "unknown error";
 }
