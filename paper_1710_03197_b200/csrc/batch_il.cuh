@@ -170,6 +170,11 @@ struct IlPlan {
     const float* wv;          // coef_mode = 1: zero-padded weights [M][24] (w0 padded[10], 2 pad, w1 padded[10], 2 pad) in V order, else null
     const float* wv_c;        // ... in the caller's order
     const int32_t* v2h;       // V-order position -> V^H-order position
+    const uint32_t* kpack_t;  // TILE order (interp_il_tile_kernel): stencil base index per axis
+    const float* delta_t;     // tile order [2][M]
+    const uint32_t* gbase_t;  // tile order: window base relative to the tile origin (row | col << 5) | shape << 10
+    const float* wv_t;        // coef_mode = 1: weights [M][12] (w0[6], w1[6]) in tile order, else null
+    const int32_t* t2h;       // tile-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
     const float* wtab;        // V^H order: [M][kTabW] = w0[6], k0_0 (int bits), pad, w1 part A[8], w1 part B[8] (float64-built)
     const int32_t* rowptr;    // [(band * 2 + class) * K0 + row]: first V^H-order sample of (band, class, row); + 1 entry
@@ -411,6 +416,180 @@ interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, f
             const int l = warp * (kIL / kIwWarps) + li, b = grp * kIL + l;
             if (b >= batch) continue;
             for (int tt = lane; tt < tot; tt += 32) y_out[(int64_t)b * g.M + s0 + tt] = otile[tt][l];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a3 with register windows fed from a SHARED tile (round 2, the sorted walk of A^H A and of the incoherent trajectories).
+// profiles/r02a: interp_il_win_kernel loads every window from L2 (16 KB per group and warp, L1 hit rate 3 %) and sits at
+// ~10 TB/s of L2 -> SM traffic.  Here the CTA = one work item (tile of T x T stencil base cells, <= NW * 32 of its samples)
+// x one image group: the padded (T+5)^2 cells x 32 images tile is staged ONCE by the copy engine (one tensor-map copy, SASS
+// UTMALDG; tiles on the periodic seam: one bulk copy per row segment) while the warps evaluate their samples' weights;
+// the windows of the groups are then read from shared memory (conflict-free 256-B rows): L2 -> SM traffic is
+// ((T+5)/T)^2 x the grid instead of 11 cells per sample.  Two CTAs per SM: one loads while the other computes.
+// Every sample jumps, warp-uniformly, to the code variant of its support offset inside the window: exactly 36 + 6 packed
+// FMAs per sample instead of the 72 zero-padded ones of interp_il_win_kernel (measured: the padded form is FMA-pipe bound
+// here once the loads come from shared memory).  Output rows y_il[group][V^H position][32].
+// Plan data in TILE order (IlPlan::kpack_t ...): samples sorted by tile, inside a tile by 3 x 3 blocks of base cells; a warp
+// takes a contiguous share of the item; group key = window base relative to the tile origin (row | col << 5 | shape << 10).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kItRec = 20;           // floats per staged sample: w0[6], w1[6], group key, output row, variant, pad (80 B: conflict-free 128-bit stores)
+template <int T, int NW> struct IlTile {
+    static constexpr int PW = T + kJ - 1;                       // padded tile edge in cells
+    static constexpr int TILE_BYTES = PW * PW * kIL * 8;
+    static constexpr int REC_BYTES = NW * 32 * kItRec * 4;
+    static constexpr int SMEM = TILE_BYTES + REC_BYTES + 16;
+    static constexpr int CAP = NW * 32;                         // samples per work item
+};
+constexpr int kItT = 14;             // stencil base cells per tile and axis: padded tile 19 x 19 cells x 32 images = 92 KB
+constexpr int kItWarps = 6;          // warps per CTA (two CTAs per SM)
+constexpr int kItAhead = 160;        // plan data of the item this many items later is prefetched into L2
+struct IlTileItem { int32_t start; int32_t cnt; int32_t r0; int32_t c0; };    // tile-order sample range, tile origin (cells)
+
+// the 6 x 6 stencil of a sample whose support starts at (O0, O1) inside the R x C register window
+template <int R, int C, int O0, int O1>
+__device__ __forceinline__ float2 it_eval(const float2 (&win)[R][C], const float (&w0)[kJ], const float (&w1)[kJ]) {
+    float2 acc0 = make_float2(0.f, 0.f), acc1 = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < kJ; ++i) {
+        float2 rs = __fmul2_rn(make_float2(w1[0], w1[0]), win[O0 + i][O1]);
+#pragma unroll
+        for (int j = 1; j < kJ; ++j) rs = __ffma2_rn(make_float2(w1[j], w1[j]), win[O0 + i][O1 + j], rs);
+        if (i & 1) acc1 = __ffma2_rn(make_float2(w0[i], w0[i]), rs, acc1);
+        else acc0 = __ffma2_rn(make_float2(w0[i], w0[i]), rs, acc0);
+    }
+    return __fadd2_rn(acc0, acc1);
+}
+#define NU_IT_VARIANT(V)                                                                     \
+    case V:                                                                                  \
+        if constexpr (V < (R - kJ + 1) * (C - kJ + 1))                                        \
+            acc = it_eval<R, C, V / (C - kJ + 1), V % (C - kJ + 1)>(win, w0, w1);             \
+        break;
+
+// one group of the walk: load its R x C window from the shared tile once, then interpolate its samples t, t + 1, ... while
+// the key stays the same
+template <int R, int C, int PW>
+__device__ __forceinline__ int it_group(const float* __restrict__ recw, int t, int cnt, int key, const float2* __restrict__ tl,
+                                        float2* __restrict__ y_il_grp, int lane) {
+    float2 win[R][C];
+    const float2* __restrict__ base = tl + ((key & 31) * PW + ((key >> 5) & 31)) * kIL;
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+#pragma unroll
+        for (int j = 0; j < C; ++j) win[i][j] = base[(i * PW + j) * kIL];
+    do {
+        const float4* r4 = reinterpret_cast<const float4*>(recw + t * kItRec);
+        const float4 a = r4[0], b = r4[1], c = r4[2], d = r4[3];
+        const float w0[kJ] = {a.x, a.y, a.z, a.w, b.x, b.y};
+        const float w1[kJ] = {b.z, b.w, c.x, c.y, c.z, c.w};
+        float2 acc = make_float2(0.f, 0.f);
+        switch (__float_as_int(d.z)) {       // warp-uniform
+            NU_IT_VARIANT(0) NU_IT_VARIANT(1) NU_IT_VARIANT(2) NU_IT_VARIANT(3) NU_IT_VARIANT(4)
+            NU_IT_VARIANT(5) NU_IT_VARIANT(6) NU_IT_VARIANT(7) NU_IT_VARIANT(8)
+            default: break;
+        }
+        y_il_grp[(int64_t)__float_as_int(d.y) * kIL + lane] = acc;
+        ++t;
+    } while (t < cnt && __float_as_int(recw[t * kItRec + 12]) == key);
+    return t;
+}
+
+template <int T, int NW, int MB>
+__global__ void __launch_bounds__(NW * 32, MB)
+interp_il_tile_kernel(IlPlan s, GridGeom g, const IlTileItem* __restrict__ items, int n_items, int ngroups,
+                      const float2* __restrict__ grid_il, float2* __restrict__ y_il, KernelPoly P,
+                      const __grid_constant__ CUtensorMap tmap, int use_tmap) {
+    using G = IlTile<T, NW>;
+    constexpr int PW = G::PW;
+    extern __shared__ __align__(128) unsigned char it_smem[];
+    float2* tile = reinterpret_cast<float2*>(it_smem);                              // [PW][PW][32]
+    float* recs = reinterpret_cast<float*>(it_smem + G::TILE_BYTES);                // [NW][32][kItRec]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(it_smem + G::TILE_BYTES + G::REC_BYTES);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // the image groups of one item run next to each other: the second one finds the item's plan data in L2
+    const int grp = blockIdx.x % ngroups, item = blockIdx.x / ngroups;
+    const IlTileItem it = items[item];
+    const int K0 = g.K[0], K1 = g.K[1];
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+    // plan data of the item that starts kItAhead items later is pulled into L2 now (it comes from DRAM otherwise: two
+    // dependent misses at the head of every CTA)
+    IlTileItem nxt{0, 0, 0, 0};
+    const bool pf = warp == NW - 1 && grp == 0 && item + kItAhead < n_items;
+    if (pf) nxt = items[item + kItAhead];
+    pdl_enter();      // the grid is the previous kernel's output
+    if (warp == 0) {
+        const bool inside = it.r0 + PW <= K0 && it.c0 + PW <= K1;
+        if (use_tmap && inside) {
+            if (lane == 0) {
+                mbar_expect_tx(bar, (uint32_t)G::TILE_BYTES);
+                tma_load_tile_4d(tile, &tmap, 0, it.c0, it.r0, grp, bar);
+            }
+        } else {
+            if (lane == 0) mbar_expect_tx(bar, (uint32_t)G::TILE_BYTES);
+            __syncwarp();
+            const float2* __restrict__ Gg = grid_il + (int64_t)grp * g.cells * kIL;
+            if (lane < PW) {      // one padded row per lane, split where it crosses the seam of axis 1
+                const float2* __restrict__ row = Gg + (int64_t)((it.r0 + lane) & (K0 - 1)) * K1 * kIL;
+                const int n1 = min(PW, K1 - it.c0);
+                bulk_g2s(tile + (lane * PW) * kIL, row + (int64_t)it.c0 * kIL, (uint32_t)(n1 * kIL * 8), bar);
+                if (n1 < PW) bulk_g2s(tile + (lane * PW + n1) * kIL, row, (uint32_t)((PW - n1) * kIL * 8), bar);
+            }
+        }
+    }
+    // the warp's share of the item; lane = sample while staging
+    const int per = (it.cnt + NW - 1) / NW;
+    const int t0 = warp * per;
+    const int cnt = max(0, min(per, it.cnt - t0));
+    float* recw = recs + warp * 32 * kItRec;
+    if (lane < cnt) {
+        const int64_t si = (int64_t)it.start + t0 + lane;
+        const uint32_t gb = __ldg(&s.gbase_t[si]);
+        const uint32_t kp = __ldg(&s.kpack_t[si]);
+        const int32_t orow = __ldg(&s.t2h[si]);
+        float w0[kJ], w1[kJ];
+        if (s.wv_t) {       // coef_mode = 1: precomputed (float64-built) weights, 48 contiguous bytes per sample
+            const float4* __restrict__ t4 = reinterpret_cast<const float4*>(s.wv_t + si * 12);
+            const float4 a = __ldg(t4), b = __ldg(t4 + 1), c = __ldg(t4 + 2);
+            w0[0] = a.x; w0[1] = a.y; w0[2] = a.z; w0[3] = a.w; w0[4] = b.x; w0[5] = b.y;
+            w1[0] = b.z; w1[1] = b.w; w1[2] = c.x; w1[3] = c.y; w1[4] = c.z; w1[5] = c.w;
+        } else {
+            kb_weights(P, 0, __ldg(&s.delta_t[si]), w0);
+            kb_weights(P, 1, __ldg(&s.delta_t[g.M + si]), w1);
+        }
+        const int sh = (int)(gb >> 10) & 7;
+        const int o0 = (int)(kp & 1023u) - it.r0 - (int)(gb & 31u), o1 = (int)((kp >> 10) & 1023u) - it.c0 - (int)((gb >> 5) & 31u);
+        float4* r4 = reinterpret_cast<float4*>(recw + lane * kItRec);
+        r4[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
+        r4[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
+        r4[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
+        r4[3] = make_float4(__int_as_float((int)gb), __int_as_float(orow), __int_as_float(o0 * (iw_cols(sh) - kJ + 1) + o1), 0.f);
+    }
+    if (pf) {         // 5 arrays x (<= NW * 32 entries x 4 B), one 128-B line per lane and round
+        constexpr int LPA = (NW * 32 * 4 + 127) / 128 + 1;      // lines per array (+1: the range is not line-aligned)
+        for (int q = lane; q < 5 * LPA; q += 32) {
+            const int arr = q / LPA, ln = q % LPA;
+            const char* bp = arr == 0 ? (const char*)(s.gbase_t + nxt.start) : arr == 1 ? (const char*)(s.kpack_t + nxt.start)
+                           : arr == 2 ? (const char*)(s.t2h + nxt.start) : arr == 3 ? (const char*)(s.delta_t + nxt.start)
+                           : (const char*)(s.delta_t + g.M + nxt.start);
+            if (ln * 128 < nxt.cnt * 4 + 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(bp + ln * 128));
+        }
+    }
+    __syncwarp();
+    mbar_wait(bar, 0);
+    const float2* __restrict__ tl = tile + lane;
+    float2* __restrict__ yg = y_il + (int64_t)grp * g.M * kIL;
+    int t = 0;
+#pragma unroll 1
+    while (t < cnt) {
+        const int key = __float_as_int(recw[t * kItRec + 12]);
+        switch ((key >> 10) & 7) {       // warp-uniform
+            case 1: t = it_group<iw_rows(1), iw_cols(1), PW>(recw, t, cnt, key, tl, yg, lane); break;
+            case 2: t = it_group<iw_rows(2), iw_cols(2), PW>(recw, t, cnt, key, tl, yg, lane); break;
+            case 3: t = it_group<iw_rows(3), iw_cols(3), PW>(recw, t, cnt, key, tl, yg, lane); break;
+            case 4: t = it_group<iw_rows(4), iw_cols(4), PW>(recw, t, cnt, key, tl, yg, lane); break;
+            default: t = it_group<iw_rows(0), iw_cols(0), PW>(recw, t, cnt, key, tl, yg, lane); break;
         }
     }
 }

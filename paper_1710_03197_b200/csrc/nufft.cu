@@ -110,6 +110,13 @@ struct nufft_plan_s {
     bool il_coherent = false;
     IlItem* d_il_items = nullptr;
     int n_il_items = 0;
+    uint32_t* d_il_kpack_t = nullptr;    // tile order of interp_il_tile_kernel
+    float* d_il_delta_t = nullptr;
+    uint32_t* d_il_gbase_t = nullptr;
+    float* d_il_wv_t = nullptr;
+    int32_t* d_il_t2h = nullptr;
+    IlTileItem* d_il_titems = nullptr;
+    int n_il_titems = 0;
     float2* noalloc_grid = nullptr;     // device address of g_noalloc_grid on the plan's device (nufft_adjoint_noalloc), or null
     float2* d_yil = nullptr;        // [groups][M][32] sorted, interleaved samples (adjoint input), lazy
     // "next" rows: density compensation and Toeplitz A^H A
@@ -225,6 +232,7 @@ static cudaError_t configure_all() {
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(interp_tiled_3d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kInterp3dSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_il_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<1>::BYTES)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(interp_il_tile_kernel<kItT, kItWarps, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, IlTile<kItT, kItWarps>::SMEM)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_il_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GridStage<2>::BYTES)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(gridding_tiled_3d_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)) != cudaSuccess) return e;
 #define NU_W3_CFG(NW)                                                                                                                   \
@@ -736,6 +744,7 @@ static IlPlan il_plan(nufft_plan_t p) {
     s.kpack_c = p->d_il_kpack_c; s.delta_c = p->d_il_delta_c;
     s.gbase = p->d_il_gbase; s.gbase_c = p->d_il_gbase_c;
     s.wv = p->d_il_wv; s.wv_c = p->d_il_wv_c;
+    s.kpack_t = p->d_il_kpack_t; s.delta_t = p->d_il_delta_t; s.gbase_t = p->d_il_gbase_t; s.wv_t = p->d_il_wv_t; s.t2h = p->d_il_t2h;
     return s;
 }
 
@@ -774,6 +783,23 @@ static int run_interp_il(nufft_plan_t p, int batch, const float2* grid, float2* 
     if (p->M == 0) return NUFFT_OK;
     const dim3 blocks((unsigned)((p->M + kInterpChunk - 1) / kInterpChunk), (unsigned)il_groups(batch));
     ProfScope ps(p, "interp", st);
+    if (p->n_il_titems > 0) {     // register windows fed from shared tiles (interp_mode = 0)
+        using G = IlTile<kItT, kItWarps>;
+        const int ng = il_groups(batch);
+        CUtensorMap tm;
+        std::memset(&tm, 0, sizeof(tm));
+        int use_tm = 0;
+        if (tmap_encode_fn enc = tmap_encoder()) {      // grid_il [groups][K0][K1][32] complex64 as float32 [groups][K0][K1][64]
+            const cuuint32_t est[4] = {1, 1, 1, 1};
+            const cuuint64_t gdim[4] = {(cuuint64_t)2 * kIL, (cuuint64_t)p->K[1], (cuuint64_t)p->K[0], (cuuint64_t)ng};
+            const cuuint64_t gstr[3] = {(cuuint64_t)kIL * 8, (cuuint64_t)p->K[1] * kIL * 8, (cuuint64_t)p->cells * kIL * 8};
+            const cuuint32_t box[4] = {2 * kIL, (cuuint32_t)G::PW, (cuuint32_t)G::PW, 1};
+            use_tm = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)grid, gdim, gstr, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS ? 1 : 0;
+        }
+        launch_pdl(interp_il_tile_kernel<kItT, kItWarps, 2>, dim3((unsigned)(p->n_il_titems * ng)), dim3(kItWarps * 32), (size_t)G::SMEM, st,
+                   il_plan(p), grid_geom(p), (const IlTileItem*)p->d_il_titems, p->n_il_titems, ng, grid, y_il, p->poly, tm, use_tm);
+    } else
     if (p->opts.interp_mode != 3) {     // register windows over the block-sorted walk (interp_mode = 3: round-1 kernel)
         const dim3 wb((unsigned)((p->M + kIwWarps * 32 - 1) / (kIwWarps * 32)), (unsigned)il_groups(batch));
         launch_pdl(interp_il_win_kernel<false>, wb, dim3(kIwWarps * 32), 0, st, il_plan(p), grid_geom(p), grid, y_il, batch, p->poly);
@@ -1048,6 +1074,87 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
             std::vector<float> tab;
             weight_table([&](int64_t i) { return (int64_t)perm_v[i]; }, gb_v, tab);
             NU_TRY(dev_upload(&p->d_il_wv, tab, &p->bytes_plan));
+        }
+    }
+    // ---- tile order (interp_il_tile_kernel): samples sorted by tile of kItT x kItT base cells, inside a tile by 3 x 3 blocks
+    // relative to the tile origin; work items of <= kItWarps * 32 samples (a tile with more is cut into equal parts); warp w of
+    // an item walks its w-th share, and window groups never cross a share.  Window bases are stored relative to the tile
+    // origin and clamped so that the window stays inside the padded tile.
+    if (p->opts.interp_mode == 0 && K0 >= IlTile<kItT, kItWarps>::PW && K1 >= IlTile<kItT, kItWarps>::PW) {
+        constexpr int T = kItT, PW = IlTile<kItT, kItWarps>::PW, CAP = IlTile<kItT, kItWarps>::CAP, NB = (T + 2) / 3;
+        const int ntr = (K0 + T - 1) / T, ntc = (K1 + T - 1) / T;
+        const int64_t per_tile = (int64_t)NB * NB * 9;
+        std::vector<int32_t> perm_t, bins_t;
+        sort_by([&](uint32_t kp) -> int64_t {
+            const int r = row_of(kp), c = col_of(kp), rr = r % T, cc = c % T;
+            return ((int64_t)(c / T) * ntr + r / T) * per_tile + ((int64_t)(cc / 3) * NB + rr / 3) * 9 + (rr % 3) * 3 + (cc % 3);
+        }, (int64_t)ntr * ntc * per_tile, perm_t, bins_t);
+        std::vector<uint32_t> kp_t(M), gb_t(M);
+        std::vector<float> dl_t((size_t)2 * M);
+        std::vector<int32_t> t2h(M);
+        for (int64_t i = 0; i < M; ++i) {
+            const int64_t m = perm_t[i];
+            kp_t[i] = kpack[m]; dl_t[i] = delta[m]; dl_t[M + i] = delta[M + m]; t2h[i] = pos_h[m];
+        }
+        std::vector<IlTileItem> titems;
+        for (int tc = 0; tc < ntc; ++tc)
+            for (int tr = 0; tr < ntr; ++tr) {
+                const int64_t tb = ((int64_t)tc * ntr + tr) * per_tile;
+                const int64_t a = bins_t[tb], n = bins_t[tb + per_tile] - a;
+                if (n == 0) continue;
+                const int64_t parts = (n + CAP - 1) / CAP;
+                for (int64_t q = 0; q < parts; ++q) {
+                    const int64_t lo = a + n * q / parts, hi = a + n * (q + 1) / parts;
+                    titems.push_back(IlTileItem{(int32_t)lo, (int32_t)(hi - lo), tr * T, tc * T});
+                }
+            }
+        for (const IlTileItem& it : titems) {
+            const int per = (it.cnt + kItWarps - 1) / kItWarps;
+            for (int w = 0; w < kItWarps; ++w) {
+                const int64_t lo = it.start + (int64_t)w * per, hi = std::min<int64_t>((int64_t)it.start + it.cnt, lo + per);
+                int64_t i = lo;
+                while (i < hi) {
+                    int best_sh = 0, best_lo0 = 0, best_lo1 = 0;
+                    int64_t best_n = 0;
+                    for (int sh = 0; sh < kIwShapes; ++sh) {
+                        const int sp0 = iw_rows(sh) - kJ, sp1 = iw_cols(sh) - kJ;
+                        int lo0 = row_of(kp_t[i]), hi0 = lo0, lo1 = col_of(kp_t[i]), hi1 = lo1;
+                        int64_t j = i + 1;
+                        for (; j < hi; ++j) {
+                            const int r = row_of(kp_t[j]), c = col_of(kp_t[j]);
+                            const int nlo0 = std::min(lo0, r), nhi0 = std::max(hi0, r), nlo1 = std::min(lo1, c), nhi1 = std::max(hi1, c);
+                            if (nhi0 - nlo0 > sp0 || nhi1 - nlo1 > sp1) break;
+                            lo0 = nlo0; hi0 = nhi0; lo1 = nlo1; hi1 = nhi1;
+                        }
+                        const int64_t n = j - i;
+                        if (best_n == 0 || (int64_t)iw_rows(sh) * iw_cols(sh) * best_n < (int64_t)iw_rows(best_sh) * iw_cols(best_sh) * n) {
+                            best_n = n; best_sh = sh; best_lo0 = lo0; best_lo1 = lo1;
+                        }
+                    }
+                    const int b0 = std::min(best_lo0 - it.r0, PW - iw_rows(best_sh)), b1 = std::min(best_lo1 - it.c0, PW - iw_cols(best_sh));
+                    const uint32_t base = (uint32_t)b0 | ((uint32_t)b1 << 5) | ((uint32_t)best_sh << 10);
+                    for (int64_t k = i; k < i + best_n; ++k) gb_t[k] = base;
+                    i += best_n;
+                }
+            }
+        }
+        std::stable_sort(titems.begin(), titems.end(), [](const IlTileItem& a, const IlTileItem& b) { return a.cnt > b.cnt; });
+        p->n_il_titems = (int)titems.size();
+        NU_TRY(dev_upload(&p->d_il_kpack_t, kp_t, &p->bytes_plan));
+        NU_TRY(dev_upload(&p->d_il_delta_t, dl_t, &p->bytes_plan));
+        NU_TRY(dev_upload(&p->d_il_gbase_t, gb_t, &p->bytes_plan));
+        NU_TRY(dev_upload(&p->d_il_t2h, t2h, &p->bytes_plan));
+        NU_TRY(dev_upload(&p->d_il_titems, titems, &p->bytes_plan));
+        if (p->opts.coef_mode == 1) {
+            std::vector<float> tab((size_t)M * 12, 0.f);
+            for (int64_t i = 0; i < M; ++i) {
+                const int64_t m = perm_t[i];
+                double w0[kJ], w1[kJ];
+                if (p->minmax) { p->mm[0].weights(delta64[m], w0); p->mm[1].weights(delta64[M + m], w1); }
+                else { host::kb_weights_f64(delta64[m], J, beta, w0); host::kb_weights_f64(delta64[M + m], J, beta, w1); }
+                for (int j = 0; j < kJ; ++j) { tab[(size_t)i * 12 + j] = (float)w0[j]; tab[(size_t)i * 12 + 6 + j] = (float)w1[j]; }
+            }
+            NU_TRY(dev_upload(&p->d_il_wv_t, tab, &p->bytes_plan));
         }
     }
     NU_TRY(dev_upload(&p->d_il_kpack, kp_s, &p->bytes_plan));
@@ -1359,6 +1466,7 @@ extern "C" int nufft_destroy(nufft_plan_t p) {
     cudaFree(p->d_il_kpack); cudaFree(p->d_il_delta); cudaFree(p->d_il_pos); cudaFree(p->d_il_wtab);
     cudaFree(p->d_il_kpack_c); cudaFree(p->d_il_delta_c); cudaFree(p->d_il_gbase); cudaFree(p->d_il_gbase_c); cudaFree(p->d_w3rec); cudaFree(p->d_il_wv); cudaFree(p->d_il_wv_c);
     cudaFree(p->d_il_rowptr); cudaFree(p->d_il_v2h); cudaFree(p->d_il_items); cudaFree(p->d_yil);
+    cudaFree(p->d_il_kpack_t); cudaFree(p->d_il_delta_t); cudaFree(p->d_il_gbase_t); cudaFree(p->d_il_wv_t); cudaFree(p->d_il_t2h); cudaFree(p->d_il_titems);
     if (p->cg_graph) cudaGraphExecDestroy(p->cg_graph);
     for (auto& og : p->op_graphs) cudaGraphExecDestroy(og.exec);
     if (p->hp_h2d) cudaStreamDestroy(p->hp_h2d);
