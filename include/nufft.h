@@ -70,8 +70,9 @@ typedef struct {
                            0 = recomputed on the fly from a piecewise polynomial fit of the kernel: 4 + 4 d bytes of plan
                                data per sample (the default: fewest bytes; measured 2-7 % slower than 1, profiles/r02_coef_mode.md);
                            1 = precomputed by the plan in float64, rounded once, stored zero-padded in a coalesced per-sample
-                               layout in walk order -- 64 B per sample for the interleaved 2-D V, 112 B for the register-window
-                               3-D V / V^H (moved to shared memory by one bulk copy per 16 samples).  Other kernels (planar
+                               layout in walk order -- 96 B per sample and walk order (48 B in tile order) for the interleaved
+                               2-D V, 112 B for the register-window 3-D V / V^H (moved to shared memory by one bulk copy
+                               per 16 samples).  Other kernels (planar
                                2-D, generic widths) recompute in either mode; the interleaved V^H always reads its
                                float64-built 96-B table.  Any other value -> NUFFT_EINVAL                                   */
     int adjoint_mode;   /* planar path: 0 = V^H by tile-sorted accumulation on chip, one TMA reduce-add flush per work item
@@ -83,10 +84,13 @@ typedef struct {
                            The interleaved path (batch >= 12) is always deterministic (gather form, fixed order)        */
     int interp_mode;    /* 0 = library default: register-window kernels -- 3-D planar V keeps an 8 x 8 x 8 window of the
                                staged tile in registers and slides it along the pencil-sorted samples; interleaved V keeps
-                               the 8 x 8 window of a group of neighbouring samples in registers and walks the CALLER's
-                               sample order, writing y directly, when the trajectory is coherent (>= 90 % of consecutive
-                               samples within two grid cells: radial spokes, spiral arms); 2-D planar V gathers through L1/L2;
-                           1 = the plain variants: direct gather in 3-D, sorted walk + layout pass on the interleaved path;
+                               the window (8 x 8, 6 x 10, ... cells) of a group of neighbouring samples in registers; the
+                               forward call walks the CALLER's sample order, writing y directly, when the trajectory is
+                               coherent (>= 90 % of consecutive samples within two grid cells: radial spokes, spiral arms);
+                               A^H A, the solvers and incoherent trajectories walk a tile order whose 19 x 19-cell tiles
+                               are staged in shared memory by one tensor-map copy each; 2-D planar V stages tiles likewise;
+                           1 = the plain variants: direct gather in 3-D and planar 2-D; on the interleaved path the block-sorted
+                               walk with windows loaded from L2 (+ layout pass), never the caller's order or shared tiles;
                            2 = the generic-width kernels (direct V, atomic V^H, planar) even at Jd = 6: what a plan
                                with Jd != 6 runs, selectable at Jd = 6 for cross-checks against the tuned kernels;
                            3 = the round-1 kernels (half-warp-per-sample 3-D V, stencil-per-sample interleaved V), kept
