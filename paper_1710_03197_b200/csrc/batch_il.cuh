@@ -25,7 +25,7 @@ namespace nufft {
 
 constexpr int kIL = 32;      // images per interleaved group (= lanes per warp)
 constexpr int kBandW = 8;    // grid columns per V^H band (accumulators per lane: kBandW complex)
-constexpr int kTabW = 24;    // floats per sample in the V^H weight table: w0[6], 2 pad, w1 band-aligned A[8], B[8]
+constexpr int kTabW = 24;    // floats per sample in the V^H weight table: w0 rotated [8], w1 band-aligned A[8], B[8]
 
 // ------------------------------------------------------------------------------------------------------------
 // FFT row passes between the caller's planar images and the interleaved grid
@@ -176,7 +176,7 @@ struct IlPlan {
     const float* wv_t;        // coef_mode = 1: weights [M][12] (w0[6], w1[6]) in tile order, else null
     const int32_t* t2h;       // tile-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
-    const float* wtab;        // V^H order: [M][kTabW] = w0[6], k0_0 (int bits), pad, w1 part A[8], w1 part B[8] (float64-built)
+    const float* wtab;        // V^H order: [M][kTabW] = w0 rotated by the base row (slot (k0_0 + j) & 7 = w0[j], others 0), w1 part A[8], w1 part B[8] (float64-built)
     const int32_t* rowptr;    // [(band * 2 + class) * K0 + row]: first V^H-order sample of (band, class, row); + 1 entry
 };
 
@@ -661,33 +661,6 @@ struct IlItem {
     int32_t load;     // row-sample interactions of the item (plan-time cost estimate; sort key)
 };
 
-// Adds the samples [b, e) of the V^H order to the 8 accumulators of output row `row`.  OFF = 8: the samples lie in this
-// band (table part A), OFF = 16: in the previous band (part B).  The samples of a range span up to 6 stencil base rows;
-// each one looks up its own row weight w0[row - k0_0].
-template <int OFF>
-__device__ __forceinline__ void il_accumulate(float2 (&acc)[kBandW], const float* __restrict__ wtab,
-                                              const float2* __restrict__ Y, int row, int kmask, int b, int e) {
-    const float* __restrict__ rec = wtab + (int64_t)b * kTabW;
-    const float2* __restrict__ yp = Y + (int64_t)b * kIL;
-#pragma unroll 4
-    for (int i = b; i < e; ++i, rec += kTabW, yp += kIL) {
-        const int j0 = (row - __float_as_int(__ldg(rec + 6))) & kmask;
-        const float w0 = __ldg(rec + j0);
-        const float4 pa = __ldg(reinterpret_cast<const float4*>(rec + OFF));
-        const float4 pb = __ldg(reinterpret_cast<const float4*>(rec + OFF + 4));
-        const float2 yv = __ldg(yp);
-        const float tx = w0 * yv.x, ty = w0 * yv.y;
-        acc[0].x = fmaf(pa.x, tx, acc[0].x); acc[0].y = fmaf(pa.x, ty, acc[0].y);
-        acc[1].x = fmaf(pa.y, tx, acc[1].x); acc[1].y = fmaf(pa.y, ty, acc[1].y);
-        acc[2].x = fmaf(pa.z, tx, acc[2].x); acc[2].y = fmaf(pa.z, ty, acc[2].y);
-        acc[3].x = fmaf(pa.w, tx, acc[3].x); acc[3].y = fmaf(pa.w, ty, acc[3].y);
-        acc[4].x = fmaf(pb.x, tx, acc[4].x); acc[4].y = fmaf(pb.x, ty, acc[4].y);
-        acc[5].x = fmaf(pb.y, tx, acc[5].x); acc[5].y = fmaf(pb.y, ty, acc[5].y);
-        acc[6].x = fmaf(pb.z, tx, acc[6].x); acc[6].y = fmaf(pb.z, ty, acc[6].y);
-        acc[7].x = fmaf(pb.w, tx, acc[7].x); acc[7].y = fmaf(pb.w, ty, acc[7].y);
-    }
-}
-
 constexpr int kStageCap = 48;      // samples per list per staging round (one group per CTA)
 constexpr int kStageCap2 = 40;     // ... when a CTA handles two groups (64 images)
 template <int NG> struct GridStage {
@@ -703,12 +676,11 @@ template <int NG> struct GridStage {
 template <int OFF, int NG, int CAP>
 __device__ __forceinline__ void il_accumulate_smem(float2 (&ax)[NG][kBandW / 2], float2 (&ay)[NG][kBandW / 2],
                                                    const float* __restrict__ rec_s, const float2* __restrict__ y_s,
-                                                   int row, int kmask, int i0, int i1) {
+                                                   int row, int i0, int i1) {
 #pragma unroll 4
     for (int i = i0; i < i1; ++i) {
         const float* rec = rec_s + i * kTabW;
-        const int j0 = (row - __float_as_int(rec[6])) & kmask;
-        const float w0 = rec[j0];
+        const float w0 = rec[row & 7];        // w0 is stored rotated by the stencil base row (slot (k0_0 + j) & 7 = w0[j])
         const float4 pa = *reinterpret_cast<const float4*>(rec + OFF);
         const float4 pb = *reinterpret_cast<const float4*>(rec + OFF + 4);
 #pragma unroll
@@ -806,8 +778,8 @@ gridding_il_kernel(IlPlan s, GridGeom g, const IlItem* __restrict__ items, const
                 if (x1 > x0) {
                     const int n = x1 - x0;
                     const int i0 = x0 - c0 + ((n * part) >> lsplit), i1 = x0 - c0 + ((n * (part + 1)) >> lsplit);
-                    if (q == 2) il_accumulate_smem<16, NG, CAP>(ax, ay, rec_s + q * CAP * kTabW, y_s + q * CAP * kIL + lane, row, K0 - 1, i0, i1);
-                    else        il_accumulate_smem<8, NG, CAP>(ax, ay, rec_s + q * CAP * kTabW, y_s + q * CAP * kIL + lane, row, K0 - 1, i0, i1);
+                    if (q == 2) il_accumulate_smem<16, NG, CAP>(ax, ay, rec_s + q * CAP * kTabW, y_s + q * CAP * kIL + lane, row, i0, i1);
+                    else        il_accumulate_smem<8, NG, CAP>(ax, ay, rec_s + q * CAP * kTabW, y_s + q * CAP * kIL + lane, row, i0, i1);
                 }
             }
             __syncthreads();      // every warp is done with the staged chunk before the next round overwrites it

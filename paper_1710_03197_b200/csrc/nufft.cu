@@ -999,9 +999,8 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
         if (p->minmax) { p->mm[0].weights(delta64[m], w0); p->mm[1].weights(delta64[M + m], w1); }
         else { host::kb_weights_f64(delta64[m], J, beta, w0); host::kb_weights_f64(delta64[M + m], J, beta, w1); }
         float* rec = &wtab[(size_t)i * kTabW];
-        for (int j = 0; j < kJ; ++j) rec[j] = (float)w0[j];
         const int32_t r = row_of(kpack[m]);
-        std::memcpy(&rec[6], &r, sizeof(r));             // stencil base row k0_0 (int bits)
+        for (int j = 0; j < kJ; ++j) rec[(r + j) & 7] = (float)w0[j];     // rotated by the base row: output row R reads slot R & 7
         const int off = col_of(kpack[m]) % kBandW;
         for (int j = 0; j < kJ; ++j) {
             const int c = off + j;                       // column relative to the start of the sample's own band
