@@ -172,7 +172,7 @@ struct IlPlan {
     const int32_t* v2h;       // V-order position -> V^H-order position
     const uint32_t* kpack_t;  // TILE order (interp_il_tile_kernel): stencil base index per axis
     const float* delta_t;     // tile order [2][M]
-    const uint32_t* gbase_t;  // tile order: window base relative to the tile origin (row | col << 5) | shape << 10
+    const uint32_t* gbase_t;  // tile order: base of the sample's 8 x 8 window relative to the tile origin (row | col << 5)
     const float* wv_t;        // coef_mode = 1: weights [M][12] (w0[6], w1[6]) in tile order, else null
     const int32_t* t2h;       // tile-order position -> V^H-order position
     const int32_t* pos;       // caller's sample index -> V^H-order position
@@ -432,7 +432,7 @@ interp_il_win_kernel(IlPlan s, GridGeom g, const float2* __restrict__ grid_il, f
 // FMAs per sample instead of the 72 zero-padded ones of interp_il_win_kernel (measured: the padded form is FMA-pipe bound
 // here once the loads come from shared memory).  Output rows y_il[group][V^H position][32].
 // Plan data in TILE order (IlPlan::kpack_t ...): samples sorted by tile, inside a tile by 3 x 3 blocks of base cells; a warp
-// takes a contiguous share of the item; group key = window base relative to the tile origin (row | col << 5 | shape << 10).
+// takes a contiguous share of the item; group key = base of the group's 8 x 8 window relative to the tile origin (row | col << 5).
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kItRec = 20;           // floats per staged sample: w0[6], w1[6], group key, output row, variant, pad (80 B: conflict-free 128-bit stores)
 template <int T, int NW> struct IlTile {
@@ -444,6 +444,7 @@ template <int T, int NW> struct IlTile {
 };
 constexpr int kItT = 14;             // stencil base cells per tile and axis: padded tile 19 x 19 cells x 32 images = 92 KB
 constexpr int kItWarps = 6;          // warps per CTA (two CTAs per SM)
+constexpr int kItWin = 8;            // window edge in cells (8 x 8 cells = 128 registers per lane)
 constexpr int kItAhead = 160;        // plan data of the item this many items later is prefetched into L2
 struct IlTileItem { int32_t start; int32_t cnt; int32_t r0; int32_t c0; };    // tile-order sample range, tile origin (cells)
 
@@ -558,13 +559,12 @@ interp_il_tile_kernel(IlPlan s, GridGeom g, const IlTileItem* __restrict__ items
             kb_weights(P, 0, __ldg(&s.delta_t[si]), w0);
             kb_weights(P, 1, __ldg(&s.delta_t[g.M + si]), w1);
         }
-        const int sh = (int)(gb >> 10) & 7;
         const int o0 = (int)(kp & 1023u) - it.r0 - (int)(gb & 31u), o1 = (int)((kp >> 10) & 1023u) - it.c0 - (int)((gb >> 5) & 31u);
         float4* r4 = reinterpret_cast<float4*>(recw + lane * kItRec);
         r4[0] = make_float4(w0[0], w0[1], w0[2], w0[3]);
         r4[1] = make_float4(w0[4], w0[5], w1[0], w1[1]);
         r4[2] = make_float4(w1[2], w1[3], w1[4], w1[5]);
-        r4[3] = make_float4(__int_as_float((int)gb), __int_as_float(orow), __int_as_float(o0 * (iw_cols(sh) - kJ + 1) + o1), 0.f);
+        r4[3] = make_float4(__int_as_float((int)gb), __int_as_float(orow), __int_as_float(o0 * (kItWin - kJ + 1) + o1), 0.f);
     }
     if (pf) {         // 5 arrays x (<= NW * 32 entries x 4 B), one 128-B line per lane and round
         constexpr int LPA = (NW * 32 * 4 + 127) / 128 + 1;      // lines per array (+1: the range is not line-aligned)
@@ -584,13 +584,7 @@ interp_il_tile_kernel(IlPlan s, GridGeom g, const IlTileItem* __restrict__ items
 #pragma unroll 1
     while (t < cnt) {
         const int key = __float_as_int(recw[t * kItRec + 12]);
-        switch ((key >> 10) & 7) {       // warp-uniform
-            case 1: t = it_group<iw_rows(1), iw_cols(1), PW>(recw, t, cnt, key, tl, yg, lane); break;
-            case 2: t = it_group<iw_rows(2), iw_cols(2), PW>(recw, t, cnt, key, tl, yg, lane); break;
-            case 3: t = it_group<iw_rows(3), iw_cols(3), PW>(recw, t, cnt, key, tl, yg, lane); break;
-            case 4: t = it_group<iw_rows(4), iw_cols(4), PW>(recw, t, cnt, key, tl, yg, lane); break;
-            default: t = it_group<iw_rows(0), iw_cols(0), PW>(recw, t, cnt, key, tl, yg, lane); break;
-        }
+        t = it_group<kItWin, kItWin, PW>(recw, t, cnt, key, tl, yg, lane);
     }
 }
 

@@ -1112,28 +1112,20 @@ static int plan_build_il(nufft_plan_t p, const std::vector<uint32_t>& kpack, con
             for (int w = 0; w < kItWarps; ++w) {
                 const int64_t lo = it.start + (int64_t)w * per, hi = std::min<int64_t>((int64_t)it.start + it.cnt, lo + per);
                 int64_t i = lo;
-                while (i < hi) {
-                    int best_sh = 0, best_lo0 = 0, best_lo1 = 0;
-                    int64_t best_n = 0;
-                    for (int sh = 0; sh < kIwShapes; ++sh) {
-                        const int sp0 = iw_rows(sh) - kJ, sp1 = iw_cols(sh) - kJ;
-                        int lo0 = row_of(kp_t[i]), hi0 = lo0, lo1 = col_of(kp_t[i]), hi1 = lo1;
-                        int64_t j = i + 1;
-                        for (; j < hi; ++j) {
-                            const int r = row_of(kp_t[j]), c = col_of(kp_t[j]);
-                            const int nlo0 = std::min(lo0, r), nhi0 = std::max(hi0, r), nlo1 = std::min(lo1, c), nhi1 = std::max(hi1, c);
-                            if (nhi0 - nlo0 > sp0 || nhi1 - nlo1 > sp1) break;
-                            lo0 = nlo0; hi0 = nhi0; lo1 = nlo1; hi1 = nhi1;
-                        }
-                        const int64_t n = j - i;
-                        if (best_n == 0 || (int64_t)iw_rows(sh) * iw_cols(sh) * best_n < (int64_t)iw_rows(best_sh) * iw_cols(best_sh) * n) {
-                            best_n = n; best_sh = sh; best_lo0 = lo0; best_lo1 = lo1;
-                        }
+                while (i < hi) {      // greedy runs whose bases fit a 3 x 3 box: one 8 x 8 window (measured: the other shapes of
+                    // interp_il_win gain nothing in this order)
+                    int lo0 = row_of(kp_t[i]), hi0 = lo0, lo1 = col_of(kp_t[i]), hi1 = lo1;
+                    int64_t j = i + 1;
+                    for (; j < hi; ++j) {
+                        const int r = row_of(kp_t[j]), c = col_of(kp_t[j]);
+                        const int nlo0 = std::min(lo0, r), nhi0 = std::max(hi0, r), nlo1 = std::min(lo1, c), nhi1 = std::max(hi1, c);
+                        if (nhi0 - nlo0 > kItWin - kJ || nhi1 - nlo1 > kItWin - kJ) break;
+                        lo0 = nlo0; hi0 = nhi0; lo1 = nlo1; hi1 = nhi1;
                     }
-                    const int b0 = std::min(best_lo0 - it.r0, PW - iw_rows(best_sh)), b1 = std::min(best_lo1 - it.c0, PW - iw_cols(best_sh));
-                    const uint32_t base = (uint32_t)b0 | ((uint32_t)b1 << 5) | ((uint32_t)best_sh << 10);
-                    for (int64_t k = i; k < i + best_n; ++k) gb_t[k] = base;
-                    i += best_n;
+                    const int b0 = std::min(lo0 - it.r0, PW - kItWin), b1 = std::min(lo1 - it.c0, PW - kItWin);
+                    const uint32_t base = (uint32_t)b0 | ((uint32_t)b1 << 5);
+                    for (int64_t k = i; k < j; ++k) gb_t[k] = base;
+                    i = j;
                 }
             }
         }
