@@ -415,7 +415,7 @@ def run_ours(args):
                     "order": "strict: copies in are ordered after the caller's stream (flush + start event), nothing moves "
                              "outside the event bracket",
                     "call": "nufft_selfadjoint_host: the forward+adjoint pair A^H(A x) per image with y kept on the device "
-                            "(sorted-walk V, no layout pass), 32-image chunks pipelined H2D / kernels / D2H",
+                            "(sorted-walk V, no layout pass), 16-image chunks pipelined H2D / kernels / D2H",
                     "relaxed_input_ready": {"value": world * B / (e2e_relaxed_ms / K_steps * 1e-3),
                                             "note": "nufft_host_input_ready(1): the copy in of a call may start before the "
                                                     "previous work on the caller's stream ends (here: during the untimed "

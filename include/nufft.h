@@ -158,7 +158,8 @@ int nufft_adjoint_noalloc(nufft_plan_t p, const nufft_c64 *y, nufft_c64 *x, void
 
 /* The same three transforms on HOST buffers (bench.py's end-to-end leg).  x / y are host pointers, read / written
  * asynchronously: they must stay valid until `stream` has passed this call, and should be page-locked (pinned) --
- * pageable memory works but serialises the copies.  The batch is cut into chunks (32 images on the interleaved path);
+ * pageable memory works but serialises the copies.  The batch is cut into chunks (16 images on the interleaved path: its
+ * kernels cost the same for 16 and 32 images, the copies do not, and the pipeline is copy-bound);
  * chunk c+1 is copied in on an internal copy stream while the kernels of chunk c run on `stream` and chunk c-1 is
  * copied back on a second copy stream; `stream` is made to wait for the last copy back before the call's work counts
  * as finished.  Device staging buffers (2 x 2 chunks) belong to the plan.
