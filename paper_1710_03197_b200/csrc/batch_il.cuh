@@ -631,11 +631,15 @@ y_from_il_kernel(const int32_t* __restrict__ pos, const float2* __restrict__ y_i
     const int cnt = (int)min((int64_t)32, M - m0);
     const int my = (lane < cnt) ? __ldg(&pos[m0 + lane]) : 0;
     const float2* __restrict__ src = y_il + (int64_t)grp * M * kIL + lane;
-#pragma unroll 8
-    for (int k = 0; k < cnt; ++k) {
+    // all 32 row loads are issued before the first one is consumed (as in y_to_il_kernel: the pass is latency-bound otherwise)
+    float2 v[kIL];
+#pragma unroll
+    for (int k = 0; k < kIL; ++k) {
         const int i = __shfl_sync(0xffffffffu, my, k);
-        tile[warp][k][lane] = __ldg(&src[(int64_t)i * kIL]);
+        v[k] = (k < cnt) ? __ldg(&src[(int64_t)i * kIL]) : make_float2(0.f, 0.f);
     }
+#pragma unroll
+    for (int k = 0; k < kIL; ++k) tile[warp][k][lane] = v[k];
     __syncwarp();
     if (lane >= cnt) return;
 #pragma unroll 8
