@@ -446,6 +446,41 @@ def test_interleaved_coherent_caller_order_interp_matches_sorted_path():
     ps.destroy()
 
 
+def test_interleaved_tile_fed_interp_matches_the_window_kernel_on_random_plans():
+    """A^H A and the incoherent forward run `interp_il_tile_kernel` (windows fed from shared tiles, tile order, seam tiles,
+    hot tiles cut into work items); `interp_mode = 1` keeps `interp_il_win_kernel` on the block-sorted walk.  Seeded random
+    plans -- grid shapes from 32 to 512 per axis, uniform / radial / one-corner-cell / clustered samples, ragged batches,
+    both coefficient modes -- must agree to rounding; the first of each kind is also compared with the oracle."""
+    import paper_1710_03197_b200 as nb
+    rng = np.random.default_rng(1234)
+    for case in range(12):
+        K0, K1 = int(rng.choice([32, 64, 128, 256, 512])), int(rng.choice([32, 64, 128, 256, 512]))
+        Nd, Kd, Jd = (K0 // 2, K1 // 2), (K0, K1), (6, 6)
+        M, B, kind = int(rng.integers(1, 12000)), int(rng.integers(12, 70)), case % 4
+        if kind == 0:
+            om = wl.traj_uniform(M, 2, seed=case)
+        elif kind == 1:
+            om = wl.traj_radial_golden(max(1, M // 128), 128)
+        elif kind == 2:       # everything in one corner cell: periodic seam on both axes and one hot tile
+            om = np.full((M, 2), -np.pi + 1e-3) + rng.uniform(0, 0.05, size=(M, 2))
+        else:                 # five clusters
+            c = rng.uniform(-np.pi, np.pi, size=(5, 2))
+            om = (c[rng.integers(0, 5, M)] + 0.2 * rng.standard_normal((M, 2)) + np.pi) % (2 * np.pi) - np.pi
+        x = wl.image_gaussian(Nd, batch=B, seed=100 + case)
+        pt = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=B, coef_mode=case % 2)
+        pw = nb.NufftPlan(Nd, Kd, Jd, om, max_batch=B, interp_mode=1)
+        st, sw = host(pt.selfadjoint(dev(x))), host(pw.selfadjoint(dev(x)))
+        ft, fw = host(pt.forward(dev(x))), host(pw.forward(dev(x)))
+        assert maxabs(st, sw) < 5e-6 and maxabs(ft, fw) < 5e-6, (case, Kd, M, B, maxabs(st, sw), maxabs(ft, fw))
+        if case < 4:
+            b = B - 1
+            yo = orc.forward(x[b].astype(np.complex128), om, Nd, Kd, Jd)
+            close(ft[b], yo, Jd)
+            close(st[b], orc.adjoint(yo, om, Nd, Kd, Jd), Jd)
+        pt.destroy()
+        pw.destroy()
+
+
 def test_interleaved_propeller_batch20():
     """The PROPELLER stand-in on the interleaved path (coherent along each readout line, jumps between lines)."""
     check_batched(wl.config_propeller(scale=4), 20, [0, 19])
